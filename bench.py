@@ -1,0 +1,343 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the Lya-forest hot path (S1 gas, S2+S3 tau, S4 normalisation, S5 flux).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--cfg C] [--impl ours|reference]
+
+A step is one pass of the whole hot path over one synthetic grid.  Default workload: BASELINE.json
+configs[1] (256^3, 65,536 sightlines x 256 px, fp32).  `value` = tau pixel-pair evaluations per second
+over the whole step, inputs resident in HBM; `e2e` = the same through lya_forest_host with pinned HOST buffers
+(H2D of delta and v_pec, D2H of F inside the timed region).  N > 1 (torchrun): every rank owns a z-slab of
+256 planes of an N*256-plane grid (weak scaling); the only exchange is S4's all-reduce of two doubles per pass.
+`--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+import torch
+
+from paper_1105_4747_b200 import inputs
+from paper_1105_4747_b200.workloads import WORKLOADS, Workload
+
+METRIC = "tau_pixel_pair_evals_per_s"
+UNIT = "pair-evals/s"
+SM_COUNT_B200, MUFU_PER_CLK_SM = 148, 16          # MUFU.EX2 results / clk / SM
+
+
+def peaks() -> dict:
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            d = json.load(f)
+        return {"hbm_gbs": float(d["hbm_gbs"]), "sm_max_mhz": float(d.get("sm_max_mhz", 1965.0)), "src": "measured"}
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0, "src": "fallback"}
+
+
+# ------------------------------------------------------------------------------------------ clocks
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    REASONS = {0x20: "sw_thermal_slowdown", 0x40: "hw_thermal_slowdown", 0x8: "hw_slowdown",
+               0x4: "sw_power_cap", 0x80: "hw_power_brake"}
+
+    def __init__(self, local_rank: int):
+        super().__init__(daemon=True)
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop_evt, self.active, self.h = threading.Event(), False, None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            idx = local_rank
+            if vis:
+                tok = vis.split(",")[local_rank].strip()
+                idx = int(tok) if tok.isdigit() else local_rank
+            self.nv, self.h = pynvml, pynvml.nvmlDeviceGetHandleByIndex(idx)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+        except Exception:
+            self.h = None
+
+    def run(self):
+        while self.h is not None and not self._stop_evt.is_set():
+            try:
+                mhz = float(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM))
+                bits = int(self.nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h))
+                if self.active:
+                    self.samples.append(mhz)
+                    self.reasons |= {v for k, v in self.REASONS.items() if bits & k}
+            except Exception:
+                pass
+            time.sleep(0.002)
+
+    def stop(self):
+        self._stop_evt.set()
+
+    def summary(self, fallback_max: float) -> dict:
+        return {"sm_mhz": statistics.median(self.samples) if self.samples else None,
+                "sm_max_mhz": self.max_mhz or fallback_max, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+# ------------------------------------------------------------------------------------------ ours
+def bench_ours(args) -> dict:
+    import torch.distributed as dist
+    from paper_1105_4747_b200 import lya
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    torch.cuda.set_device(local)
+    w: Workload = WORKLOADS[args.cfg]
+    n = w.n
+    pk = peaks()
+
+    # inputs: rank r owns planes of its own seeded 256-plane slab (weak scaling: independent slabs of one
+    # N*n-plane grid; complete x-rows, so S1-S3 and S5 need no exchange)
+    wl = w if world == 1 else Workload(**{**w.as_dict(), "axes": tuple(w.axes), "cfg": w.cfg + 100 * rank})
+    fields = inputs.make_fields(wl, device="cuda")
+    delta = fields["delta"]
+    vels = [fields["v_pec"][ax] for ax in w.axes]
+    p = lya.Params.from_workload(w)
+    ctx = lya.Context(local)
+    n_hi, b = torch.empty_like(delta), torch.empty_like(delta)
+    tau, flux = torch.empty_like(delta), torch.empty_like(delta)
+    n_cells = delta.numel()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")       # > 126 MB L2
+
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    results = {}
+
+    def step(timers=None):
+        """S1 once, then S2-S5 per sightline axis (config 3 has three; the others one)."""
+        t = [ev() for _ in range(2 + 3 * len(w.axes))] if timers is not None else None
+        if t: t[0].record()
+        ctx.gas_from_density(p, delta, n_hi, b)
+        if t: t[1].record()
+        for k, ax in enumerate(w.axes):
+            ctx.tau_sightlines(p, ax, n_hi, b, vels[k], tau)
+            if t: t[2 + 3 * k].record()
+            if world == 1:
+                A, f, it, _ = ctx.normalize_mean_flux(tau, w.f_target, rel_tol=1e-7, max_iter=60)
+            else:
+                A, f, it = lya.normalize_mean_flux_sharded(ctx, tau, w.f_target, n_cells * world, rel_tol=1e-7)
+            if t: t[3 + 3 * k].record()
+            ctx.flux(tau, A, flux)
+            if t: t[4 + 3 * k].record()
+            results.update(A=A, f=f, passes=it)
+        if timers is not None:
+            timers.append(t)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+
+    sampler = ClockSampler(local)
+    sampler.start()
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    launches0 = ctx.launch_count
+    timers, step_ev = [], []
+    sampler.active = True
+    wall0 = time.perf_counter()
+    for _ in range(args.steps):
+        flush.zero_()                                   # L2 flush, outside the event-timed span
+        s, e = ev(), ev()
+        s.record()
+        step(timers)
+        e.record()
+        step_ev.append((s, e))
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    wall = time.perf_counter() - wall0
+    sampler.active = False
+    launches = ctx.launch_count - launches0
+
+    step_ms = [s.elapsed_time(e) for s, e in step_ev]
+    total_ms = sum(step_ms)
+    if world > 1:
+        tt = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        total_ms = float(tt.item())
+    ms_per_step = total_ms / args.steps
+    n_ax = len(w.axes)
+    pairs_per_step = float(n) ** 4 * n_ax * world
+    pix_per_step = float(n) ** 3 * n_ax * world
+
+    # per-kernel means (rank 0): gas | tau | normalize | flux
+    k_ms = {"gas": 0.0, "tau": 0.0, "normalize": 0.0, "flux": 0.0}
+    for t in timers:
+        k_ms["gas"] += t[0].elapsed_time(t[1])
+        for k in range(n_ax):
+            prev = t[1] if k == 0 else t[4 + 3 * (k - 1)]
+            k_ms["tau"] += prev.elapsed_time(t[2 + 3 * k])
+            k_ms["normalize"] += t[2 + 3 * k].elapsed_time(t[3 + 3 * k])
+            k_ms["flux"] += t[3 + 3 * k].elapsed_time(t[4 + 3 * k])
+    k_ms["gas"] /= args.steps
+    for k in ("tau", "normalize", "flux"):
+        k_ms[k] /= args.steps * n_ax                    # per launch (per axis pass)
+
+    # ---- end to end through lya_forest_host: pinned host inputs, F read back, every step
+    e2e = None
+    if not args.no_e2e:
+        dh = delta.cpu().pin_memory()
+        vh = [v.cpu().pin_memory() for v in vels]
+        fh = torch.empty_like(dh).pin_memory()
+        for _ in range(2):
+            ctx.forest_host(p, w.axes[0], dh, vh[0], w.f_target, flux_h=fh)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            for k, ax in enumerate(w.axes):
+                ctx.forest_host(p, ax, dh, vh[k], w.f_target, flux_h=fh)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        if world > 1:
+            tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            dt = float(tt.item())
+        e2e = {"value": pairs_per_step * args.steps / dt, "unit": UNIT,
+               "h2d_bytes_per_step": int(2 * 4 * n_cells * n_ax), "d2h_bytes_per_step": int(4 * n_cells * n_ax),
+               "ms_per_step": 1e3 * dt / args.steps,
+               "note": "lya_forest_host: S1 is recomputed per axis pass; multi-rank runs normalise per rank here"}
+    sampler.stop()
+
+    clocks = sampler.summary(pk["sm_max_mhz"])
+    f_peak = MUFU_PER_CLK_SM * ctx.sm_count * pk["sm_max_mhz"] * 1e6          # pair-evals/s at max SM clock
+    tau_rate = float(n) ** 4 / (k_ms["tau"] * 1e-3)
+    hbm = pk["hbm_gbs"]
+    gbs = lambda bytes_, ms: bytes_ / (ms * 1e-3) / 1e9
+    passes = results["passes"]
+    out = {
+        "metric": METRIC, "value": pairs_per_step / (ms_per_step * 1e-3), "unit": UNIT,
+        "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": w.name, "grid": [n, n, n * world], "sightlines": n * n * world * n_ax,
+                   "pixels_per_sightline": n, "axes": list(w.axes), "f_target": w.f_target,
+                   "l2": "256 MiB memset between steps (outside the event spans); working set %d MiB" %
+                         (6 * 4 * n_cells >> 20),
+                   "parallelism": "z-slabs per rank; S4 all-reduce of 2 doubles per pass" if world > 1 else "1 GPU"},
+        "sightline_pixels_per_s": pix_per_step / (ms_per_step * 1e-3),
+        "tau_kernel_pixels_per_s": float(n) ** 3 / (k_ms["tau"] * 1e-3),
+        "A": results["A"], "mean_flux": results["f"], "normalize_passes": passes,
+        "kernel_ms": k_ms, "wall_s_timed_region_incl_flush": wall,
+        "roofline": {"bound": "alu", "kernel": "tau_kernel", "achieved": tau_rate / 1e9, "peak": f_peak / 1e9,
+                     "unit": "Gpair-evals/s", "frac": tau_rate / f_peak, "traffic": None,
+                     "peak_def": "16 MUFU.EX2/clk/SM x %d SMs x %.0f MHz (max SM clock, %s)" %
+                                 (ctx.sm_count, pk["sm_max_mhz"], pk["src"]),
+                     "frac_at_measured_clock": (tau_rate / (MUFU_PER_CLK_SM * ctx.sm_count * clocks["sm_mhz"] * 1e6))
+                     if clocks["sm_mhz"] else None},
+        "roofline_hbm": {
+            "peak_gbs": hbm, "peak_src": pk["src"],
+            "gas": {"bytes": 12 * n_cells, "gbs": gbs(12 * n_cells, k_ms["gas"]), "frac": gbs(12 * n_cells, k_ms["gas"]) / hbm},
+            "normalize": {"bytes": 4 * n_cells * passes, "passes": passes,
+                          "gbs": gbs(4 * n_cells * passes, k_ms["normalize"]),
+                          "frac": gbs(4 * n_cells * passes, k_ms["normalize"]) / hbm},
+            "flux": {"bytes": 8 * n_cells, "gbs": gbs(8 * n_cells, k_ms["flux"]), "frac": gbs(8 * n_cells, k_ms["flux"]) / hbm}},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "sm_count": ctx.sm_count,
+    }
+    if rank == 0 and world == 1 and not args.no_cpu:
+        out["cpu_baseline"] = cpu_baseline(w, delta, vels[0], budget_s=args.cpu_seconds)
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+    return out if rank == 0 else {}
+
+
+# ------------------------------------------------------------------------------------------ oracle legs
+def _oracle_sample(orc, w, d_rows, v_rows):
+    """The oracle's whole path (S1..S5, plain mode: one exp per pair) on a set of sightlines."""
+    po = orc.Params.from_workload(w)
+    _, n_ref, b_ref = orc.gas_from_density(po, d_rows)
+    tau = orc.tau_rows(po, n_ref, b_ref, v_rows, mode=0)
+    A, _, _ = orc.normalize_mean_flux(tau, w.f_target)
+    orc.flux(tau, A)
+    return A
+
+
+def _calibrated_rows(orc, w, d, v, seconds):
+    n = w.n
+    probe = min(64, d.shape[0])
+    t0 = time.perf_counter()
+    _oracle_sample(orc, w, d[:probe], v[:probe])
+    rate = probe / max(time.perf_counter() - t0, 1e-4)                       # sightlines / s
+    return int(max(probe, min(d.shape[0], rate * seconds)))
+
+
+def cpu_baseline(w, delta, v, budget_s=12.0) -> dict:
+    from oracle import lya_oracle as orc
+    n = w.n
+    d = delta.reshape(-1, n).cpu().numpy()
+    vv = v.reshape(-1, n).cpu().numpy()
+    rows = _calibrated_rows(orc, w, d, vv, budget_s)
+    t0 = time.perf_counter()
+    _oracle_sample(orc, w, d[:rows], vv[:rows])
+    dt = time.perf_counter() - t0
+    return {"value": rows * float(n) ** 2 / dt, "unit": UNIT, "cores": orc.threads(), "kind": "oracle",
+            "sample": f"first {rows} of {d.shape[0]} sightlines of {w.name}, whole path S1..S5 in double, "
+                      f"plain mode, {dt:.1f} s"}
+
+
+def bench_reference(args) -> dict:
+    if int(os.environ.get("RANK", "0")) != 0:
+        return {}
+    from oracle import lya_oracle as orc
+    w = WORKLOADS[args.cfg]
+    n = w.n
+    # the same seeded fields as our arm, only the planes the sample needs (generated on the CPU)
+    nz_need = 8
+    f = inputs.make_fields(w, device="cpu", z0=0, z1=nz_need)
+    d = f["delta"].reshape(-1, n).numpy()
+    v = f["v_pec"][w.axes[0]].reshape(-1, n).numpy()
+    rows = _calibrated_rows(orc, w, d, v, seconds=1.5)
+    for _ in range(min(args.warmup, 1)):
+        _oracle_sample(orc, w, d[:rows], v[:rows])
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        _oracle_sample(orc, w, d[:rows], v[:rows])
+    dt = time.perf_counter() - t0
+    val = rows * float(n) ** 2 * args.steps / dt
+    sample = f"{rows} sightlines (first planes) of {w.name} per step, whole path S1..S5 in double, plain mode"
+    return {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": w.name, "sample": sample},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": orc.threads(), "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--cfg", type=int, default=2, choices=[1, 2, 3, 4])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    args = ap.parse_args()
+    out = bench_reference(args) if args.impl == "reference" else bench_ours(args)
+    if out:
+        print(json.dumps(out))
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,152 @@
+/* lya.h -- C ABI of the B200 (sm_100a) Lyman-alpha forest hot path of arXiv:1105.4747
+ * (Greig, Bolton & Wyithe), section 2.3, PAPER.md:70-92:
+ *
+ *   S1  gas state        T = T0 (1+delta)^(gamma-1) with the pivot at 1+delta = 10   Eq.5
+ *                        n_HI from photo-ionisation equilibrium                     Eq.4
+ *                        b = sqrt(2 k_B T / m_p)
+ *   S2  u(j) = v_H(j) + v_pec(j)
+ *   S3  tau(i) = c sigma_a dR / sqrt(pi) * sum_j n_HI(j)/b(j) exp(-((v_H(i)-u(j))/b(j))^2)   Eq.6
+ *       (periodic in velocity: nearest image, reading C7)
+ *   S4  A with <exp(-A tau)> = observed mean flux, over all pixels of all spectra
+ *   S5  F = exp(-A tau)
+ *
+ * Every entry point is extern "C", takes plain pointers and sizes, returns a status code and never
+ * throws, exits or prints.  Pointers are marked DEVICE (CUDA global memory of ctx's device, owned by
+ * the caller, fp32, 4-byte aligned at least; 16-byte alignment enables the vector / bulk-copy paths)
+ * or HOST.  The library never retains or frees a caller pointer; its only allocations are private
+ * scratch inside lya_ctx.  There is no CPU fallback: without a CUDA device lya_create fails with
+ * LYA_ECUDA and nothing else can be called.
+ *
+ * Grid layout everywhere: C order [iz][iy][ix], ix contiguous.  axis 0 = sightlines along x
+ * (contiguous rows), 1 = along y (stride nx), 2 = along z (stride nx*ny).
+ */
+#ifndef LYA_H
+#define LYA_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LYA_VERSION 100   /* 0.1.0 */
+
+typedef struct lya_ctx lya_ctx;   /* opaque: device, stream, SM count, reduction scratch, workspace */
+
+typedef enum {
+    LYA_OK      = 0,
+    LYA_EINVAL  = 1,   /* null / misaligned pointer, n < 1, bad axis, T0 <= 0, f_target outside (0,1), aliasing ... */
+    LYA_ECUDA   = 2,   /* a CUDA runtime call failed; text via lya_last_error()                                      */
+    LYA_ENOROOT = 3,   /* no A > 0 solves <exp(-A tau)> = f_target (e.g. all tau == 0)                               */
+    LYA_ENOCONV = 4,   /* max_iter reached; *a_out holds the best estimate                                           */
+    LYA_ENOMEM  = 5    /* device or pinned-host allocation failed                                                    */
+} lya_status;
+
+/* The paper's free parameters. All host-side doubles. */
+typedef struct {
+    int32_t nx, ny, nz;     /* full grid                                                                   */
+    double  box_mpch;       /* comoving box length ALONG THE SIGHTLINE AXIS [h^-1 Mpc]                      */
+    double  z;              /* redshift                                                                    */
+    double  omega_m, h;     /* flat LCDM: omega_lambda = 1 - omega_m, radiation neglected                  */
+    double  omega_b_h2;     /* Eq.4; its pivot value is 0.024                                              */
+    double  gamma_m12;      /* HI photo-ionisation rate / 1e-12 s^-1, Eq.4 (degenerate with A) */
+    double  y_he;           /* helium mass fraction in nbar_H = (1-Y) rho_b / m_H (reading C9)             */
+    double  T0, gamma;      /* Eq.5                                                                        */
+    double  delta_pivot;    /* Eq.5 pivot in 1+delta (paper: 10); <= 0 disables it                         */
+} lya_params;
+
+/* Derived scalars of one sightline direction (host double precision). */
+typedef struct {
+    int32_t n_pix;          /* pixels along the axis                                  */
+    double  Ez, Hz;         /* E(z); H(z) [km/s/Mpc]                                  */
+    double  dR_cm;          /* proper pixel width                        */
+    double  dv_kms;         /* Hubble velocity width of one pixel = H(z) dR           */
+    double  V_kms;          /* n_pix * dv: period of the velocity axis                */
+    double  b0_kms;         /* sqrt(2 k_B T0 / m_p)                                   */
+    double  nbarH, nbarHI;  /* mean proper H density; Eq.4 at delta = 0  [cm^-3]      */
+    double  K;              /* c sigma_alpha dR / sqrt(pi), Eq.6 prefactor [cm^4/s]   */
+    double  tau0;           /* K nbarHI / b0: line-centre amplitude at mean density   */
+    double  tauGP;          /* c sigma_alpha nbarHI / H(z): Gunn-Peterson depth       */
+} lya_scalars;
+
+/* Host only, no GPU needed. LYA_EINVAL on null pointers, axis not in {0,1,2}, n < 1, box/h/T0/gamma_m12 <= 0. */
+lya_status lya_scalars_from_params(const lya_params *p, int axis, lya_scalars *out);
+
+int         lya_version(void);
+const char *lya_status_string(lya_status s);
+
+/* device: CUDA ordinal.  cuda_stream: a cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream) or
+ * NULL for the legacy default stream; every kernel below is enqueued on it.  One ctx per host thread. */
+lya_status  lya_create(lya_ctx **out, int device, void *cuda_stream);
+void        lya_destroy(lya_ctx *ctx);
+const char *lya_last_error(const lya_ctx *ctx);          /* "" if none; valid until the next call on ctx */
+int         lya_sm_count(const lya_ctx *ctx);
+
+/* S1 (Eq.4, Eq.5 + pivot, b).  delta, n_hi, b_kms: DEVICE, n_cells floats each; outputs may not alias
+ * the input.  n_hi in cm^-3, b in km/s.  Precondition (not scanned): 1 + delta > 0 and finite.
+ * Asynchronous on ctx's stream. */
+lya_status lya_gas_from_density(lya_ctx *ctx, const lya_params *p, const float *delta, size_t n_cells,
+                                float *n_hi, float *b_kms);
+
+/* S2 + S3 (Eq.6, full periodic sum: every (i,j) pair of a sightline is evaluated).
+ * All four arrays: DEVICE, [nz_local][ny][nx] floats (nz_local == nz for a whole grid; a z-slab of
+ * complete rows otherwise; axis == 2 requires nz_local == nz).  v_pec_kms is the proper peculiar velocity
+ * component ALONG `axis` in km/s; positive values move absorption to higher pixel index.  tau may not alias
+ * an input.  Asynchronous on ctx's stream. */
+lya_status lya_tau_sightlines(lya_ctx *ctx, const lya_params *p, int axis, int32_t nz_local,
+                              const float *n_hi, const float *b_kms, const float *v_pec_kms, float *tau);
+
+/* S4.  tau: DEVICE, n_pix floats in any layout (the mean runs over all of them).  Finds the unique A > 0
+ * with mean(exp(-A tau)) = f_target by a bracketed Newton/bisection iteration that runs entirely on the
+ * device (one cooperative kernel); synchronises the stream because A returns to the HOST.
+ * rel_tol: stop when the step or the bracket is below rel_tol * A (suggest 1e-7); max_iter passes over tau
+ * (suggest 60).  a_out, f_achieved, iters: HOST, any may be NULL. */
+lya_status lya_normalize_mean_flux(lya_ctx *ctx, const float *tau, size_t n_pix, double f_target,
+                                   double rel_tol, int max_iter,
+                                   double *a_out, double *f_achieved, int *iters);
+
+/* Building block of S4 for slab-wise or multi-GPU normalisation: for k trial values (1 <= k <= 8) returns
+ * sums[t] = sum_p exp(-a_trial[t] tau_p) and, if dsums != NULL, dsums[t] = sum_p tau_p exp(-a_trial[t] tau_p).
+ * tau DEVICE; a_trial, sums, dsums HOST.  Synchronises the stream. */
+lya_status lya_flux_partial_sums(lya_ctx *ctx, const float *tau, size_t n_pix,
+                                 const double *a_trial, int k, double *sums, double *dsums);
+
+/* Host-side root iteration shared by lya_normalize_mean_flux's device loop (restated there) and by
+ * callers that own the reduction (slabs, ranks): feed the GLOBAL sums of the current trial, get the next.
+ * No GPU needed. */
+typedef struct {
+    double f_target, rel_tol;
+    double n_pix;           /* global pixel count                                        */
+    double lo, hi;          /* bracket: f(lo) > f_target >= f(hi); hi < 0 means unknown   */
+    double a;               /* current trial                                             */
+    double f_at_a;          /* mean flux at the last evaluated trial                     */
+    int32_t iters;          /* passes consumed                                           */
+    int32_t done;           /* 1 converged (a is final and f_at_a was evaluated AT a)    */
+    int32_t status;         /* lya_status                                                */
+    int32_t finishing;      /* internal: the next update only records f at the final a   */
+} lya_root_state;
+lya_status lya_root_init(lya_root_state *s, double f_target, double rel_tol, double n_pix_global);
+lya_status lya_root_update(lya_root_state *s, double sum_exp, double sum_tau_exp);
+
+/* S5.  tau, flux: DEVICE, n_pix floats; flux == tau (in place) allowed.  Asynchronous. */
+lya_status lya_flux(lya_ctx *ctx, const float *tau, size_t n_pix, double a, float *flux);
+
+/* End-to-end S1..S5 from HOST buffers (the call bench.py's e2e number times).  delta_h, v_pec_h: HOST
+ * [nz][ny][nx] floats (pinned memory makes the copies asynchronous).  The grid is processed in z-slabs of
+ * slab_nz planes (0 = choose; axis 2 forces one slab): H2D copy of slab s+1 overlaps S1+S3 of slab s on a
+ * second stream; tau stays resident on the device for S4; S5 then streams F back.  tau_h, flux_h: HOST
+ * outputs, either may be NULL.  Device workspace is cached in ctx and freed by lya_destroy. */
+lya_status lya_forest_host(lya_ctx *ctx, const lya_params *p, int axis, int32_t slab_nz,
+                           const float *delta_h, const float *v_pec_h, double f_target,
+                           double rel_tol, int max_iter,
+                           float *tau_h, float *flux_h,
+                           double *a_out, double *f_achieved, int *iters);
+
+/* Number of kernels the library has launched on this ctx since creation (bench.py's gpu_launches). */
+uint64_t lya_launch_count(const lya_ctx *ctx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LYA_H */

@@ -1,0 +1,79 @@
+// gas.cu -- S1: gas state per cell (Eq.4, Eq.5 with pivot, Doppler parameter).
+//
+//   D   = 1 + delta                      Dt = min(D, pivot)
+//   T   = T0 Dt^(gamma-1)                                              (Eq.5)
+//   b   = sqrt(2 kB T / m_p) = b0 Dt^((gamma-1)/2)
+//   nHI = nbarHI (T/T0)^-0.7 D^2 = nbarHI Dt^(-1.4 (gamma-1)/2) D^2    (Eq.4 with the local T: reading C4)
+//
+// HBM-bound: 4 B read + 8 B written per cell.  One lg2 and two ex2 per cell; 128-bit loads/stores,
+// grid-stride over a grid that is a multiple of the SM count.
+#include "lya_internal.h"
+
+namespace {
+
+struct GasK {
+    float nbar_hi;   // Eq.4 at delta = 0, T = T0 [cm^-3]
+    float b0;        // km/s
+    float h;         // (gamma-1)/2
+    float e_n;       // -0.7 (gamma-1)
+    float pivot;     // +inf when disabled
+};
+
+__device__ __forceinline__ void gas_cell(const GasK &k, float delta, float &n_hi, float &b)
+{
+    float D  = 1.0f + delta;
+    float Dt = fminf(D, k.pivot);
+    float l  = log2f(Dt);                       // full-precision log2 (kernel stays HBM-bound)
+    b    = k.b0 * exp2f(k.h * l);
+    n_hi = (k.nbar_hi * exp2f(k.e_n * l)) * (D * D);
+}
+
+__global__ void __launch_bounds__(256) gas_vec4_kernel(const float4 *__restrict__ delta, size_t n4,
+                                                       float4 *__restrict__ n_hi, float4 *__restrict__ b,
+                                                       GasK k)
+{
+    size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += stride) {
+        float4 d = __ldcs(delta + i);           // streamed once
+        float4 n, w;
+        gas_cell(k, d.x, n.x, w.x);
+        gas_cell(k, d.y, n.y, w.y);
+        gas_cell(k, d.z, n.z, w.z);
+        gas_cell(k, d.w, n.w, w.w);
+        n_hi[i] = n;
+        b[i]    = w;
+    }
+}
+
+__global__ void __launch_bounds__(256) gas_scalar_kernel(const float *__restrict__ delta, size_t i0, size_t n,
+                                                         float *__restrict__ n_hi, float *__restrict__ b, GasK k)
+{
+    size_t stride = (size_t)gridDim.x * blockDim.x;
+    for (size_t i = i0 + (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += stride)
+        gas_cell(k, delta[i], n_hi[i], b[i]);
+}
+
+}  // namespace
+
+lya_status lya_launch_gas(lya_ctx *ctx, const float *delta, size_t n, float *n_hi, float *b,
+                          float nbar_hi, float b0, float half_gm1, float pivot)
+{
+    GasK k{nbar_hi, b0, half_gm1, (float)(2.0 * LYA_ALPHA_T) * half_gm1, pivot};
+    bool aligned = (((uintptr_t)delta | (uintptr_t)n_hi | (uintptr_t)b) & 15) == 0;
+    size_t n4 = aligned ? n / 4 : 0;
+    if (n4) {
+        size_t want = (n4 + 255) / 256;
+        int grid = (int)(want < (size_t)ctx->sm_count * 8 ? want : (size_t)ctx->sm_count * 8);
+        gas_vec4_kernel<<<grid, 256, 0, ctx->stream>>>((const float4 *)delta, n4, (float4 *)n_hi, (float4 *)b, k);
+        ctx->launches++;
+    }
+    if (n4 * 4 < n) {
+        size_t rem = n - n4 * 4;
+        size_t want = (rem + 255) / 256;
+        int grid = (int)(want < (size_t)ctx->sm_count * 8 ? want : (size_t)ctx->sm_count * 8);
+        gas_scalar_kernel<<<grid, 256, 0, ctx->stream>>>(delta, n4 * 4, n, n_hi, b, k);
+        ctx->launches++;
+    }
+    LYA_CUDA(ctx, cudaGetLastError());
+    return LYA_OK;
+}

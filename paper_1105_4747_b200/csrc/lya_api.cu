@@ -1,0 +1,221 @@
+// lya_api.cu -- host side of the C ABI declared in include/lya.h: context, argument validation, the
+// double-precision scalars of DESIGN.md "Notation", and the kernel launch wrappers.  No CPU fallback.
+#include <math.h>
+#include <new>
+
+#include "lya_internal.h"
+#include "root_iter.h"
+
+namespace {
+
+int axis_len(const lya_params *p, int axis) { return axis == 0 ? p->nx : (axis == 1 ? p->ny : p->nz); }
+
+bool params_ok(const lya_params *p)
+{
+    return p && p->nx >= 1 && p->ny >= 1 && p->nz >= 1 && p->box_mpch > 0 && p->h > 0 && p->T0 > 0 &&
+           p->gamma_m12 > 0 && p->omega_b_h2 > 0 && p->z > -1.0 && isfinite(p->gamma) && p->y_he < 1.0 &&
+           p->omega_m >= 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+int lya_version(void) { return LYA_VERSION; }
+
+const char *lya_status_string(lya_status s)
+{
+    switch (s) {
+        case LYA_OK:      return "ok";
+        case LYA_EINVAL:  return "invalid argument";
+        case LYA_ECUDA:   return "CUDA error";
+        case LYA_ENOROOT: return "no root";
+        case LYA_ENOCONV: return "not converged";
+        case LYA_ENOMEM:  return "out of memory";
+    }
+    return "unknown";
+}
+
+// Scalars of Eq.4 / Eq.6, all in double on the host.
+lya_status lya_scalars_from_params(const lya_params *p, int axis, lya_scalars *s)
+{
+    if (!s || !params_ok(p) || axis < 0 || axis > 2) return LYA_EINVAL;
+    const int n = axis_len(p, axis);
+    const double zp1 = 1.0 + p->z;
+    s->n_pix  = n;
+    s->Ez     = sqrt(p->omega_m * zp1 * zp1 * zp1 + (1.0 - p->omega_m));
+    s->Hz     = 100.0 * p->h * s->Ez;
+    const double dR_mpc = p->box_mpch / ((double)n * p->h * zp1);           // proper pixel width [Mpc]
+    s->dR_cm  = dR_mpc * LYA_CM_PER_MPC;
+    s->dv_kms = s->Hz * dR_mpc;
+    s->V_kms  = s->dv_kms * (double)n;
+    s->b0_kms = sqrt(2.0 * LYA_K_BOLTZ * p->T0 / LYA_M_PROTON) * 1.0e-5;
+    s->nbarH  = (1.0 - p->y_he) * p->omega_b_h2 * LYA_RHOCRIT100 * (zp1 * zp1 * zp1) / LYA_M_HATOM;
+    s->nbarHI = LYA_NHI_COEFF * s->nbarH * pow(p->T0 * 1.0e-4, LYA_ALPHA_T) * (p->omega_b_h2 / 0.024) /
+                p->gamma_m12 * pow(zp1 * 0.25, 3.0);                        // Eq.4 at delta = 0
+    s->K      = LYA_C_CGS * LYA_SIGMA_LYA * s->dR_cm / sqrt(M_PI);          // Eq.6 prefactor
+    s->tau0   = s->K * s->nbarHI / (s->b0_kms * 1.0e5);
+    s->tauGP  = LYA_C_CGS * LYA_SIGMA_LYA * s->nbarHI / (s->Hz * 1.0e5 / LYA_CM_PER_MPC);
+    return LYA_OK;
+}
+
+lya_status lya_create(lya_ctx **out, int device, void *cuda_stream)
+{
+    if (!out) return LYA_EINVAL;
+    *out = nullptr;
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || device < 0 || device >= n_dev) {
+        cudaGetLastError();
+        return LYA_ECUDA;                                   // no device: there is no fallback path
+    }
+    lya_ctx *ctx = new (std::nothrow) lya_ctx();
+    if (!ctx) return LYA_ENOMEM;
+    memset(ctx, 0, sizeof(*ctx));
+    ctx->device = device;
+    ctx->stream = (cudaStream_t)cuda_stream;
+    cudaError_t e = cudaSetDevice(device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->coop_ok, cudaDevAttrCooperativeLaunch, device);
+    const size_t part_bytes = (size_t)2 * LYA_MAX_RED_BLOCKS * 2 * LYA_MAX_TRIALS * sizeof(double);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->d_partials, part_bytes);
+    if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->d_root, 64 * sizeof(double));
+    if (e == cudaSuccess) e = cudaMallocHost((void **)&ctx->h_pinned, 64 * sizeof(double));
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking);
+    for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
+        e = cudaEventCreateWithFlags(&ctx->ev_copy[i], cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->ev_comp[i], cudaEventDisableTiming);
+    }
+    if (e != cudaSuccess) {
+        lya_destroy(ctx);
+        return e == cudaErrorMemoryAllocation ? LYA_ENOMEM : LYA_ECUDA;
+    }
+    *out = ctx;
+    return LYA_OK;
+}
+
+void lya_destroy(lya_ctx *ctx)
+{
+    if (!ctx) return;
+    cudaSetDevice(ctx->device);
+    if (ctx->ws) cudaFree(ctx->ws);
+    if (ctx->d_partials) cudaFree(ctx->d_partials);
+    if (ctx->d_root) cudaFree(ctx->d_root);
+    if (ctx->h_pinned) cudaFreeHost(ctx->h_pinned);
+    for (int i = 0; i < 2; ++i) {
+        if (ctx->ev_copy[i]) cudaEventDestroy(ctx->ev_copy[i]);
+        if (ctx->ev_comp[i]) cudaEventDestroy(ctx->ev_comp[i]);
+    }
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+    delete ctx;
+}
+
+const char *lya_last_error(const lya_ctx *ctx) { return ctx ? ctx->err : "null context"; }
+int lya_sm_count(const lya_ctx *ctx) { return ctx ? ctx->sm_count : 0; }
+uint64_t lya_launch_count(const lya_ctx *ctx) { return ctx ? ctx->launches : 0; }
+
+lya_status lya_gas_from_density(lya_ctx *ctx, const lya_params *p, const float *delta, size_t n_cells,
+                                float *n_hi, float *b_kms)
+{
+    if (!ctx) return LYA_EINVAL;
+    ctx->err[0] = 0;
+    if (!params_ok(p)) return lya_fail(ctx, LYA_EINVAL, "lya_gas_from_density: bad parameters");
+    if (!delta || !n_hi || !b_kms) return lya_fail(ctx, LYA_EINVAL, "lya_gas_from_density: null pointer");
+    if ((((uintptr_t)delta | (uintptr_t)n_hi | (uintptr_t)b_kms) & 3) != 0)
+        return lya_fail(ctx, LYA_EINVAL, "lya_gas_from_density: pointers must be 4-byte aligned");
+    if (n_hi == delta || b_kms == delta || n_hi == b_kms)
+        return lya_fail(ctx, LYA_EINVAL, "lya_gas_from_density: outputs may not alias");
+    if (n_cells == 0) return LYA_OK;
+    lya_scalars s;
+    lya_scalars_from_params(p, 0, &s);          // nbarHI and b0 do not depend on the axis
+    LYA_CUDA(ctx, cudaSetDevice(ctx->device));
+    const float pivot = p->delta_pivot > 0.0 ? (float)p->delta_pivot : INFINITY;
+    return lya_launch_gas(ctx, delta, n_cells, n_hi, b_kms, (float)s.nbarHI, (float)s.b0_kms,
+                          (float)(0.5 * (p->gamma - 1.0)), pivot);
+}
+
+lya_status lya_tau_sightlines(lya_ctx *ctx, const lya_params *p, int axis, int32_t nz_local,
+                              const float *n_hi, const float *b_kms, const float *v_pec_kms, float *tau)
+{
+    if (!ctx) return LYA_EINVAL;
+    ctx->err[0] = 0;
+    if (!params_ok(p)) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: bad parameters");
+    if (axis < 0 || axis > 2) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: axis must be 0, 1 or 2");
+    if (nz_local < 1 || nz_local > p->nz) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: bad nz_local");
+    if (axis == 2 && nz_local != p->nz)
+        return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: axis 2 needs the whole grid (nz_local == nz)");
+    if (!n_hi || !b_kms || !v_pec_kms || !tau) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: null pointer");
+    if ((((uintptr_t)n_hi | (uintptr_t)b_kms | (uintptr_t)v_pec_kms | (uintptr_t)tau) & 3) != 0)
+        return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: pointers must be 4-byte aligned");
+    if (tau == n_hi || tau == b_kms || tau == v_pec_kms)
+        return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: tau may not alias an input");
+    if (axis_len(p, axis) > (1 << 22))
+        return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: more than 2^22 pixels per sightline");
+    lya_scalars s;
+    lya_scalars_from_params(p, axis, &s);
+    LYA_CUDA(ctx, cudaSetDevice(ctx->device));
+    // amplitude a_j = K nHI / (b[km/s] 1e5 cm/km): K 1e-5 is passed so that fp32 operands stay O(1e11 x 1e-11)
+    return lya_launch_tau(ctx, axis, p->nx, p->ny, nz_local, n_hi, b_kms, v_pec_kms, tau, s.K * 1.0e-5, s.dv_kms);
+}
+
+lya_status lya_normalize_mean_flux(lya_ctx *ctx, const float *tau, size_t n_pix, double f_target,
+                                   double rel_tol, int max_iter, double *a_out, double *f_achieved, int *iters)
+{
+    if (!ctx) return LYA_EINVAL;
+    ctx->err[0] = 0;
+    if (!tau || ((uintptr_t)tau & 3)) return lya_fail(ctx, LYA_EINVAL, "lya_normalize_mean_flux: bad tau pointer");
+    if (n_pix == 0) return lya_fail(ctx, LYA_EINVAL, "lya_normalize_mean_flux: n_pix == 0");
+    if (!(f_target > 0.0 && f_target < 1.0))
+        return lya_fail(ctx, LYA_EINVAL, "lya_normalize_mean_flux: f_target must lie in (0,1)");
+    if (!(rel_tol > 0.0) || max_iter < 2)
+        return lya_fail(ctx, LYA_EINVAL, "lya_normalize_mean_flux: rel_tol > 0 and max_iter >= 2 required");
+    LYA_CUDA(ctx, cudaSetDevice(ctx->device));
+    return lya_run_normalize(ctx, tau, n_pix, f_target, rel_tol, max_iter, a_out, f_achieved, iters);
+}
+
+lya_status lya_flux_partial_sums(lya_ctx *ctx, const float *tau, size_t n_pix, const double *a_trial, int k,
+                                 double *sums, double *dsums)
+{
+    if (!ctx) return LYA_EINVAL;
+    ctx->err[0] = 0;
+    if (!tau || ((uintptr_t)tau & 3) || !a_trial || !sums)
+        return lya_fail(ctx, LYA_EINVAL, "lya_flux_partial_sums: null or misaligned pointer");
+    if (k < 1 || k > LYA_MAX_TRIALS) return lya_fail(ctx, LYA_EINVAL, "lya_flux_partial_sums: k must be 1..8");
+    for (int i = 0; i < k; ++i)
+        if (!(a_trial[i] >= 0.0) || !(a_trial[i] < 1.0e30))
+            return lya_fail(ctx, LYA_EINVAL, "lya_flux_partial_sums: trial A must be finite and >= 0");
+    if (n_pix == 0) {
+        for (int i = 0; i < k; ++i) { sums[i] = 0.0; if (dsums) dsums[i] = 0.0; }
+        return LYA_OK;
+    }
+    LYA_CUDA(ctx, cudaSetDevice(ctx->device));
+    return lya_run_partial_sums(ctx, tau, n_pix, a_trial, k, sums, dsums);
+}
+
+lya_status lya_root_init(lya_root_state *s, double f_target, double rel_tol, double n_pix_global)
+{
+    if (!s || !(f_target > 0.0 && f_target < 1.0) || !(rel_tol > 0.0) || !(n_pix_global >= 1.0)) return LYA_EINVAL;
+    lya_root_reset(s, f_target, rel_tol, n_pix_global);
+    return LYA_OK;
+}
+
+lya_status lya_root_update(lya_root_state *s, double sum_exp, double sum_tau_exp)
+{
+    if (!s || s->done) return LYA_EINVAL;
+    lya_root_step(s, sum_exp, sum_tau_exp);
+    return (lya_status)s->status;
+}
+
+lya_status lya_flux(lya_ctx *ctx, const float *tau, size_t n_pix, double a, float *flux)
+{
+    if (!ctx) return LYA_EINVAL;
+    ctx->err[0] = 0;
+    if (!tau || !flux || (((uintptr_t)tau | (uintptr_t)flux) & 3))
+        return lya_fail(ctx, LYA_EINVAL, "lya_flux: null or misaligned pointer");
+    if (!(a >= 0.0) || !(a < 1.0e30)) return lya_fail(ctx, LYA_EINVAL, "lya_flux: A must be finite and >= 0");
+    if (n_pix == 0) return LYA_OK;
+    LYA_CUDA(ctx, cudaSetDevice(ctx->device));
+    return lya_launch_flux(ctx, tau, n_pix, a, flux);
+}
+
+}  // extern "C"

@@ -1,0 +1,74 @@
+// lya_internal.h -- private to the CUDA library (never included by oracle/ or tests).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string.h>
+
+#include "../../include/lya.h"
+
+struct lya_ctx {
+    int           device;
+    cudaStream_t  stream;         // caller's stream: every kernel goes here
+    cudaStream_t  copy_stream;    // lya_forest_host: H2D/D2H overlap
+    cudaEvent_t   ev_copy[2], ev_comp[2];
+    int           sm_count;
+    int           max_smem_optin; // bytes per block
+    int           coop_ok;        // cooperative launch supported
+    uint64_t      launches;
+    // reduction scratch (device): per-block partial sums, root state
+    double       *d_partials;     // [2 parities][LYA_MAX_RED_BLOCKS][2*LYA_MAX_TRIALS]
+    double       *d_root;         // device copy of the root-iteration result (see normalize.cu)
+    double       *h_pinned;       // small pinned host mirror
+    // lya_forest_host workspace (device), grown on demand
+    void         *ws;
+    size_t        ws_bytes;
+    char          err[512];
+};
+
+#define LYA_MAX_RED_BLOCKS 2048
+#define LYA_MAX_TRIALS     8
+
+static inline lya_status lya_fail(lya_ctx *ctx, lya_status s, const char *msg)
+{
+    if (ctx) {
+        strncpy(ctx->err, msg, sizeof(ctx->err) - 1);
+        ctx->err[sizeof(ctx->err) - 1] = 0;
+    }
+    return s;
+}
+
+static inline lya_status lya_cuda_fail(lya_ctx *ctx, cudaError_t e, const char *where)
+{
+    if (ctx) snprintf(ctx->err, sizeof(ctx->err), "%s: %s", where, cudaGetErrorString(e));
+    return e == cudaErrorMemoryAllocation ? LYA_ENOMEM : LYA_ECUDA;
+}
+
+#define LYA_CUDA(ctx, call)                                              \
+    do {                                                                 \
+        cudaError_t e__ = (call);                                        \
+        if (e__ != cudaSuccess) return lya_cuda_fail((ctx), e__, #call); \
+    } while (0)
+
+// Physical constants (cgs, CODATA 2018 / IAU 2015), typed in here independently of oracle/.
+#define LYA_K_BOLTZ    1.380649e-16           // erg/K
+#define LYA_M_PROTON   1.67262192369e-24      // g   (b uses m_p: DESIGN.md reading C6)
+#define LYA_M_HATOM    1.6735575e-24          // g   (nbar_H)
+#define LYA_CM_PER_MPC 3.0856775814913673e24
+#define LYA_C_CGS      2.99792458e10          // cm/s
+#define LYA_SIGMA_LYA  4.48e-18               // cm^2
+#define LYA_RHOCRIT100 1.87834e-29            // g/cm^3 for h = 1
+#define LYA_NHI_COEFF  7.24e-6                // Eq.4
+#define LYA_ALPHA_T    (-0.7)                 // recombination-rate temperature slope
+
+// kernels' host launchers (each enqueues on ctx->stream and bumps ctx->launches)
+lya_status lya_launch_gas(lya_ctx *ctx, const float *delta, size_t n, float *n_hi, float *b,
+                          float nbar_hi, float b0, float half_gm1, float pivot);
+lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
+                          const float *n_hi, const float *b, const float *v, float *tau,
+                          double amp_scale, double dv_kms);
+lya_status lya_launch_flux(lya_ctx *ctx, const float *tau, size_t n, double a, float *flux);
+lya_status lya_run_normalize(lya_ctx *ctx, const float *tau, size_t n, double f_target, double rel_tol,
+                             int max_iter, double *a_out, double *f_out, int *iters);
+lya_status lya_run_partial_sums(lya_ctx *ctx, const float *tau, size_t n, const double *a_trial, int k,
+                                double *sums, double *dsums);

@@ -1,0 +1,292 @@
+// normalize.cu -- S4 and S5: mean-flux normalisation constant A and F = exp(-A tau).
+//
+// S4: one cooperative, persistent kernel runs the whole iteration on the device.  Each pass streams tau once
+// (4 B / pixel, 128-bit loads), evaluates e = ex2(-A log2(e) tau) on the MUFU pipe and reduces both
+// sum(e) and sum(tau e) -- fp32 only inside one float4, double from the thread level up, warp shuffles, then
+// one partial pair per block.  After a grid-wide barrier EVERY block reduces the same partials in the same
+// order and applies the same scalar update (root_iter.h), so no second barrier or broadcast is needed and the
+// result is bit-reproducible.  The host sees only the final (A, <F>, passes, status).
+//
+// A log2(e) is split into an fp32 hi/lo pair so that f(A) is not quantised at 6e-8 in A.
+#include <cooperative_groups.h>
+
+#include "lya_internal.h"
+#include "root_iter.h"
+
+namespace cg = cooperative_groups;
+
+namespace {
+
+constexpr int RED_THREADS = 256;
+constexpr double LOG2E_D  = 1.4426950408889634074;
+
+__device__ __forceinline__ float ex2_ftz(float x)
+{
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+struct Trial { float c_hi, c_lo; };        // -A log2(e) = c_hi + c_lo
+
+__host__ __device__ inline Trial make_trial(double a)
+{
+    double c = -a * LOG2E_D;
+    Trial t;
+    t.c_hi = (float)c;
+    t.c_lo = (float)(c - (double)t.c_hi);
+    return t;
+}
+
+__device__ __forceinline__ float flux_of(float tau, const Trial &t)
+{
+    return ex2_ftz(fmaf(tau, t.c_hi, tau * t.c_lo));
+}
+
+// sum over this thread's share of tau of (e, tau e) for K trials; grid-stride float4 body + scalar edges.
+template <int K>
+__device__ __forceinline__ void accumulate(const float *__restrict__ tau, size_t n, const Trial (&tr)[K],
+                                           double (&s0)[K], double (&s1)[K])
+{
+#pragma unroll
+    for (int k = 0; k < K; ++k) { s0[k] = 0.0; s1[k] = 0.0; }
+    const size_t gtid = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t gsz  = (size_t)gridDim.x * blockDim.x;
+    size_t head = ((16 - ((uintptr_t)tau & 15)) & 15) >> 2;      // scalars before 16-byte alignment
+    if (head > n) head = n;
+    const size_t n4 = (n - head) >> 2;
+    const float4 *t4 = reinterpret_cast<const float4 *>(tau + head);
+#pragma unroll 2
+    for (size_t i = gtid; i < n4; i += gsz) {
+        const float4 t = __ldg(t4 + i);              // re-read every pass: let L2 keep what fits
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            float e0 = flux_of(t.x, tr[k]), e1 = flux_of(t.y, tr[k]);
+            float e2 = flux_of(t.z, tr[k]), e3 = flux_of(t.w, tr[k]);
+            s0[k] += (double)((e0 + e1) + (e2 + e3));
+            s1[k] += (double)(fmaf(t.x, e0, t.y * e1) + fmaf(t.z, e2, t.w * e3));
+        }
+    }
+    // edges: head scalars and the < 4 tail scalars
+    const size_t tail0 = head + (n4 << 2);
+    const size_t n_edge = head + (n - tail0);
+    for (size_t e = gtid; e < n_edge; e += gsz) {
+        const size_t i = e < head ? e : tail0 + (e - head);
+        const float t = tau[i];
+#pragma unroll
+        for (int k = 0; k < K; ++k) {
+            float ex = flux_of(t, tr[k]);
+            s0[k] += (double)ex;
+            s1[k] += (double)(t * ex);
+        }
+    }
+}
+
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// block-wide sum of NV doubles per thread; result valid in every thread of warp 0 (and written by thread 0)
+template <int NV>
+__device__ __forceinline__ void block_sum(double (&v)[NV], double *sh /* [NV][warps] */)
+{
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = blockDim.x >> 5;
+#pragma unroll
+    for (int k = 0; k < NV; ++k) {
+        v[k] = warp_sum(v[k]);
+        if (lane == 0) sh[k * 32 + warp] = v[k];
+    }
+    __syncthreads();
+    if (warp == 0) {
+#pragma unroll
+        for (int k = 0; k < NV; ++k) {
+            double x = lane < nw ? sh[k * 32 + lane] : 0.0;
+            v[k] = warp_sum(x);
+        }
+    }
+    __syncthreads();
+}
+
+struct NormArgs {
+    const float *tau;
+    size_t       n;
+    double       f_target, rel_tol;
+    int          max_iter;
+    double      *partials;     // [2][gridDim.x][2]
+    double      *result;       // [0] A, [1] <F> at A, [2] passes, [3] status
+};
+
+__global__ void __launch_bounds__(RED_THREADS) normalize_kernel(const NormArgs a)
+{
+    cg::grid_group grid = cg::this_grid();
+    __shared__ double sh[2 * 32];
+    __shared__ lya_root_state st;
+    if (threadIdx.x == 0) lya_root_reset(&st, a.f_target, a.rel_tol, (double)a.n);
+    __syncthreads();
+
+    for (int pass = 0;; ++pass) {
+        Trial tr[1] = {make_trial(st.a)};
+        double s[2], s0[1], s1[1];
+        accumulate<1>(a.tau, a.n, tr, s0, s1);
+        s[0] = s0[0]; s[1] = s1[0];
+        block_sum<2>(s, sh);
+        double *part = a.partials + (size_t)(pass & 1) * gridDim.x * 2;
+        if (threadIdx.x == 0) { part[2 * blockIdx.x] = s[0]; part[2 * blockIdx.x + 1] = s[1]; }
+        grid.sync();
+        // every block: identical fixed-order reduction of all partials
+        double t[2] = {0.0, 0.0};
+        for (unsigned b = threadIdx.x; b < gridDim.x; b += blockDim.x) {
+            t[0] += __ldcg(part + 2 * b);
+            t[1] += __ldcg(part + 2 * b + 1);
+        }
+        block_sum<2>(t, sh);
+        if (threadIdx.x == 0) {
+            lya_root_step(&st, t[0], t[1]);
+            if (!st.done && st.iters >= a.max_iter) { st.status = LYA_ENOCONV; st.done = 1; }
+        }
+        __syncthreads();
+        if (st.done) break;
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        a.result[0] = st.a;
+        a.result[1] = st.f_at_a;
+        a.result[2] = (double)st.iters;
+        a.result[3] = (double)st.status;
+    }
+}
+
+struct TrialSet { Trial t[LYA_MAX_TRIALS]; };
+
+template <int K>
+__global__ void __launch_bounds__(RED_THREADS) partial_sums_kernel(const float *__restrict__ tau, size_t n,
+                                                                   const TrialSet ts, double *partials)
+{
+    __shared__ double sh[2 * K * 32];
+    Trial tr[K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) tr[k] = ts.t[k];
+    double s0[K], s1[K], s[2 * K];
+    accumulate<K>(tau, n, tr, s0, s1);
+#pragma unroll
+    for (int k = 0; k < K; ++k) { s[k] = s0[k]; s[K + k] = s1[k]; }
+    block_sum<2 * K>(s, sh);
+    if (threadIdx.x == 0)
+#pragma unroll
+        for (int k = 0; k < 2 * K; ++k) partials[(size_t)blockIdx.x * 2 * K + k] = s[k];
+}
+
+// one block: fixed-order sum of the per-block partials -> out[0 .. nv)
+__global__ void __launch_bounds__(RED_THREADS) finish_sums_kernel(const double *partials, int n_blocks, int nv,
+                                                                  double *out)
+{
+    __shared__ double sh[32];
+    for (int k = 0; k < nv; ++k) {
+        double v[1] = {0.0};
+        for (int b = threadIdx.x; b < n_blocks; b += blockDim.x) v[0] += partials[(size_t)b * nv + k];
+        block_sum<1>(v, sh);
+        if (threadIdx.x == 0) out[k] = v[0];
+    }
+}
+
+__global__ void __launch_bounds__(256) flux_kernel(const float *tau, size_t n, Trial tr, float *flux)
+{
+    const size_t gtid = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t gsz  = (size_t)gridDim.x * blockDim.x;
+    size_t head = ((16 - ((uintptr_t)tau & 15)) & 15) >> 2;
+    if (head > n) head = n;
+    const bool vec = (((uintptr_t)(flux + head)) & 15) == 0;
+    const size_t n4 = vec ? (n - head) >> 2 : 0;
+    const float4 *t4 = reinterpret_cast<const float4 *>(tau + head);
+    float4 *f4 = reinterpret_cast<float4 *>(flux + head);
+#pragma unroll 2
+    for (size_t i = gtid; i < n4; i += gsz) {
+        const float4 t = __ldcs(t4 + i);
+        float4 f;
+        f.x = flux_of(t.x, tr); f.y = flux_of(t.y, tr); f.z = flux_of(t.z, tr); f.w = flux_of(t.w, tr);
+        __stcs(f4 + i, f);
+    }
+    const size_t tail0 = head + (n4 << 2);
+    const size_t n_edge = head + (n - tail0);
+    for (size_t e = gtid; e < n_edge; e += gsz) {
+        const size_t i = e < head ? e : tail0 + (e - head);
+        flux[i] = flux_of(tau[i], tr);
+    }
+}
+
+int red_grid(lya_ctx *ctx, size_t n, int per_sm)
+{
+    size_t want = (n / 4 + RED_THREADS - 1) / RED_THREADS;
+    if (want < 1) want = 1;
+    size_t cap = (size_t)ctx->sm_count * per_sm;
+    if (cap > LYA_MAX_RED_BLOCKS) cap = LYA_MAX_RED_BLOCKS;
+    return (int)(want < cap ? want : cap);
+}
+
+}  // namespace
+
+lya_status lya_run_normalize(lya_ctx *ctx, const float *tau, size_t n, double f_target, double rel_tol,
+                             int max_iter, double *a_out, double *f_out, int *iters)
+{
+    if (!ctx->coop_ok) return lya_fail(ctx, LYA_ECUDA, "device does not support cooperative launch");
+    int per_sm = 0;
+    LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, normalize_kernel, RED_THREADS, 0));
+    if (per_sm < 1) return lya_fail(ctx, LYA_ECUDA, "normalize_kernel: zero occupancy");
+    NormArgs a{tau, n, f_target, rel_tol, max_iter, ctx->d_partials, ctx->d_root};
+    int grid = red_grid(ctx, n, per_sm);
+    void *args[] = {(void *)&a};
+    LYA_CUDA(ctx, cudaLaunchCooperativeKernel((void *)normalize_kernel, dim3(grid), dim3(RED_THREADS), args, 0,
+                                              ctx->stream));
+    ctx->launches++;
+    LYA_CUDA(ctx, cudaMemcpyAsync(ctx->h_pinned, ctx->d_root, 4 * sizeof(double), cudaMemcpyDeviceToHost,
+                                  ctx->stream));
+    LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    if (a_out) *a_out = ctx->h_pinned[0];
+    if (f_out) *f_out = ctx->h_pinned[1];
+    if (iters) *iters = (int)ctx->h_pinned[2];
+    lya_status st = (lya_status)(int)ctx->h_pinned[3];
+    if (st == LYA_ENOROOT) return lya_fail(ctx, st, "lya_normalize_mean_flux: no A > 0 reaches f_target");
+    if (st == LYA_ENOCONV) return lya_fail(ctx, st, "lya_normalize_mean_flux: max_iter reached");
+    return st;
+}
+
+lya_status lya_run_partial_sums(lya_ctx *ctx, const float *tau, size_t n, const double *a_trial, int k,
+                                double *sums, double *dsums)
+{
+    TrialSet ts;
+    for (int i = 0; i < LYA_MAX_TRIALS; ++i) ts.t[i] = make_trial(i < k ? a_trial[i] : 0.0);
+    int grid = red_grid(ctx, n, 8);
+    double *part = ctx->d_partials;
+    switch (k) {
+#define LYA_PS_CASE(K) case K: partial_sums_kernel<K><<<grid, RED_THREADS, 0, ctx->stream>>>(tau, n, ts, part); break;
+        LYA_PS_CASE(1) LYA_PS_CASE(2) LYA_PS_CASE(3) LYA_PS_CASE(4)
+        LYA_PS_CASE(5) LYA_PS_CASE(6) LYA_PS_CASE(7) LYA_PS_CASE(8)
+#undef LYA_PS_CASE
+        default: return lya_fail(ctx, LYA_EINVAL, "lya_flux_partial_sums: k must be 1..8");
+    }
+    finish_sums_kernel<<<1, RED_THREADS, 0, ctx->stream>>>(part, grid, 2 * k, ctx->d_root);
+    ctx->launches += 2;
+    LYA_CUDA(ctx, cudaGetLastError());
+    LYA_CUDA(ctx, cudaMemcpyAsync(ctx->h_pinned, ctx->d_root, 2 * k * sizeof(double), cudaMemcpyDeviceToHost,
+                                  ctx->stream));
+    LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    for (int i = 0; i < k; ++i) {
+        sums[i] = ctx->h_pinned[i];
+        if (dsums) dsums[i] = ctx->h_pinned[k + i];
+    }
+    return LYA_OK;
+}
+
+lya_status lya_launch_flux(lya_ctx *ctx, const float *tau, size_t n, double a, float *flux)
+{
+    size_t want = (n / 4 + 255) / 256;
+    if (want < 1) want = 1;
+    size_t cap = (size_t)ctx->sm_count * 8;
+    int grid = (int)(want < cap ? want : cap);
+    flux_kernel<<<grid, 256, 0, ctx->stream>>>(tau, n, make_trial(a), flux);
+    ctx->launches++;
+    LYA_CUDA(ctx, cudaGetLastError());
+    return LYA_OK;
+}

@@ -1,0 +1,253 @@
+"""ctypes binding of the C-ABI library include/lya.h (paper_1105_4747_b200/liblya.so).
+
+Argument marshalling only: every step of the hot path (S1 gas state, S2+S3 tau, S4 normalisation, S5 flux;
+PAPER.md:70-92) runs in the library's CUDA kernels.  PyTorch supplies device memory and the stream.  There is
+no CPU fallback: if the library is missing it is built with nvcc, and if that fails, or no CUDA device is
+present, the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import torch
+
+from . import build as _build
+
+OK, EINVAL, ECUDA, ENOROOT, ENOCONV, ENOMEM = range(6)
+
+
+class LyaError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"lya status {status}: {msg}")
+        self.status = status
+
+
+class CParams(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
+                ("box_mpch", C.c_double), ("z", C.c_double), ("omega_m", C.c_double), ("h", C.c_double),
+                ("omega_b_h2", C.c_double), ("gamma_m12", C.c_double), ("y_he", C.c_double),
+                ("T0", C.c_double), ("gamma", C.c_double), ("delta_pivot", C.c_double)]
+
+
+class CScalars(C.Structure):
+    _fields_ = [("n_pix", C.c_int32)] + [(k, C.c_double) for k in
+                ("Ez", "Hz", "dR_cm", "dv_kms", "V_kms", "b0_kms", "nbarH", "nbarHI", "K", "tau0", "tauGP")]
+
+
+class CRootState(C.Structure):
+    _fields_ = [("f_target", C.c_double), ("rel_tol", C.c_double), ("n_pix", C.c_double),
+                ("lo", C.c_double), ("hi", C.c_double), ("a", C.c_double), ("f_at_a", C.c_double),
+                ("iters", C.c_int32), ("done", C.c_int32), ("status", C.c_int32), ("finishing", C.c_int32)]
+
+
+@dataclass
+class Params:
+    """The paper's free parameters (include/lya.h: lya_params)."""
+    nx: int
+    ny: int
+    nz: int
+    box_mpch: float
+    z: float
+    T0: float
+    gamma: float
+    omega_m: float = 0.3
+    h: float = 0.7
+    omega_b_h2: float = 0.024
+    gamma_m12: float = 1.0
+    y_he: float = 0.24
+    delta_pivot: float = 10.0
+
+    @classmethod
+    def from_workload(cls, w) -> "Params":
+        return cls(nx=w.n, ny=w.n, nz=w.n, box_mpch=w.box_mpch, z=w.z, T0=w.T0, gamma=w.gamma,
+                   omega_m=w.omega_m, h=w.h, omega_b_h2=w.omega_b_h2, gamma_m12=w.gamma_m12,
+                   y_he=w.y_he, delta_pivot=w.delta_pivot)
+
+    def c(self) -> CParams:
+        return CParams(self.nx, self.ny, self.nz, self.box_mpch, self.z, self.omega_m, self.h,
+                       self.omega_b_h2, self.gamma_m12, self.y_he, self.T0, self.gamma, self.delta_pivot)
+
+
+EXPORTS = ("lya_version", "lya_status_string", "lya_scalars_from_params", "lya_create", "lya_destroy",
+           "lya_last_error", "lya_sm_count", "lya_gas_from_density", "lya_tau_sightlines",
+           "lya_normalize_mean_flux", "lya_flux_partial_sums", "lya_root_init", "lya_root_update",
+           "lya_flux", "lya_forest_host", "lya_launch_count")
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Load (building if stale) liblya.so and declare the signatures of include/lya.h."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build()
+    L = C.CDLL(path)
+    vp, fp, dp, ip = C.c_void_p, C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int)
+    pp, sp = C.POINTER(CParams), C.POINTER(CScalars)
+    L.lya_version.restype = C.c_int
+    L.lya_status_string.restype = C.c_char_p
+    L.lya_status_string.argtypes = [C.c_int]
+    L.lya_scalars_from_params.argtypes = [pp, C.c_int, sp]
+    L.lya_create.argtypes = [C.POINTER(vp), C.c_int, vp]
+    L.lya_destroy.argtypes = [vp]
+    L.lya_destroy.restype = None
+    L.lya_last_error.argtypes = [vp]
+    L.lya_last_error.restype = C.c_char_p
+    L.lya_sm_count.argtypes = [vp]
+    L.lya_launch_count.argtypes = [vp]
+    L.lya_launch_count.restype = C.c_uint64
+    L.lya_gas_from_density.argtypes = [vp, pp, fp, C.c_size_t, fp, fp]
+    L.lya_tau_sightlines.argtypes = [vp, pp, C.c_int, C.c_int32, fp, fp, fp, fp]
+    L.lya_normalize_mean_flux.argtypes = [vp, fp, C.c_size_t, C.c_double, C.c_double, C.c_int, dp, dp, ip]
+    L.lya_flux_partial_sums.argtypes = [vp, fp, C.c_size_t, dp, C.c_int, dp, dp]
+    L.lya_root_init.argtypes = [C.POINTER(CRootState), C.c_double, C.c_double, C.c_double]
+    L.lya_root_update.argtypes = [C.POINTER(CRootState), C.c_double, C.c_double]
+    L.lya_flux.argtypes = [vp, fp, C.c_size_t, C.c_double, fp]
+    L.lya_forest_host.argtypes = [vp, pp, C.c_int, C.c_int32, fp, fp, C.c_double, C.c_double, C.c_int,
+                                  fp, fp, dp, dp, ip]
+    _lib = L
+    return L
+
+
+def scalars(p: Params, axis: int = 0) -> dict:
+    """Host-only: the derived scalars of one sightline direction (no GPU needed)."""
+    s, cp = CScalars(), p.c()
+    st = lib().lya_scalars_from_params(C.byref(cp), axis, C.byref(s))
+    if st != OK:
+        raise LyaError(st, "lya_scalars_from_params: bad parameters")
+    return {k: getattr(s, k) for k, _ in CScalars._fields_}
+
+
+def _dev(t: torch.Tensor, name: str) -> int:
+    if not (t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+        raise TypeError(f"{name}: contiguous float32 CUDA tensor required")
+    return t.data_ptr()
+
+
+def _host(t: torch.Tensor | None, name: str):
+    if t is None:
+        return None
+    if t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous():
+        raise TypeError(f"{name}: contiguous float32 host tensor required")
+    return t.data_ptr()
+
+
+class Context:
+    """One lya_ctx bound to a CUDA device and to torch's current stream on it."""
+
+    def __init__(self, device: int | None = None, stream: torch.cuda.Stream | None = None):
+        if not torch.cuda.is_available():
+            raise LyaError(ECUDA, "no CUDA device: this library has no CPU path")
+        self.device = torch.cuda.current_device() if device is None else int(device)
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self._h = C.c_void_p()
+        st = lib().lya_create(C.byref(self._h), self.device, C.c_void_p(self.stream.cuda_stream))
+        if st != OK:
+            raise LyaError(st, "lya_create failed")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib().lya_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def _check(self, st: int, allow=()):
+        if st != OK and st not in allow:
+            raise LyaError(st, lib().lya_last_error(self._h).decode())
+        return st
+
+    @property
+    def sm_count(self) -> int:
+        return lib().lya_sm_count(self._h)
+
+    @property
+    def launch_count(self) -> int:
+        return int(lib().lya_launch_count(self._h))
+
+    # S1
+    def gas_from_density(self, p: Params, delta: torch.Tensor, n_hi=None, b_kms=None):
+        n_hi = torch.empty_like(delta) if n_hi is None else n_hi
+        b_kms = torch.empty_like(delta) if b_kms is None else b_kms
+        cp = p.c()
+        self._check(lib().lya_gas_from_density(self._h, C.byref(cp), _dev(delta, "delta"), delta.numel(),
+                                               _dev(n_hi, "n_hi"), _dev(b_kms, "b_kms")))
+        return n_hi, b_kms
+
+    # S2 + S3
+    def tau_sightlines(self, p: Params, axis: int, n_hi, b_kms, v_pec, tau=None, nz_local=None):
+        tau = torch.empty_like(n_hi) if tau is None else tau
+        nz_local = n_hi.shape[0] if nz_local is None else nz_local
+        if n_hi.numel() != nz_local * p.ny * p.nx or b_kms.numel() != n_hi.numel() or \
+                v_pec.numel() != n_hi.numel() or tau.numel() != n_hi.numel():
+            raise ValueError("tau_sightlines: arrays must be [nz_local][ny][nx]")
+        cp = p.c()
+        self._check(lib().lya_tau_sightlines(self._h, C.byref(cp), axis, nz_local, _dev(n_hi, "n_hi"),
+                                             _dev(b_kms, "b_kms"), _dev(v_pec, "v_pec"), _dev(tau, "tau")))
+        return tau
+
+    # S4
+    def normalize_mean_flux(self, tau, f_target: float, rel_tol: float = 1e-7, max_iter: int = 60,
+                            allow_noconv: bool = False):
+        a, f, it = C.c_double(), C.c_double(), C.c_int()
+        st = self._check(lib().lya_normalize_mean_flux(self._h, _dev(tau, "tau"), tau.numel(), f_target,
+                                                       rel_tol, max_iter, C.byref(a), C.byref(f), C.byref(it)),
+                         allow=(ENOCONV,) if allow_noconv else ())
+        return a.value, f.value, it.value, st
+
+    def flux_partial_sums(self, tau, a_trials):
+        k = len(a_trials)
+        at = (C.c_double * k)(*a_trials)
+        s, d = (C.c_double * k)(), (C.c_double * k)()
+        self._check(lib().lya_flux_partial_sums(self._h, _dev(tau, "tau"), tau.numel(), at, k, s, d))
+        return list(s), list(d)
+
+    # S5
+    def flux(self, tau, a: float, out=None):
+        out = torch.empty_like(tau) if out is None else out
+        self._check(lib().lya_flux(self._h, _dev(tau, "tau"), tau.numel(), a, _dev(out, "flux")))
+        return out
+
+    # S1..S5 from host buffers
+    def forest_host(self, p: Params, axis: int, delta_h, v_pec_h, f_target: float, rel_tol: float = 1e-7,
+                    max_iter: int = 60, slab_nz: int = 0, tau_h=None, flux_h=None):
+        a, f, it = C.c_double(), C.c_double(), C.c_int()
+        cp = p.c()
+        self._check(lib().lya_forest_host(self._h, C.byref(cp), axis, slab_nz, _host(delta_h, "delta_h"),
+                                          _host(v_pec_h, "v_pec_h"), f_target, rel_tol, max_iter,
+                                          _host(tau_h, "tau_h"), _host(flux_h, "flux_h"),
+                                          C.byref(a), C.byref(f), C.byref(it)))
+        return a.value, f.value, it.value
+
+
+def normalize_mean_flux_sharded(ctx: Context, tau_local, f_target: float, n_pix_global: int,
+                                rel_tol: float = 1e-7, max_iter: int = 60, group=None, partial_sums=None):
+    """S4 when the pixels are sharded over ranks (z-slabs per GPU).
+
+    Each pass: local (sum e, sum tau e) from lya_flux_partial_sums, one all-reduce of two doubles, then the
+    library's scalar update lya_root_update -- identical on every rank, so all ranks hold the same A.
+    `partial_sums` lets a CPU test (gloo) stand in for the kernel; the product path leaves it None.
+    """
+    import torch.distributed as dist
+    L = lib()
+    st = CRootState()
+    if L.lya_root_init(C.byref(st), f_target, rel_tol, float(n_pix_global)) != OK:
+        raise LyaError(EINVAL, "lya_root_init: bad arguments")
+    sums_fn = partial_sums if partial_sums is not None else (lambda a: ctx.flux_partial_sums(tau_local, [a]))
+    while not st.done:
+        s, d = sums_fn(st.a)
+        buf = torch.tensor([s[0], d[0]], dtype=torch.float64)
+        if dist.is_available() and dist.is_initialized():
+            if dist.get_backend(group) == "nccl":
+                buf = buf.cuda()
+            dist.all_reduce(buf, op=dist.ReduceOp.SUM, group=group)
+            buf = buf.cpu()
+        rc = L.lya_root_update(C.byref(st), float(buf[0]), float(buf[1]))
+        if rc == ENOROOT:
+            raise LyaError(rc, "no A > 0 reaches f_target")
+        if not st.done and st.iters >= max_iter:
+            break
+    return st.a, st.f_at_a, st.iters
