@@ -20,6 +20,7 @@ struct lya_ctx {
     double       *d_partials;     // [2 parities][LYA_MAX_RED_BLOCKS][2*LYA_MAX_TRIALS]
     double       *d_root;         // device copy of the root-iteration result (see normalize.cu)
     double       *h_pinned;       // small pinned host mirror
+    unsigned int *d_sched;        // tau_x_kernel row counter {next row, groups finished}; zero between launches
     // lya_forest_host workspace (device), grown on demand
     void         *ws;
     size_t        ws_bytes;

@@ -3,38 +3,46 @@
 //   tau(i) = K sum_j nHI(j)/b(j) exp(-((v_H(i) - u(j))/b(j))^2),   u(j) = v_H(j) + v_pec(j),
 //   v_H(i) - v_H(j) = (i-j) dv, nearest periodic image (period V = N dv; reading C7).
 //
-// Every (i,j) pair is evaluated (N^2 per sightline): the kernel is bound by MUFU.EX2 (16 /clk/SM), so the
-// pair body is kept at 4 FP32 instructions + 1 MUFU:
+// Every (i,j) pair is evaluated (N^2 per sightline): the kernel is bound by MUFU.EX2 (16 /clk/SM, measured),
+// and on sm_100a every extra FP32 instruction per pair costs MUFU rate long before the issue limit
+// (profiles/r1_tau_loop_probe.md), so the pair body is 3.25 FP32 instructions + 1 MUFU:
 //
 //   staged per source cell j (once per sightline, in shared memory, one float4):
 //       m_j = j + P_j          P_j = round(v_pec/dv), reduced mod N          (integer-valued float, exact)
 //       w_j = (dv/b_j) sqrt(log2 e)                                          (so exp(-x^2) = ex2(-(x')^2))
 //       g_j = -f_j w_j         f_j = v_pec/dv - round(v_pec/dv)  in [-1/2,1/2] (computed in double)
 //       a_j = K 1e-5 nHI_j / b_j                                             (line-centre amplitude)
-//   per pair:  E = c_i - m_j (exact) ; x = fma(E, w_j, g_j) ; e = ex2(-x*x) ; acc = fma(a_j, e, acc)
+//   a thread owns R CONSECUTIVE pixels i_0 .. i_0+R-1; per source cell:
+//       E   = (i_0 + R/2) - m_j (exact) ;  x_ref = fma(E, w_j, g_j)          (2 FP32 per R pairs)
+//       x_r = fma(r - R/2, w_j, x_ref)                                       (1 FFMA, none for r = R/2)
+//       e   = ex2(-x_r * x_r)  ;  acc_r = fma(a_j, e, acc_r)                 (FMUL + MUFU + FFMA)
 //
 // Keeping the integer part of the pixel separation exact is what holds the error at ~1e-6 for N = 2048
-// (forming u_j and v_i in fp32 km/s loses 3 digits there).
+// (forming u_j and v_i in fp32 km/s loses 3 digits there); x_ref is at most R/2 cells away
+// from the pixel it serves, so for every pair that contributes its rounding error is ulp(|x| + 2 w)/2.
 //
 // Periodic wrap without per-pair work: a warp owns a tile of 32*R consecutive pixels and walks the sources
 // in UNWRAPPED order jj = c - N/2 ... c + N/2 - 1 around the tile centre c (two contiguous index segments),
 // so i - jj is already the nearest image for every pair that can contribute.  That is valid when, for every
 // source of the sightline, (N/2 - 16R - |P_j| - 1) w_j >= 12.5, i.e. a pair whose chosen image is not the
 // nearest has ex2(-x^2) == 0 in fp32 (and < 2^-156 of a_j in the oracle's double).  The staging pass checks
-// the condition; a batch that fails it (tiny N, |v_pec| of order V) takes the general loop with a per-pair
-// image choice.  Both loops evaluate all N^2 pairs.
+// the condition; a sightline that fails it (tiny N, |v_pec| of order V) takes the general loop with a
+// per-pair image choice.  Both loops evaluate all N^2 pairs.
 //
-// Mapping: persistent CTAs (grid = k * SM count) loop over batches of B sightlines; a batch's nHI/b/v_pec
-// rows are fetched by cp.async.bulk into a 2-stage shared-memory ring (mbarrier complete_tx) while the
-// previous batch is being summed; the 8 warps of the CTA then take (sightline, pixel-tile) items, every
-// lane reading the same staged cell (broadcast LDS.128) for R pixels.  Sightlines along y / z are gathered
-// 8 (or fewer) neighbouring x at a time so that global accesses stay 32-byte segments, and tau goes back
-// through a shared-memory tile the same way.
+// Mapping, sightlines along x (contiguous rows): a GROUP of G warps (G = 1 unless the row is too long for
+// enough groups to fit in shared memory) owns one sightline at a time: it stages the row with 128-bit
+// coalesced loads straight into its private float4 cells, syncs only itself (named barrier / __syncwarp),
+// sums its tiles and stores R consecutive tau values per lane (128-bit).  Groups never wait for each other,
+// so the MUFU pipe always has warps in the pair loop while others stage; rows are handed out by a global
+// atomic counter, which removes the wave-quantisation tail of a static partition (65,536 rows over
+// ~6,000 resident warps would lose 8 %).
+// Sightlines along y / z: a CTA gathers 8 (or fewer) neighbouring x at a time so that global accesses stay
+// 32-byte segments, its 8 warps sum (sightline, tile) items, and tau goes back through a shared-memory tile.
 #include "lya_internal.h"
 
 namespace {
 
-constexpr int   TAU_WARPS   = 8;
+constexpr int   TAU_WARPS   = 8;       // strided kernel: warps per CTA
 constexpr int   TAU_THREADS = TAU_WARPS * 32;
 constexpr float TAU_XCUT    = 12.5f;   // ex2(-12.5^2) = 2^-156: exactly 0 in fp32 (ftz)
 
@@ -43,17 +51,20 @@ struct TauArgs {
     float       *tau;
     int          n;           // pixels per sightline
     int          tiles;       // pixel tiles of 32*R per sightline
-    int          bsl;         // sightlines per batch (x-axis) / x-width of a gathered batch (y,z; power of 2)
-    int          bshift;      // log2(bsl) for the strided modes
+    int          vec;         // x-axis: rows are 16-byte aligned and n % 4 == 0
+    int          bsl;         // strided: x-width of a gathered batch (power of 2)
+    int          bshift;      // log2(bsl)
     long long    n_sl;        // x-axis: number of sightlines (rows)
-    long long    n_batches;
+    long long    n_batches;   // strided: number of gathered batches
+    unsigned int *sched;      // x-axis: [0] next row, [1] groups finished (self-resetting)
     // strided modes (axis 1, 2)
     int          nx;          // x extent
     int          nxb;         // ceil(nx / bsl)
     long long    outer_stride; // elements between consecutive "outer" indices (axis 1: ny*nx per iz; axis 2: nx per iy)
     long long    stride;      // elements between consecutive pixels of a sightline
     double       inv_dv;      // 1 / dv  [s/km]
-    float        amp_scale;   // K * 1e-5  [cm^3 * km/s ... so that a_j is dimensionless]
+    double       inv_n_d;     // 1 / N
+    float        amp_scale;   // K * 1e-5  [so that a_j is dimensionless]
     float        w_scale;     // dv * sqrt(log2 e) [km/s]
     float        inv_n, n_f;  // 1/N, N
 };
@@ -65,35 +76,6 @@ __device__ __forceinline__ float ex2_ftz(float x)
     return y;
 }
 
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-// 1-D bulk copy global -> shared, completion signalled on an mbarrier (SASS: UBLKCP).
-__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
-
 // One source cell -> staged float4 (m, w, g, a); returns 1 if the cell breaks the fast-path condition.
 __device__ __forceinline__ int stage_cell(const TauArgs &a, int j, float nh, float bb, float vv, int half_span,
                                           float4 &out)
@@ -101,7 +83,8 @@ __device__ __forceinline__ int stage_cell(const TauArgs &a, int j, float nh, flo
     double p  = (double)vv * a.inv_dv;                 // displacement in pixels (reading C11: +v -> higher index)
     double P  = rint(p);
     float  f  = (float)(p - P);                        // [-1/2, 1/2], full fp32 precision
-    double Pr = P - (double)a.n * rint(P / (double)a.n);   // integer displacement reduced to [-N/2, N/2]
+    // integer displacement reduced to [-N/2, N/2]; at an exact half-way point either image is nearest
+    double Pr = P - (double)a.n * rint(P * a.inv_n_d);
     float  w  = a.w_scale / bb;
     out.x = (float)((double)j + Pr);
     out.y = w;
@@ -111,37 +94,36 @@ __device__ __forceinline__ int stage_cell(const TauArgs &a, int j, float nh, flo
     return !(room * w >= TAU_XCUT);
 }
 
-// Fast path: unwrapped walk around the tile centre, no per-pair image logic.
+// Fast path: unwrapped walk around the tile centre, no per-pair image logic.  Lane owns pixels
+// i0 + lane*R + r, r = 0..R-1.
 template <int R>
 __device__ __forceinline__ void tile_fast(const float4 *__restrict__ cs, int n, int i0, int lane, float (&acc)[R])
 {
+    constexpr int RH = R / 2;                          // reference pixel of the lane
     const int c     = i0 + 16 * R;
     const int start = c - (n >> 1);                    // first unwrapped source index
     int j0 = start % n;
     if (j0 < 0) j0 += n;                               // slot holding jj = start
     const int off = start - j0;                        // jj = j + off on [j0, n), jj = j + off + n on [0, j0)
-    float cr[R];
+    float cref = (float)(i0 + lane * R + RH - off);
 #pragma unroll
-    for (int r = 0; r < R; ++r) {
-        acc[r] = 0.0f;
-        cr[r]  = (float)(i0 + lane + 32 * r - off);
-    }
+    for (int r = 0; r < R; ++r) acc[r] = 0.0f;
 #pragma unroll 1
     for (int seg = 0; seg < 2; ++seg) {
         const int lo = seg ? 0 : j0, hi = seg ? j0 : n;
-#pragma unroll 4
+#pragma unroll 8
         for (int j = lo; j < hi; ++j) {
             const float4 q = cs[j];
+            const float E  = cref - q.x;
+            const float xr = fmaf(E, q.y, q.z);
 #pragma unroll
             for (int r = 0; r < R; ++r) {
-                float E = cr[r] - q.x;
-                float x = fmaf(E, q.y, q.z);
-                float e = ex2_ftz(-(x * x));
-                acc[r]  = fmaf(q.w, e, acc[r]);
+                const float x = (r == RH) ? xr : fmaf((float)(r - RH), q.y, xr);
+                const float e = ex2_ftz(-(x * x));
+                acc[r] = fmaf(q.w, e, acc[r]);
             }
         }
-#pragma unroll
-        for (int r = 0; r < R; ++r) cr[r] -= (float)n;
+        cref -= (float)n;
     }
 }
 
@@ -154,7 +136,7 @@ __device__ __forceinline__ void tile_general(const float4 *__restrict__ cs, int 
 #pragma unroll
     for (int r = 0; r < R; ++r) {
         acc[r] = 0.0f;
-        ci[r]  = (float)(i0 + lane + 32 * r);
+        ci[r]  = (float)(i0 + lane * R + r);
     }
 #pragma unroll 2
     for (int j = 0; j < n; ++j) {
@@ -172,93 +154,114 @@ __device__ __forceinline__ void tile_general(const float4 *__restrict__ cs, int 
     }
 }
 
-// MODE 0: x-axis, cp.async.bulk ring.  MODE 1: x-axis, plain loads (unaligned / N % 4 != 0).
-// MODE 2: strided sightlines (y or z), gathered bsl neighbouring x at a time.
-template <int R, int MODE>
-__global__ void __launch_bounds__(TAU_THREADS) tau_kernel(const TauArgs a)
+__device__ __forceinline__ void group_sync(int G, int bar_id)
 {
-    extern __shared__ __align__(128) unsigned char smem[];
+    if (G == 1) __syncwarp();
+    else asm volatile("bar.sync %0, %1;" ::"r"(bar_id), "r"(G * 32) : "memory");
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Sightlines along x.  blockDim = 32 * G * (groups per CTA); dynamic shared memory: groups x n float4 cells,
+// then one int4 control word per group {row, bad, -, -}.
+template <int R>
+__global__ void __launch_bounds__(1024, 1) tau_x_kernel(const TauArgs a, const int G, const int gpc)
+{
+    extern __shared__ __align__(16) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int grp = warp / G, wg = warp - grp * G;       // group in CTA, warp in group
     const int n = a.n;
-    const int cstride = (MODE == 2) ? n + 1 : n;        // +1 cell: conflict-free transposed staging
-    float4 *cells = reinterpret_cast<float4 *>(smem);
-    const size_t cells_bytes = (size_t)a.bsl * cstride * sizeof(float4);
-    float *aux = reinterpret_cast<float *>(smem + cells_bytes);     // MODE 0: raw ring; MODE 2: tau tile
-    const int per_arr = a.bsl * n;                                  // floats per raw array per stage
-    uint64_t *mbar = reinterpret_cast<uint64_t *>(smem + cells_bytes + (size_t)6 * per_arr * sizeof(float));
+    float4 *cells = reinterpret_cast<float4 *>(smem) + (size_t)grp * n;
+    volatile int *ctl = reinterpret_cast<volatile int *>(smem + (size_t)gpc * n * sizeof(float4)) + 4 * grp;
+    const int bar_id = grp;                              // named barrier of the group (G >= 2: at most 16 groups; __syncthreads is not used here)
+    const int gl = wg * 32 + lane, gthreads = G * 32;    // thread index / count inside the group
 
-    auto issue = [&](long long batch, int stage) {                  // MODE 0, one thread
-        long long s0 = batch * a.bsl;
-        int nb = (int)((a.n_sl - s0 < a.bsl) ? (a.n_sl - s0) : a.bsl);
-        uint32_t bytes = (uint32_t)nb * n * 4u;
-        float *dst = aux + (size_t)stage * 3 * per_arr;
-        mbar_expect_tx(&mbar[stage], 3u * bytes);
-        bulk_g2s(dst,               a.n_hi + s0 * n, bytes, &mbar[stage]);
-        bulk_g2s(dst + per_arr,     a.b    + s0 * n, bytes, &mbar[stage]);
-        bulk_g2s(dst + 2 * per_arr, a.v    + s0 * n, bytes, &mbar[stage]);
-    };
-
-    if (MODE == 0) {
-        if (tid == 0) {
-            mbar_init(&mbar[0], 1);
-            mbar_init(&mbar[1], 1);
-            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    for (;;) {
+        if (gl == 0) {
+            ctl[0] = (int)atomicAdd(&a.sched[0], 1u);
+            ctl[1] = 0;
         }
-        __syncthreads();
-        if (tid == 0 && (long long)blockIdx.x < a.n_batches) issue(blockIdx.x, 0);
+        group_sync(G, bar_id);
+        const long long row = (unsigned int)ctl[0];
+        if (row >= a.n_sl) break;
+        const size_t g0 = (size_t)row * n;
+
+        // ---- stage the row: (nHI, b, v_pec) -> (m, w, g, a) per cell; 128-byte coalesced loads
+        int bad = 0;
+#pragma unroll 4
+        for (int j = gl; j < n; j += gthreads) {
+            float4 q;
+            bad |= stage_cell(a, j, __ldcs(a.n_hi + g0 + j), __ldcs(a.b + g0 + j), __ldcs(a.v + g0 + j), 16 * R, q);
+            cells[j] = q;
+        }
+        bad = __any_sync(0xffffffffu, bad);
+        if (G > 1 && bad && lane == 0) ctl[1] = 1;
+        group_sync(G, bar_id);
+        if (G > 1) bad = ctl[1];
+
+        // ---- sum: the group's warps take the pixel tiles of the row
+        for (int tile = wg; tile < a.tiles; tile += G) {
+            const int i0 = tile * 32 * R;
+            float acc[R];
+            if (!bad) tile_fast<R>(cells, n, i0, lane, acc);
+            else      tile_general<R>(cells, n, a.n_f, a.inv_n, i0, lane, acc);
+            const int i = i0 + lane * R;
+            float *dst = a.tau + g0 + i;
+            if (R == 4 && a.vec) {
+                if (i < n) __stcs(reinterpret_cast<float4 *>(dst), make_float4(acc[0], acc[1], acc[2], acc[3]));
+            } else if (R == 2 && a.vec) {
+                if (i < n) __stcs(reinterpret_cast<float2 *>(dst), make_float2(acc[0], acc[1]));
+            } else {
+#pragma unroll
+                for (int r = 0; r < R; ++r)
+                    if (i + r < n) dst[r] = acc[r];
+            }
+        }
+        group_sync(G, bar_id);                           // cells and ctl consumed
     }
 
-    int it = 0;
-    for (long long batch = blockIdx.x; batch < a.n_batches; batch += gridDim.x, ++it) {
-        int nb;                       // sightlines in this batch
-        long long base = 0;           // strided: element offset of (pixel 0, first x of the batch)
-        if (MODE == 2) {
-            long long outer = batch / a.nxb;
-            int xb = (int)(batch - outer * a.nxb);
-            int x0 = xb << a.bshift;
-            nb   = (a.nx - x0 < a.bsl) ? (a.nx - x0) : a.bsl;
-            base = outer * a.outer_stride + x0;
-        } else {
-            long long s0 = batch * a.bsl;
-            nb = (int)((a.n_sl - s0 < a.bsl) ? (a.n_sl - s0) : a.bsl);
+    // the last group to finish re-arms the row counter for the next launch on this ctx
+    if (gl == 0) {
+        __threadfence();
+        const unsigned int total = gridDim.x * (unsigned int)gpc;
+        if (atomicAdd(&a.sched[1], 1u) == total - 1u) {
+            a.sched[0] = 0u;
+            a.sched[1] = 0u;
+            __threadfence();
         }
+    }
+}
 
-        // ---- stage the batch: (nHI, b, v_pec) -> (m, w, g, a) per cell
+// ---------------------------------------------------------------------------------------------------------
+// Sightlines along y or z, gathered bsl neighbouring x at a time (persistent CTAs, static batches).
+template <int R>
+__global__ void __launch_bounds__(TAU_THREADS) tau_strided_kernel(const TauArgs a)
+{
+    extern __shared__ __align__(16) unsigned char smem[];
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int n = a.n;
+    const int cstride = n + 1;                           // +1 cell: conflict-free transposed staging
+    float4 *cells = reinterpret_cast<float4 *>(smem);
+    float *ttile = reinterpret_cast<float *>(smem + (size_t)a.bsl * cstride * sizeof(float4));   // [n][bsl]
+
+    for (long long batch = blockIdx.x; batch < a.n_batches; batch += gridDim.x) {
+        const long long outer = batch / a.nxb;
+        const int xb = (int)(batch - outer * a.nxb);
+        const int x0 = xb << a.bshift;
+        const int nb = (a.nx - x0 < a.bsl) ? (a.nx - x0) : a.bsl;
+        const long long base = outer * a.outer_stride + x0;   // element offset of (pixel 0, first x of the batch)
+
         int bad = 0;
-        if (MODE == 0) {
-            const int stage = it & 1;
-            long long next = batch + gridDim.x;
-            if (tid == 0 && next < a.n_batches) issue(next, stage ^ 1);
-            mbar_wait(&mbar[stage], (uint32_t)((it >> 1) & 1));
-            const float *raw = aux + (size_t)stage * 3 * per_arr;
-            for (int c = tid; c < nb * n; c += TAU_THREADS) {
-                int j = c % n;
+        for (int c = tid; c < (n << a.bshift); c += TAU_THREADS) {
+            const int bx = c & (a.bsl - 1), j = c >> a.bshift;
+            if (bx < nb) {
+                const long long g = base + (long long)j * a.stride + bx;
                 float4 q;
-                bad |= stage_cell(a, j, raw[c], raw[per_arr + c], raw[2 * per_arr + c], 16 * R, q);
-                cells[c] = q;
-            }
-        } else if (MODE == 1) {
-            const long long g0 = batch * a.bsl * n;
-            for (int c = tid; c < nb * n; c += TAU_THREADS) {
-                int j = c % n;
-                float4 q;
-                bad |= stage_cell(a, j, __ldg(a.n_hi + g0 + c), __ldg(a.b + g0 + c), __ldg(a.v + g0 + c), 16 * R, q);
-                cells[c] = q;
-            }
-        } else {
-            for (int c = tid; c < (n << a.bshift); c += TAU_THREADS) {
-                int bx = c & (a.bsl - 1), j = c >> a.bshift;
-                if (bx < nb) {
-                    long long g = base + (long long)j * a.stride + bx;
-                    float4 q;
-                    bad |= stage_cell(a, j, __ldg(a.n_hi + g), __ldg(a.b + g), __ldg(a.v + g), 16 * R, q);
-                    cells[bx * cstride + j] = q;
-                }
+                bad |= stage_cell(a, j, __ldcs(a.n_hi + g), __ldcs(a.b + g), __ldcs(a.v + g), 16 * R, q);
+                cells[bx * cstride + j] = q;
             }
         }
         bad = __syncthreads_or(bad);
 
-        // ---- sum: warps take (sightline, pixel tile) items
         const int items = nb * a.tiles;
         for (int item = warp; item < items; item += TAU_WARPS) {
             const int sl = item / a.tiles, tile = item - sl * a.tiles;
@@ -269,28 +272,48 @@ __global__ void __launch_bounds__(TAU_THREADS) tau_kernel(const TauArgs a)
             else      tile_general<R>(cs, n, a.n_f, a.inv_n, i0, lane, acc);
 #pragma unroll
             for (int r = 0; r < R; ++r) {
-                int i = i0 + lane + 32 * r;
-                if (i < n) {
-                    if (MODE == 2) aux[(i << a.bshift) + sl] = acc[r];
-                    else           a.tau[(batch * a.bsl + sl) * n + i] = acc[r];
-                }
+                const int i = i0 + lane * R + r;
+                if (i < n) ttile[(i << a.bshift) + sl] = acc[r];
             }
         }
-        __syncthreads();                                 // cells (and the tau tile) complete / consumed
-        if (MODE == 2) {
-            for (int c = tid; c < (n << a.bshift); c += TAU_THREADS) {
-                int bx = c & (a.bsl - 1), j = c >> a.bshift;
-                if (bx < nb) a.tau[base + (long long)j * a.stride + bx] = aux[c];
-            }
-            __syncthreads();
+        __syncthreads();                                 // cells consumed, tau tile complete
+        for (int c = tid; c < (n << a.bshift); c += TAU_THREADS) {
+            const int bx = c & (a.bsl - 1), j = c >> a.bshift;
+            if (bx < nb) __stcs(a.tau + base + (long long)j * a.stride + bx, ttile[c]);
         }
+        __syncthreads();
     }
 }
 
-template <int R, int MODE>
-lya_status launch_rm(lya_ctx *ctx, const TauArgs &a, size_t smem_bytes)
+template <int R>
+lya_status launch_x(lya_ctx *ctx, const TauArgs &a)
 {
-    auto kern = tau_kernel<R, MODE>;
+    auto kern = tau_x_kernel<R>;
+    const size_t cap = (size_t)ctx->max_smem_optin;
+    const size_t per_group = (size_t)a.n * sizeof(float4) + 16;
+    int groups = (int)(cap / per_group);                 // groups that fit in one SM's shared memory
+    if (groups < 1) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: sightline too long for shared memory");
+    // G warps per group: as few as keep >= 24 warps resident and no more than the row has tiles
+    int G = 1;
+    while (G < 16 && G * (groups < 32 / G ? groups : 32 / G) < 24 && 2 * G <= a.tiles) G *= 2;
+    if (groups > 32 / G) groups = 32 / G;
+    // one persistent CTA per SM; never more groups than rows
+    long long want = (a.n_sl + ctx->sm_count - 1) / ctx->sm_count;
+    if (groups > want) groups = (int)(want < 1 ? 1 : want);
+    const size_t smem_bytes = (size_t)groups * per_group;
+    LYA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
+    long long ctas = (a.n_sl + groups - 1) / groups;
+    const int grid = (int)(ctas < ctx->sm_count ? ctas : ctx->sm_count);
+    kern<<<grid, 32 * G * groups, smem_bytes, ctx->stream>>>(a, G, groups);
+    ctx->launches++;
+    LYA_CUDA(ctx, cudaGetLastError());
+    return LYA_OK;
+}
+
+template <int R>
+lya_status launch_strided(lya_ctx *ctx, const TauArgs &a, size_t smem_bytes)
+{
+    auto kern = tau_strided_kernel<R>;
     LYA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
     int per_sm = 0;
     LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, TAU_THREADS, smem_bytes));
@@ -301,16 +324,6 @@ lya_status launch_rm(lya_ctx *ctx, const TauArgs &a, size_t smem_bytes)
     ctx->launches++;
     LYA_CUDA(ctx, cudaGetLastError());
     return LYA_OK;
-}
-
-template <int MODE>
-lya_status launch_m(lya_ctx *ctx, int R, const TauArgs &a, size_t smem_bytes)
-{
-    switch (R) {
-        case 1:  return launch_rm<1, MODE>(ctx, a, smem_bytes);
-        case 2:  return launch_rm<2, MODE>(ctx, a, smem_bytes);
-        default: return launch_rm<4, MODE>(ctx, a, smem_bytes);
-    }
 }
 
 }  // namespace
@@ -325,6 +338,7 @@ lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
     const int n = axis == 0 ? nx : (axis == 1 ? ny : nz_local);
     a.n = n;
     a.inv_dv    = 1.0 / dv_kms;
+    a.inv_n_d   = 1.0 / (double)n;
     a.amp_scale = (float)amp_scale;
     a.w_scale   = (float)(dv_kms * 1.2011224087864498);   // sqrt(log2 e)
     a.n_f = (float)n;
@@ -335,21 +349,14 @@ lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
 
     if (axis == 0) {
         a.n_sl = (long long)ny * nz_local;
-        int bsl = TAU_WARPS / a.tiles;
-        if (bsl < 1) bsl = 1;
-        if ((long long)bsl > a.n_sl) bsl = (int)a.n_sl;
-        bool bulk = (n % 4 == 0) && ((((uintptr_t)n_hi | (uintptr_t)b | (uintptr_t)v) & 15) == 0);
-        // shrink the batch if it would not fit (very long sightlines)
-        auto need = [&](int bs, bool blk) {
-            return (size_t)bs * n * 16 + (blk ? (size_t)bs * n * 24 + 16 : 0);
-        };
-        while (bsl > 1 && need(bsl, bulk) > smem_cap / 2) bsl >>= 1;
-        if (bulk && need(bsl, true) > smem_cap) bulk = false;
-        if (need(bsl, bulk) > smem_cap)
-            return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: sightline too long for shared memory");
-        a.bsl = bsl;
-        a.n_batches = (a.n_sl + bsl - 1) / bsl;
-        return bulk ? launch_m<0>(ctx, R, a, need(bsl, true)) : launch_m<1>(ctx, R, a, need(bsl, false));
+        if (a.n_sl >= (1LL << 31)) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: more than 2^31 sightlines");
+        a.vec = (n % 4 == 0) && (((uintptr_t)tau & 15) == 0);
+        a.sched = ctx->d_sched;
+        switch (R) {
+            case 1:  return launch_x<1>(ctx, a);
+            case 2:  return launch_x<2>(ctx, a);
+            default: return launch_x<4>(ctx, a);
+        }
     }
 
     // strided: axis 1 (pixels along y, outer index iz) or axis 2 (pixels along z, outer index iy)
@@ -366,5 +373,9 @@ lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
     a.bsl = 1 << bshift;
     a.nxb = (nx + a.bsl - 1) / a.bsl;
     a.n_batches = n_outer * a.nxb;
-    return launch_m<2>(ctx, R, a, need2(bshift));
+    switch (R) {
+        case 1:  return launch_strided<1>(ctx, a, need2(bshift));
+        case 2:  return launch_strided<2>(ctx, a, need2(bshift));
+        default: return launch_strided<4>(ctx, a, need2(bshift));
+    }
 }

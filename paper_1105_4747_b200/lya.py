@@ -149,8 +149,8 @@ class Context:
             raise LyaError(st, "lya_create failed")
 
     def close(self):
-        if getattr(self, "_h", None):
-            lib().lya_destroy(self._h)
+        if getattr(self, "_h", None) and _lib is not None:      # _lib is None only at interpreter shutdown
+            _lib.lya_destroy(self._h)
             self._h = None
 
     __del__ = close

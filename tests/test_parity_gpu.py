@@ -198,7 +198,10 @@ def test_gpu_invariants_shift_and_velocity_offset(ctx, oracle):
     s = 37                                                            # P4: cyclic shift
     tau_s = ctx.tau_sightlines(p, 0, n_hi.roll(s, 2).contiguous(), b.roll(s, 2).contiguous(),
                                vx.roll(s, 2).contiguous())
-    assert torch.allclose(tau_s, tau.roll(s, 2), rtol=2e-6, atol=1e-9)
+    # a pixel's rounding depends on where it sits in its lane's group of R pixels (x_ref is up to 2 cells away:
+    # dx <= ulp(|x| + 2w)/2 ~ 2e-6, i.e. ~ln2 * 2 x dx <= 5e-6 relative per term), so two
+    # evaluations of the same sum at shifted positions may differ by twice that
+    assert torch.allclose(tau_s, tau.roll(s, 2), rtol=1e-5, atol=1e-9)
     k = 5                                                             # P5: +k dv moves tau by +k pixels
     tau_k = ctx.tau_sightlines(p, 0, n_hi, b, (vx.double() + k * dv).float())
     assert torch.allclose(tau_k, tau.roll(k, 2), rtol=3e-5, atol=1e-8)
