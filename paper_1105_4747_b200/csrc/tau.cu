@@ -10,7 +10,7 @@
 //   staged per source cell j (once per sightline, in shared memory, one float4):
 //       m_j = j + P_j          P_j = round(v_pec/dv), reduced mod N          (integer-valued float, exact)
 //       w_j = (dv/b_j) sqrt(log2 e)                                          (so exp(-x^2) = ex2(-(x')^2))
-//       g_j = -f_j w_j         f_j = v_pec/dv - round(v_pec/dv)  in [-1/2,1/2] (computed in double)
+//       g_j = -f_j w_j         f_j = v_pec/dv - round(v_pec/dv)  in [-1/2,1/2] (exact fma residual)
 //       a_j = K 1e-5 nHI_j / b_j                                             (line-centre amplitude)
 //   a thread owns R CONSECUTIVE pixels i_0 .. i_0+R-1; per source cell:
 //       E   = (i_0 + R/2) - m_j (exact) ;  x_ref = fma(E, w_j, g_j)          (2 FP32 per R pairs)
@@ -38,6 +38,8 @@
 // ~6,000 resident warps would lose 8 %).
 // Sightlines along y / z: a CTA gathers 8 (or fewer) neighbouring x at a time so that global accesses stay
 // 32-byte segments, its 8 warps sum (sightline, tile) items, and tau goes back through a shared-memory tile.
+#include <stdlib.h>
+
 #include "lya_internal.h"
 
 namespace {
@@ -62,8 +64,7 @@ struct TauArgs {
     int          nxb;         // ceil(nx / bsl)
     long long    outer_stride; // elements between consecutive "outer" indices (axis 1: ny*nx per iz; axis 2: nx per iy)
     long long    stride;      // elements between consecutive pixels of a sightline
-    double       inv_dv;      // 1 / dv  [s/km]
-    double       inv_n_d;     // 1 / N
+    float        inv_dv_hi, inv_dv_lo;   // 1 / dv [s/km] as an fp32 pair (hi + lo = the double value)
     float        amp_scale;   // K * 1e-5  [so that a_j is dimensionless]
     float        w_scale;     // dv * sqrt(log2 e) [km/s]
     float        inv_n, n_f;  // 1/N, N
@@ -77,20 +78,24 @@ __device__ __forceinline__ float ex2_ftz(float x)
 }
 
 // One source cell -> staged float4 (m, w, g, a); returns 1 if the cell breaks the fast-path condition.
+// All fp32: p = v_pec/dv is split as P + f with P = rint(v * inv_dv_hi) and f = fma(v, inv_dv_hi, -P) +
+// v * inv_dv_lo -- the fma forms the residual of the exact 48-bit product with ONE rounding of a number
+// below 1, so f carries an absolute error < 1e-7 pixel however large P is (|P| < 2^23 assumed: |v_pec| <
+// 8e6 dv).  No FP64 instruction is needed (reading C11: +v -> higher pixel index).
 __device__ __forceinline__ int stage_cell(const TauArgs &a, int j, float nh, float bb, float vv, int half_span,
                                           float4 &out)
 {
-    double p  = (double)vv * a.inv_dv;                 // displacement in pixels (reading C11: +v -> higher index)
-    double P  = rint(p);
-    float  f  = (float)(p - P);                        // [-1/2, 1/2], full fp32 precision
+    const float P  = rintf(vv * a.inv_dv_hi);
+    const float f  = fmaf(vv, a.inv_dv_lo, fmaf(vv, a.inv_dv_hi, -P));
     // integer displacement reduced to [-N/2, N/2]; at an exact half-way point either image is nearest
-    double Pr = P - (double)a.n * rint(P * a.inv_n_d);
-    float  w  = a.w_scale / bb;
-    out.x = (float)((double)j + Pr);
+    const float Pr = fmaf(-a.n_f, rintf(P * a.inv_n), P);
+    const float ib = 1.0f / bb;
+    const float w  = a.w_scale * ib;
+    out.x = (float)j + Pr;
     out.y = w;
     out.z = -f * w;
-    out.w = a.amp_scale * nh / bb;
-    float room = (float)(a.n >> 1) - (float)half_span - fabsf((float)Pr) - 1.0f;
+    out.w = (a.amp_scale * nh) * ib;
+    const float room = (float)(a.n >> 1) - (float)half_span - fabsf(Pr) - 1.0f;
     return !(room * w >= TAU_XCUT);
 }
 
@@ -161,42 +166,113 @@ __device__ __forceinline__ void group_sync(int G, int bar_id)
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// Sightlines along x.  blockDim = 32 * G * (groups per CTA); dynamic shared memory: groups x n float4 cells,
-// then one int4 control word per group {row, bad, -, -}.
-template <int R>
+// mbarrier / bulk-copy helpers (SASS: SYNCS, UBLKCP)
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// 1-D bulk copy global -> shared, completion signalled on an mbarrier
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+// Sightlines along x.  blockDim = 32 * G * gpc (gpc = groups per CTA).  Dynamic shared memory, per group:
+// n float4 cells [+ PF: 3 n floats of raw nHI | b | v_pec, filled by cp.async.bulk], then per group one
+// int4 control word {row, bad, next row, -} and (PF) one mbarrier.
+// PF = 1 (rows 16-byte aligned, n % 4 == 0): the NEXT row's three input rows are bulk-copied into the
+// group's raw buffer while the current row is being summed, so a row change costs only the conversion
+// raw -> cells.  PF = 0: plain coalesced loads at the row change.
+template <int R, int PF>
 __global__ void __launch_bounds__(1024, 1) tau_x_kernel(const TauArgs a, const int G, const int gpc)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int grp = warp / G, wg = warp - grp * G;       // group in CTA, warp in group
     const int n = a.n;
-    float4 *cells = reinterpret_cast<float4 *>(smem) + (size_t)grp * n;
-    volatile int *ctl = reinterpret_cast<volatile int *>(smem + (size_t)gpc * n * sizeof(float4)) + 4 * grp;
-    const int bar_id = grp;                              // named barrier of the group (G >= 2: at most 16 groups; __syncthreads is not used here)
+    const size_t cell_bytes = (size_t)n * (sizeof(float4) + (PF ? 3 * sizeof(float) : 0));
+    float4 *cells = reinterpret_cast<float4 *>(smem + (size_t)grp * cell_bytes);
+    float *raw = reinterpret_cast<float *>(cells + n);   // PF only
+    unsigned char *tail = smem + (size_t)gpc * cell_bytes;
+    volatile int *ctl = reinterpret_cast<volatile int *>(tail) + 4 * grp;
+    uint64_t *mbar = reinterpret_cast<uint64_t *>(tail + (size_t)gpc * 16) + grp;   // PF only
+    const int bar_id = grp;      // named barrier of the group (G >= 2: at most 16 groups; no __syncthreads here)
     const int gl = wg * 32 + lane, gthreads = G * 32;    // thread index / count inside the group
+    const uint32_t row_bytes = (uint32_t)n * 4u;
 
-    for (;;) {
-        if (gl == 0) {
-            ctl[0] = (int)atomicAdd(&a.sched[0], 1u);
-            ctl[1] = 0;
+    auto prefetch = [&](long long row) {                 // one thread of the group
+        const size_t g = (size_t)row * n;
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // raw was read through the generic proxy
+        mbar_expect_tx(mbar, 3u * row_bytes);
+        bulk_g2s(raw,         a.n_hi + g, row_bytes, mbar);
+        bulk_g2s(raw + n,     a.b + g,    row_bytes, mbar);
+        bulk_g2s(raw + 2 * n, a.v + g,    row_bytes, mbar);
+    };
+
+    if (gl == 0) {
+        const unsigned int r0 = atomicAdd(&a.sched[0], 1u);
+        ctl[0] = (int)r0;
+        if (PF) {
+            mbar_init(mbar, 1);
+            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+            if ((long long)r0 < a.n_sl) prefetch(r0);
         }
-        group_sync(G, bar_id);
+    }
+    group_sync(G, bar_id);
+
+    for (uint32_t it = 0;; ++it) {
         const long long row = (unsigned int)ctl[0];
         if (row >= a.n_sl) break;
         const size_t g0 = (size_t)row * n;
 
-        // ---- stage the row: (nHI, b, v_pec) -> (m, w, g, a) per cell; 128-byte coalesced loads
+        // ---- stage the row: (nHI, b, v_pec) -> (m, w, g, a) per cell
         int bad = 0;
+        if (PF) {
+            mbar_wait(mbar, it & 1u);
+            for (int j = gl; j < n; j += gthreads) {
+                float4 q;
+                bad |= stage_cell(a, j, raw[j], raw[n + j], raw[2 * n + j], 16 * R, q);
+                cells[j] = q;
+            }
+        } else {
 #pragma unroll 4
-        for (int j = gl; j < n; j += gthreads) {
-            float4 q;
-            bad |= stage_cell(a, j, __ldcs(a.n_hi + g0 + j), __ldcs(a.b + g0 + j), __ldcs(a.v + g0 + j), 16 * R, q);
-            cells[j] = q;
+            for (int j = gl; j < n; j += gthreads) {
+                float4 q;
+                bad |= stage_cell(a, j, __ldcs(a.n_hi + g0 + j), __ldcs(a.b + g0 + j), __ldcs(a.v + g0 + j), 16 * R, q);
+                cells[j] = q;
+            }
         }
         bad = __any_sync(0xffffffffu, bad);
+        if (gl == 0) ctl[1] = 0;
+        group_sync(G, bar_id);                           // cells complete, raw consumed, ctl[0] read
         if (G > 1 && bad && lane == 0) ctl[1] = 1;
-        group_sync(G, bar_id);
-        if (G > 1) bad = ctl[1];
+        if (gl == 0) {                                   // claim the next row and start fetching it
+            const unsigned int nx = atomicAdd(&a.sched[0], 1u);
+            ctl[2] = (int)nx;
+            if (PF && (long long)nx < a.n_sl) prefetch(nx);
+        }
+        if (G > 1) {
+            group_sync(G, bar_id);
+            bad = ctl[1];
+        }
 
         // ---- sum: the group's warps take the pixel tiles of the row
         for (int tile = wg; tile < a.tiles; tile += G) {
@@ -216,7 +292,9 @@ __global__ void __launch_bounds__(1024, 1) tau_x_kernel(const TauArgs a, const i
                     if (i + r < n) dst[r] = acc[r];
             }
         }
-        group_sync(G, bar_id);                           // cells and ctl consumed
+        group_sync(G, bar_id);                           // cells consumed by every warp of the group
+        if (gl == 0) ctl[0] = ctl[2];
+        group_sync(G, bar_id);
     }
 
     // the last group to finish re-arms the row counter for the next launch on this ctx
@@ -285,18 +363,22 @@ __global__ void __launch_bounds__(TAU_THREADS) tau_strided_kernel(const TauArgs 
     }
 }
 
-template <int R>
+template <int R, int PF>
 lya_status launch_x(lya_ctx *ctx, const TauArgs &a)
 {
-    auto kern = tau_x_kernel<R>;
+    auto kern = tau_x_kernel<R, PF>;
     const size_t cap = (size_t)ctx->max_smem_optin;
-    const size_t per_group = (size_t)a.n * sizeof(float4) + 16;
+    const size_t per_group = (size_t)a.n * (sizeof(float4) + (PF ? 3 * sizeof(float) : 0)) + 16 + 8;
     int groups = (int)(cap / per_group);                 // groups that fit in one SM's shared memory
-    if (groups < 1) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: sightline too long for shared memory");
-    // G warps per group: as few as keep >= 24 warps resident and no more than the row has tiles
+    if (groups < 1) {
+        if (PF) return launch_x<R, 0>(ctx, a);           // very long rows: give the raw buffer up
+        return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: sightline too long for shared memory");
+    }
+    // G warps per group: as few as keep >= 24 warps resident, never more than the row has tiles
     int G = 1;
     while (G < 16 && G * (groups < 32 / G ? groups : 32 / G) < 24 && 2 * G <= a.tiles) G *= 2;
     if (groups > 32 / G) groups = 32 / G;
+    if (G > 1 && groups > 16) groups = 16;               // 16 named barriers per CTA
     // one persistent CTA per SM; never more groups than rows
     long long want = (a.n_sl + ctx->sm_count - 1) / ctx->sm_count;
     if (groups > want) groups = (int)(want < 1 ? 1 : want);
@@ -337,8 +419,8 @@ lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
     a.n_hi = n_hi; a.b = b; a.v = v; a.tau = tau;
     const int n = axis == 0 ? nx : (axis == 1 ? ny : nz_local);
     a.n = n;
-    a.inv_dv    = 1.0 / dv_kms;
-    a.inv_n_d   = 1.0 / (double)n;
+    a.inv_dv_hi = (float)(1.0 / dv_kms);
+    a.inv_dv_lo = (float)(1.0 / dv_kms - (double)a.inv_dv_hi);
     a.amp_scale = (float)amp_scale;
     a.w_scale   = (float)(dv_kms * 1.2011224087864498);   // sqrt(log2 e)
     a.n_f = (float)n;
@@ -352,10 +434,13 @@ lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
         if (a.n_sl >= (1LL << 31)) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: more than 2^31 sightlines");
         a.vec = (n % 4 == 0) && (((uintptr_t)tau & 15) == 0);
         a.sched = ctx->d_sched;
+        // bulk copies need 16-byte aligned rows of a multiple of 16 bytes
+        bool pf = (n % 4 == 0) && ((((uintptr_t)n_hi | (uintptr_t)b | (uintptr_t)v) & 15) == 0);
+        if (getenv("LYA_TAU_PF")) pf = pf && atoi(getenv("LYA_TAU_PF"));   // TEMP experiment switch
         switch (R) {
-            case 1:  return launch_x<1>(ctx, a);
-            case 2:  return launch_x<2>(ctx, a);
-            default: return launch_x<4>(ctx, a);
+            case 1:  return pf ? launch_x<1, 1>(ctx, a) : launch_x<1, 0>(ctx, a);
+            case 2:  return pf ? launch_x<2, 1>(ctx, a) : launch_x<2, 0>(ctx, a);
+            default: return pf ? launch_x<4, 1>(ctx, a) : launch_x<4, 0>(ctx, a);
         }
     }
 
