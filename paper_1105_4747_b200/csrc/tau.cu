@@ -5,7 +5,7 @@
 //
 // Every (i,j) pair is evaluated (N^2 per sightline): the kernel is bound by MUFU.EX2 (16 /clk/SM, measured),
 // and on sm_100a every extra FP32 instruction per pair costs MUFU rate long before the issue limit
-// (profiles/r1_tau_loop_probe.md), so the pair body is 3.25 FP32 instructions + 1 MUFU:
+// ("pair loop"), so the pair body is 3.25 FP32 instructions + 1 MUFU:
 //
 //   staged per source cell j (once per sightline, in shared memory, one float4):
 //       m_j = j + P_j          P_j = round(v_pec/dv), reduced mod N          (integer-valued float, exact)
@@ -30,7 +30,7 @@
 // per-pair image choice.  Both loops evaluate all N^2 pairs.
 //
 // Mapping, sightlines along x (contiguous rows): a GROUP of G warps (G = 1 unless the row is too long for
-// enough groups to fit in shared memory) owns one sightline at a time: it stages the row with 128-bit
+// enough groups to fit in shared memory) owns one sightline at a time: it stages the row with 128-byte
 // coalesced loads straight into its private float4 cells, syncs only itself (named barrier / __syncwarp),
 // sums its tiles and stores R consecutive tau values per lane (128-bit).  Groups never wait for each other,
 // so the MUFU pipe always has warps in the pair loop while others stage; rows are handed out by a global
@@ -38,8 +38,6 @@
 // ~6,000 resident warps would lose 8 %).
 // Sightlines along y / z: a CTA gathers 8 (or fewer) neighbouring x at a time so that global accesses stay
 // 32-byte segments, its 8 warps sum (sightline, tile) items, and tau goes back through a shared-memory tile.
-#include <stdlib.h>
-
 #include "lya_internal.h"
 
 namespace {
@@ -77,26 +75,35 @@ __device__ __forceinline__ float ex2_ftz(float x)
     return y;
 }
 
+// round to nearest integer on the FP32 pipe (valid for |x| < 2^22; MUFU/XU-pipe FRND would compete with ex2)
+__device__ __forceinline__ float round_magic(float x)
+{
+    const float big = 12582912.0f;                     // 1.5 * 2^23
+    return __fsub_rn(__fadd_rn(x, big), big);
+}
+
 // One source cell -> staged float4 (m, w, g, a); returns 1 if the cell breaks the fast-path condition.
-// All fp32: p = v_pec/dv is split as P + f with P = rint(v * inv_dv_hi) and f = fma(v, inv_dv_hi, -P) +
+// All fp32: p = v_pec/dv is split as P + f with P = round(v * inv_dv_hi) and f = fma(v, inv_dv_hi, -P) +
 // v * inv_dv_lo -- the fma forms the residual of the exact 48-bit product with ONE rounding of a number
-// below 1, so f carries an absolute error < 1e-7 pixel however large P is (|P| < 2^23 assumed: |v_pec| <
-// 8e6 dv).  No FP64 instruction is needed (reading C11: +v -> higher pixel index).
-__device__ __forceinline__ int stage_cell(const TauArgs &a, int j, float nh, float bb, float vv, int half_span,
+// below 1, so f carries an absolute error < 1e-7 pixel however large P is.  Precondition |v_pec| < 2^22 dv
+// (4e6 pixels; beyond it P is no longer an integer and the cell is sent to the general path with a
+// meaningless but finite displacement).  No FP64 and, apart from one reciprocal, no XU-pipe instruction.
+// jf = (float)j.  Reading C11: +v -> higher pixel index.
+__device__ __forceinline__ int stage_cell(const TauArgs &a, float jf, float nh, float bb, float vv, int half_span,
                                           float4 &out)
 {
-    const float P  = rintf(vv * a.inv_dv_hi);
+    const float P  = round_magic(vv * a.inv_dv_hi);
     const float f  = fmaf(vv, a.inv_dv_lo, fmaf(vv, a.inv_dv_hi, -P));
     // integer displacement reduced to [-N/2, N/2]; at an exact half-way point either image is nearest
-    const float Pr = fmaf(-a.n_f, rintf(P * a.inv_n), P);
+    const float Pr = fmaf(-a.n_f, round_magic(P * a.inv_n), P);
     const float ib = 1.0f / bb;
     const float w  = a.w_scale * ib;
-    out.x = (float)j + Pr;
+    out.x = jf + Pr;
     out.y = w;
     out.z = -f * w;
     out.w = (a.amp_scale * nh) * ib;
     const float room = (float)(a.n >> 1) - (float)half_span - fabsf(Pr) - 1.0f;
-    return !(room * w >= TAU_XCUT);
+    return !(room * w >= TAU_XCUT) || !(fabsf(P) < 4194304.0f);
 }
 
 // Fast path: unwrapped walk around the tile centre, no per-pair image logic.  Lane owns pixels
@@ -166,109 +173,46 @@ __device__ __forceinline__ void group_sync(int G, int bar_id)
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// mbarrier / bulk-copy helpers (SASS: SYNCS, UBLKCP)
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_%=:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra DONE_%=;\n"
-        "bra WAIT_%=;\n"
-        "DONE_%=:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-// 1-D bulk copy global -> shared, completion signalled on an mbarrier
-__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
-}
-
-// Sightlines along x.  blockDim = 32 * G * gpc (gpc = groups per CTA).  Dynamic shared memory, per group:
-// n float4 cells [+ PF: 3 n floats of raw nHI | b | v_pec, filled by cp.async.bulk], then per group one
-// int4 control word {row, bad, next row, -} and (PF) one mbarrier.
-// PF = 1 (rows 16-byte aligned, n % 4 == 0): the NEXT row's three input rows are bulk-copied into the
-// group's raw buffer while the current row is being summed, so a row change costs only the conversion
-// raw -> cells.  PF = 0: plain coalesced loads at the row change.
-template <int R, int PF>
+// Sightlines along x.  blockDim = 32 * G * gpc (gpc = groups per CTA).  Dynamic shared memory: per group n
+// float4 cells, then per group one int4 control word {row, bad, next row, -}.
+// (A variant that bulk-copied the next row into a raw buffer with cp.async.bulk + mbarrier while the current
+// one was summed measured 4 % slower: profiles/r1_tau_prefetch_ab.md.  The row change here is plain coalesced
+// loads; the other resident groups keep the MUFU pipe busy meanwhile.)
+template <int R>
 __global__ void __launch_bounds__(1024, 1) tau_x_kernel(const TauArgs a, const int G, const int gpc)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int grp = warp / G, wg = warp - grp * G;       // group in CTA, warp in group
     const int n = a.n;
-    const size_t cell_bytes = (size_t)n * (sizeof(float4) + (PF ? 3 * sizeof(float) : 0));
-    float4 *cells = reinterpret_cast<float4 *>(smem + (size_t)grp * cell_bytes);
-    float *raw = reinterpret_cast<float *>(cells + n);   // PF only
-    unsigned char *tail = smem + (size_t)gpc * cell_bytes;
-    volatile int *ctl = reinterpret_cast<volatile int *>(tail) + 4 * grp;
-    uint64_t *mbar = reinterpret_cast<uint64_t *>(tail + (size_t)gpc * 16) + grp;   // PF only
+    float4 *cells = reinterpret_cast<float4 *>(smem) + (size_t)grp * n;
+    volatile int *ctl = reinterpret_cast<volatile int *>(smem + (size_t)gpc * n * sizeof(float4)) + 4 * grp;
     const int bar_id = grp;      // named barrier of the group (G >= 2: at most 16 groups; no __syncthreads here)
     const int gl = wg * 32 + lane, gthreads = G * 32;    // thread index / count inside the group
-    const uint32_t row_bytes = (uint32_t)n * 4u;
 
-    auto prefetch = [&](long long row) {                 // one thread of the group
-        const size_t g = (size_t)row * n;
-        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // raw was read through the generic proxy
-        mbar_expect_tx(mbar, 3u * row_bytes);
-        bulk_g2s(raw,         a.n_hi + g, row_bytes, mbar);
-        bulk_g2s(raw + n,     a.b + g,    row_bytes, mbar);
-        bulk_g2s(raw + 2 * n, a.v + g,    row_bytes, mbar);
-    };
-
-    if (gl == 0) {
-        const unsigned int r0 = atomicAdd(&a.sched[0], 1u);
-        ctl[0] = (int)r0;
-        if (PF) {
-            mbar_init(mbar, 1);
-            asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-            if ((long long)r0 < a.n_sl) prefetch(r0);
-        }
-    }
+    if (gl == 0) ctl[0] = (int)atomicAdd(&a.sched[0], 1u);
     group_sync(G, bar_id);
 
-    for (uint32_t it = 0;; ++it) {
+    for (;;) {
         const long long row = (unsigned int)ctl[0];
         if (row >= a.n_sl) break;
         const size_t g0 = (size_t)row * n;
 
-        // ---- stage the row: (nHI, b, v_pec) -> (m, w, g, a) per cell
+        // ---- stage the row: (nHI, b, v_pec) -> (m, w, g, a) per cell; 128-byte coalesced loads
         int bad = 0;
-        if (PF) {
-            mbar_wait(mbar, it & 1u);
-            for (int j = gl; j < n; j += gthreads) {
-                float4 q;
-                bad |= stage_cell(a, j, raw[j], raw[n + j], raw[2 * n + j], 16 * R, q);
-                cells[j] = q;
-            }
-        } else {
+        float jf = (float)gl;
 #pragma unroll 4
-            for (int j = gl; j < n; j += gthreads) {
-                float4 q;
-                bad |= stage_cell(a, j, __ldcs(a.n_hi + g0 + j), __ldcs(a.b + g0 + j), __ldcs(a.v + g0 + j), 16 * R, q);
-                cells[j] = q;
-            }
+        for (int j = gl; j < n; j += gthreads) {
+            float4 q;
+            bad |= stage_cell(a, jf, __ldcs(a.n_hi + g0 + j), __ldcs(a.b + g0 + j), __ldcs(a.v + g0 + j), 16 * R, q);
+            cells[j] = q;
+            jf += (float)gthreads;
         }
         bad = __any_sync(0xffffffffu, bad);
         if (gl == 0) ctl[1] = 0;
-        group_sync(G, bar_id);                           // cells complete, raw consumed, ctl[0] read
+        group_sync(G, bar_id);                           // cells complete, ctl[0] read
         if (G > 1 && bad && lane == 0) ctl[1] = 1;
-        if (gl == 0) {                                   // claim the next row and start fetching it
-            const unsigned int nx = atomicAdd(&a.sched[0], 1u);
-            ctl[2] = (int)nx;
-            if (PF && (long long)nx < a.n_sl) prefetch(nx);
-        }
+        if (gl == 0) ctl[2] = (int)atomicAdd(&a.sched[0], 1u);   // claim the next row early: latency hidden
         if (G > 1) {
             group_sync(G, bar_id);
             bad = ctl[1];
@@ -334,7 +278,7 @@ __global__ void __launch_bounds__(TAU_THREADS) tau_strided_kernel(const TauArgs 
             if (bx < nb) {
                 const long long g = base + (long long)j * a.stride + bx;
                 float4 q;
-                bad |= stage_cell(a, j, __ldcs(a.n_hi + g), __ldcs(a.b + g), __ldcs(a.v + g), 16 * R, q);
+                bad |= stage_cell(a, (float)j, __ldcs(a.n_hi + g), __ldcs(a.b + g), __ldcs(a.v + g), 16 * R, q);
                 cells[bx * cstride + j] = q;
             }
         }
@@ -363,17 +307,14 @@ __global__ void __launch_bounds__(TAU_THREADS) tau_strided_kernel(const TauArgs 
     }
 }
 
-template <int R, int PF>
+template <int R>
 lya_status launch_x(lya_ctx *ctx, const TauArgs &a)
 {
-    auto kern = tau_x_kernel<R, PF>;
+    auto kern = tau_x_kernel<R>;
     const size_t cap = (size_t)ctx->max_smem_optin;
-    const size_t per_group = (size_t)a.n * (sizeof(float4) + (PF ? 3 * sizeof(float) : 0)) + 16 + 8;
+    const size_t per_group = (size_t)a.n * sizeof(float4) + 16;
     int groups = (int)(cap / per_group);                 // groups that fit in one SM's shared memory
-    if (groups < 1) {
-        if (PF) return launch_x<R, 0>(ctx, a);           // very long rows: give the raw buffer up
-        return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: sightline too long for shared memory");
-    }
+    if (groups < 1) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: sightline too long for shared memory");
     // G warps per group: as few as keep >= 24 warps resident, never more than the row has tiles
     int G = 1;
     while (G < 16 && G * (groups < 32 / G ? groups : 32 / G) < 24 && 2 * G <= a.tiles) G *= 2;
@@ -434,13 +375,10 @@ lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
         if (a.n_sl >= (1LL << 31)) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: more than 2^31 sightlines");
         a.vec = (n % 4 == 0) && (((uintptr_t)tau & 15) == 0);
         a.sched = ctx->d_sched;
-        // bulk copies need 16-byte aligned rows of a multiple of 16 bytes
-        bool pf = (n % 4 == 0) && ((((uintptr_t)n_hi | (uintptr_t)b | (uintptr_t)v) & 15) == 0);
-        if (getenv("LYA_TAU_PF")) pf = pf && atoi(getenv("LYA_TAU_PF"));   // TEMP experiment switch
         switch (R) {
-            case 1:  return pf ? launch_x<1, 1>(ctx, a) : launch_x<1, 0>(ctx, a);
-            case 2:  return pf ? launch_x<2, 1>(ctx, a) : launch_x<2, 0>(ctx, a);
-            default: return pf ? launch_x<4, 1>(ctx, a) : launch_x<4, 0>(ctx, a);
+            case 1:  return launch_x<1>(ctx, a);
+            case 2:  return launch_x<2>(ctx, a);
+            default: return launch_x<4>(ctx, a);
         }
     }
 
