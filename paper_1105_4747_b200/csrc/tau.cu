@@ -37,7 +37,8 @@
 // atomic counter, which removes the wave-quantisation tail of a static partition (65,536 rows over
 // ~6,000 resident warps would lose 8 %).
 // Sightlines along y / z: a CTA gathers 8 (or fewer) neighbouring x at a time so that global accesses stay
-// 32-byte segments, its 8 warps sum (sightline, tile) items, and tau goes back through a shared-memory tile.
+// 32- or 16-byte segments, its 8 warps sum (sightline, tile) items, and tau goes back through a shared-memory
+// tile; batches come from the same atomic counter.
 #include "lya_internal.h"
 
 namespace {
@@ -54,6 +55,8 @@ struct TauArgs {
     int          vec;         // x-axis: rows are 16-byte aligned and n % 4 == 0
     int          bsl;         // strided: x-width of a gathered batch (power of 2)
     int          bshift;      // log2(bsl)
+    int          cstride;     // strided: float4 cells per staged sightline (n + pad)
+    int          tstride;     // strided: floats per sightline of the tau tile (tiles*32*R + pad)
     long long    n_sl;        // x-axis: number of sightlines (rows)
     long long    n_batches;   // strided: number of gathered batches
     unsigned int *sched;      // x-axis: [0] next row, [1] groups finished (self-resetting)
@@ -254,18 +257,28 @@ __global__ void __launch_bounds__(1024, 1) tau_x_kernel(const TauArgs a, const i
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// Sightlines along y or z, gathered bsl neighbouring x at a time (persistent CTAs, static batches).
+// Sightlines along y or z.  A CTA (8 warps) gathers bsl neighbouring x at a time so that global accesses are
+// 4*bsl-byte segments (the sibling batches run at the same time on other CTAs, so L2 serves the rest of each
+// sector), its warps sum (sightline, tile) items, and tau goes back through a shared-memory tile the same
+// way.  Batches are handed out by the atomic counter; bsl is chosen so that >= 4 CTAs are resident per SM and
+// one CTA's gather overlaps the others' pair loops.  cstride / tstride are padded so that neither the
+// transposed staging stores nor the tile read-out have shared-memory bank conflicts.
 template <int R>
 __global__ void __launch_bounds__(TAU_THREADS) tau_strided_kernel(const TauArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem[];
+    __shared__ unsigned int s_batch;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int n = a.n;
-    const int cstride = n + 1;                           // +1 cell: conflict-free transposed staging
-    float4 *cells = reinterpret_cast<float4 *>(smem);
-    float *ttile = reinterpret_cast<float *>(smem + (size_t)a.bsl * cstride * sizeof(float4));   // [n][bsl]
+    const int cstride = a.cstride, tstride = a.tstride;
+    float4 *cells = reinterpret_cast<float4 *>(smem);                                          // [bsl][cstride]
+    float *ttile = reinterpret_cast<float *>(smem + (size_t)a.bsl * cstride * sizeof(float4)); // [bsl][tstride]
 
-    for (long long batch = blockIdx.x; batch < a.n_batches; batch += gridDim.x) {
+    if (tid == 0) s_batch = atomicAdd(&a.sched[0], 1u);
+    __syncthreads();
+    for (;;) {
+        const long long batch = s_batch;
+        if (batch >= a.n_batches) break;
         const long long outer = batch / a.nxb;
         const int xb = (int)(batch - outer * a.nxb);
         const int x0 = xb << a.bshift;
@@ -273,6 +286,7 @@ __global__ void __launch_bounds__(TAU_THREADS) tau_strided_kernel(const TauArgs 
         const long long base = outer * a.outer_stride + x0;   // element offset of (pixel 0, first x of the batch)
 
         int bad = 0;
+#pragma unroll 4
         for (int c = tid; c < (n << a.bshift); c += TAU_THREADS) {
             const int bx = c & (a.bsl - 1), j = c >> a.bshift;
             if (bx < nb) {
@@ -282,7 +296,8 @@ __global__ void __launch_bounds__(TAU_THREADS) tau_strided_kernel(const TauArgs 
                 cells[bx * cstride + j] = q;
             }
         }
-        bad = __syncthreads_or(bad);
+        bad = __syncthreads_or(bad);                     // cells complete; s_batch read by everyone
+        if (tid == 0) s_batch = atomicAdd(&a.sched[0], 1u);
 
         const int items = nb * a.tiles;
         for (int item = warp; item < items; item += TAU_WARPS) {
@@ -292,18 +307,27 @@ __global__ void __launch_bounds__(TAU_THREADS) tau_strided_kernel(const TauArgs 
             float acc[R];
             if (!bad) tile_fast<R>(cs, n, i0, lane, acc);
             else      tile_general<R>(cs, n, a.n_f, a.inv_n, i0, lane, acc);
-#pragma unroll
-            for (int r = 0; r < R; ++r) {
-                const int i = i0 + lane * R + r;
-                if (i < n) ttile[(i << a.bshift) + sl] = acc[r];
-            }
+            const int i = i0 + lane * R;
+            float *dst = ttile + (size_t)sl * tstride + i;     // tstride covers tiles * 32 * R: no bound check
+            if (R == 4)      *reinterpret_cast<float4 *>(dst) = make_float4(acc[0], acc[1], acc[2], acc[3]);
+            else if (R == 2) *reinterpret_cast<float2 *>(dst) = make_float2(acc[0], acc[1]);
+            else             dst[0] = acc[0];
         }
-        __syncthreads();                                 // cells consumed, tau tile complete
+        __syncthreads();                                 // cells consumed, tau tile complete, s_batch written
         for (int c = tid; c < (n << a.bshift); c += TAU_THREADS) {
             const int bx = c & (a.bsl - 1), j = c >> a.bshift;
-            if (bx < nb) __stcs(a.tau + base + (long long)j * a.stride + bx, ttile[c]);
+            if (bx < nb) __stcs(a.tau + base + (long long)j * a.stride + bx, ttile[bx * tstride + j]);
         }
-        __syncthreads();
+        __syncthreads();                                 // tile read out before the next batch's sums
+    }
+
+    if (tid == 0) {                                      // the last CTA re-arms the counter
+        __threadfence();
+        if (atomicAdd(&a.sched[1], 1u) == gridDim.x - 1u) {
+            a.sched[0] = 0u;
+            a.sched[1] = 0u;
+            __threadfence();
+        }
     }
 }
 
@@ -387,15 +411,32 @@ lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
     a.stride = axis == 1 ? (long long)nx : (long long)nx * ny;
     a.outer_stride = axis == 1 ? (long long)nx * ny : (long long)nx;
     const long long n_outer = axis == 1 ? nz_local : ny;
-    int bshift = 3;
-    auto need2 = [&](int sh) { return ((size_t)(n + 1) * 16 + (size_t)n * 4) << sh; };
-    while (bshift > 0 && need2(bshift) > smem_cap / 2) --bshift;
+    // per staged sightline: cstride float4 cells + tstride floats of tau tile; strides padded against bank
+    // conflicts: cstride = 8/bsl (mod 8) float4s for the transposed STS.128, tstride = 32/bsl (mod 32) floats
+    // for the read-out (both trivially fine for bsl = 1)
+    auto pad_to = [](int v, int mod, int want) { return v + ((want - v % mod) % mod + mod) % mod; };
+    auto strides = [&](int sh, int &cs, int &ts) {
+        const int bs = 1 << sh;
+        cs = pad_to(n, 8, (8 / bs) % 8);
+        ts = pad_to(a.tiles * 32 * R, 32, (32 / bs) % 32);
+    };
+    auto need2 = [&](int sh) {
+        int cs, ts;
+        strides(sh, cs, ts);
+        return ((size_t)cs * 16 + (size_t)ts * 4) << sh;
+    };
+    int bshift = 3;                                      // 32-byte segments if >= 4 CTAs still fit per SM
+    while (bshift > 1 && 4 * (need2(bshift) + 1024) > smem_cap) --bshift;
+    while (bshift > 0 && need2(bshift) > smem_cap) --bshift;
     if (need2(bshift) > smem_cap)
         return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: sightline too long for shared memory");
     a.bshift = bshift;
     a.bsl = 1 << bshift;
+    strides(bshift, a.cstride, a.tstride);
     a.nxb = (nx + a.bsl - 1) / a.bsl;
     a.n_batches = n_outer * a.nxb;
+    if (a.n_batches >= (1LL << 31)) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: more than 2^31 batches");
+    a.sched = ctx->d_sched;
     switch (R) {
         case 1:  return launch_strided<1>(ctx, a, need2(bshift));
         case 2:  return launch_strided<2>(ctx, a, need2(bshift));
