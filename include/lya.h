@@ -143,6 +143,11 @@ lya_status lya_forest_host(lya_ctx *ctx, const lya_params *p, int axis, int32_t 
                            float *tau_h, float *flux_h,
                            double *a_out, double *f_achieved, int *iters);
 
+/* Roofline denominator of the tau kernel (BASELINE.json: "MUFU.EX2 ... issue rate from SM count x clock"):
+ * runs a pure ex2.approx micro-kernel on every SM of ctx's device and returns MUFU.EX2 results per second
+ * (HOST double; best of 3 after a warm-up).  Synchronises the stream.  16 / clk / SM on B200. */
+lya_status lya_measure_mufu_peak(lya_ctx *ctx, double *ex2_per_s);
+
 /* Number of kernels the library has launched on this ctx since creation (bench.py's gpu_launches). */
 uint64_t lya_launch_count(const lya_ctx *ctx);
 

@@ -73,7 +73,7 @@ class Params:
 EXPORTS = ("lya_version", "lya_status_string", "lya_scalars_from_params", "lya_create", "lya_destroy",
            "lya_last_error", "lya_sm_count", "lya_gas_from_density", "lya_tau_sightlines",
            "lya_normalize_mean_flux", "lya_flux_partial_sums", "lya_root_init", "lya_root_update",
-           "lya_flux", "lya_forest_host", "lya_launch_count")
+           "lya_flux", "lya_forest_host", "lya_launch_count", "lya_measure_mufu_peak")
 
 _lib = None
 
@@ -108,6 +108,7 @@ def lib() -> C.CDLL:
     L.lya_flux.argtypes = [vp, fp, C.c_size_t, C.c_double, fp]
     L.lya_forest_host.argtypes = [vp, pp, C.c_int, C.c_int32, fp, fp, C.c_double, C.c_double, C.c_int,
                                   fp, fp, dp, dp, ip]
+    L.lya_measure_mufu_peak.argtypes = [vp, dp]
     _lib = L
     return L
 
@@ -167,6 +168,12 @@ class Context:
     @property
     def launch_count(self) -> int:
         return int(lib().lya_launch_count(self._h))
+
+    def measure_mufu_peak(self) -> float:
+        """MUFU.EX2 results per second of this device (the tau kernel's roofline denominator)."""
+        r = C.c_double()
+        self._check(lib().lya_measure_mufu_peak(self._h, C.byref(r)))
+        return r.value
 
     # S1
     def gas_from_density(self, p: Params, delta: torch.Tensor, n_hi=None, b_kms=None):

@@ -1,0 +1,70 @@
+"""N > 1 path on CPU (gloo, world_size 2): the sharded normalisation of DESIGN.md "Multi-GPU".
+
+Each rank owns half of the pixels; per pass the ranks all-reduce (sum exp(-A tau), sum tau exp(-A tau)) -- two
+doubles -- and apply the library's host-side scalar update lya_root_update, so every rank must end with the
+same A, equal to the oracle's bisection over ALL pixels.  The per-rank partial sums, which the product takes
+from the CUDA kernel behind lya_flux_partial_sums, are stood in for here by numpy (test-only) because this
+container has no GPU; everything else (init, all-reduce, update, stopping rule) is the product's code.
+"""
+import os
+import socket
+
+import numpy as np
+import pytest
+import torch
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+
+def _free_port() -> int:
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        return s.getsockname()[1]
+
+
+def _worker(rank: int, world: int, port: int, f_target: float, out_path: str):
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    from paper_1105_4747_b200 import lya
+    rng = np.random.default_rng(4747)                          # same stream on both ranks, split below
+    tau_all = rng.lognormal(mean=-1.0, sigma=1.2, size=200_003).astype(np.float32)
+    lo, hi = (0, 120_000) if rank == 0 else (120_000, tau_all.size)   # uneven shards on purpose
+    tau = tau_all[lo:hi].astype(np.float64)
+
+    def partial_sums(a):
+        e = np.exp(-a * tau)
+        return [float(e.sum())], [float((tau * e).sum())]
+
+    A, f, iters = lya.normalize_mean_flux_sharded(None, None, f_target, tau_all.size, rel_tol=1e-10,
+                                                  partial_sums=partial_sums)
+    got = torch.tensor([A, f, float(iters)], dtype=torch.float64)
+    gathered = [torch.zeros_like(got) for _ in range(world)]
+    dist.all_gather(gathered, got)
+    if rank == 0:
+        np.save(out_path, np.stack([g.numpy() for g in gathered]))
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("f_target", [0.80, 0.35])
+def test_sharded_normalisation_two_ranks_gloo(tmp_path, oracle, f_target):
+    out = str(tmp_path / "res.npy")
+    mp.spawn(_worker, args=(2, _free_port(), f_target, out), nprocs=2, join=True)
+    res = np.load(out)
+    assert np.array_equal(res[0], res[1]), "ranks disagree on (A, <F>, passes)"
+    A, f, iters = res[0]
+    rng = np.random.default_rng(4747)
+    tau_all = rng.lognormal(mean=-1.0, sigma=1.2, size=200_003).astype(np.float32).astype(np.float64)
+    A_ref, f_ref, _ = oracle.normalize_mean_flux(tau_all, f_target)
+    assert abs(A / A_ref - 1.0) < 1e-8
+    assert abs(f - f_target) < 1e-9 and iters <= 20
+
+
+def test_sharded_weak_scaling_slabs_are_independent_problems():
+    """bench.py's N > 1 layout: rank r generates ITS slab from (seed + 100 r): no rank needs another's cells."""
+    from paper_1105_4747_b200 import inputs
+    from paper_1105_4747_b200.workloads import WORKLOADS, Workload, scaled
+    w = scaled(WORKLOADS[1], 32)
+    w1 = Workload(**{**w.as_dict(), "axes": tuple(w.axes), "cfg": w.cfg + 100})
+    a = inputs.make_fields(w, device="cpu", z0=0, z1=4)["delta"]
+    b = inputs.make_fields(w1, device="cpu", z0=0, z1=4)["delta"]
+    assert a.shape == b.shape == (4, 32, 32) and not torch.equal(a, b)
