@@ -28,20 +28,37 @@ __device__ __forceinline__ void gas_cell(const GasK &k, float delta, float &n_hi
     n_hi = (k.nbar_hi * exp2f(k.e_n * l)) * (D * D);
 }
 
+__device__ __forceinline__ void gas_cell4(const GasK &k, const float4 &d, float4 &n, float4 &w)
+{
+    gas_cell(k, d.x, n.x, w.x);
+    gas_cell(k, d.y, n.y, w.y);
+    gas_cell(k, d.z, n.z, w.z);
+    gas_cell(k, d.w, n.w, w.w);
+}
+
+// two independent 128-bit loads in flight per thread and iteration; streaming (evict-first) loads and stores
 __global__ void __launch_bounds__(256) gas_vec4_kernel(const float4 *__restrict__ delta, size_t n4,
                                                        float4 *__restrict__ n_hi, float4 *__restrict__ b,
                                                        GasK k)
 {
-    size_t stride = (size_t)gridDim.x * blockDim.x;
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n4; i += stride) {
-        float4 d = __ldcs(delta + i);           // streamed once
-        float4 n, w;
-        gas_cell(k, d.x, n.x, w.x);
-        gas_cell(k, d.y, n.y, w.y);
-        gas_cell(k, d.z, n.z, w.z);
-        gas_cell(k, d.w, n.w, w.w);
-        n_hi[i] = n;
-        b[i]    = w;
+    const size_t stride = (size_t)gridDim.x * blockDim.x;
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    for (; i + stride < n4; i += 2 * stride) {
+        const float4 d0 = __ldcs(delta + i), d1 = __ldcs(delta + i + stride);
+        float4 n0, w0, n1, w1;
+        gas_cell4(k, d0, n0, w0);
+        gas_cell4(k, d1, n1, w1);
+        __stcs(n_hi + i, n0);
+        __stcs(b + i, w0);
+        __stcs(n_hi + i + stride, n1);
+        __stcs(b + i + stride, w1);
+    }
+    if (i < n4) {
+        const float4 d0 = __ldcs(delta + i);
+        float4 n0, w0;
+        gas_cell4(k, d0, n0, w0);
+        __stcs(n_hi + i, n0);
+        __stcs(b + i, w0);
     }
 }
 
