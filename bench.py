@@ -107,41 +107,72 @@ def bench_ours(args) -> dict:
     n = w.n
     pk = peaks()
 
-    # inputs: rank r owns planes of its own seeded 256-plane slab (weak scaling: independent slabs of one
-    # N*n-plane grid; complete x-rows, so S1-S3 and S5 need no exchange)
+    # inputs: rank r owns planes of its own seeded slab (weak scaling: independent slabs of one N*n-plane grid;
+    # complete x-rows, so S1-S3 and S5 need no exchange).  Config 5 (32 GiB per field) is generated and
+    # processed in z-slabs: delta, v_pec and tau stay resident (96 GiB), n_HI / b exist for one slab at a time
+    # and F overwrites tau.
     wl = w if world == 1 else Workload(**{**w.as_dict(), "axes": tuple(w.axes), "cfg": w.cfg + 100 * rank})
-    fields = inputs.make_fields(wl, device="cuda")
-    delta = fields["delta"]
-    vels = [fields["v_pec"][ax] for ax in w.axes]
+    slab_nz = 64 if w.cfg == 5 else n
+    if w.cfg == 5:
+        delta = torch.empty((n, n, n), dtype=torch.float32, device="cuda")
+        vels = [torch.empty_like(delta)]
+        for z0 in range(0, n, 32):
+            f = inputs.make_fields(wl, device="cuda", z0=z0, z1=z0 + 32)
+            delta[z0:z0 + 32] = f["delta"]
+            vels[0][z0:z0 + 32] = f["v_pec"][w.axes[0]]
+            del f
+    else:
+        fields = inputs.make_fields(wl, device="cuda")
+        delta = fields["delta"]
+        vels = [fields["v_pec"][ax] for ax in w.axes]
     p = lya.Params.from_workload(w)
     ctx = lya.Context(local)
-    n_hi, b = torch.empty_like(delta), torch.empty_like(delta)
-    tau, flux = torch.empty_like(delta), torch.empty_like(delta)
+    n_hi, b = (torch.empty((slab_nz, n, n), dtype=torch.float32, device="cuda") for _ in range(2))
+    tau = torch.empty_like(delta)
+    flux = tau if w.cfg == 5 else torch.empty_like(delta)
     n_cells = delta.numel()
+    n_slabs = n // slab_nz
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")       # > 126 MB L2
 
     ev = lambda: torch.cuda.Event(enable_timing=True)
     results = {}
 
     def step(timers=None):
-        """S1 once, then S2-S5 per sightline axis (config 3 has three; the others one)."""
-        t = [ev() for _ in range(2 + 3 * len(w.axes))] if timers is not None else None
-        if t: t[0].record()
-        ctx.gas_from_density(p, delta, n_hi, b)
-        if t: t[1].record()
+        """S1 once, then S2-S5 per sightline axis (config 3 has three; the others one).  With slabs (config 5)
+        S1 and S3 alternate per slab; the per-kernel event pairs of gas and tau bracket the FIRST slab's launch."""
+        t = {"gas": [], "tau": [], "normalize": [], "flux": []} if timers is not None else None
+
+        def timed(name, fn):
+            if t is None:
+                return fn()
+            e0, e1 = ev(), ev()
+            e0.record()
+            r = fn()
+            e1.record()
+            t[name].append((e0, e1))
+            return r
+
         for k, ax in enumerate(w.axes):
-            ctx.tau_sightlines(p, ax, n_hi, b, vels[k], tau)
-            if t: t[2 + 3 * k].record()
+            for sl in range(n_slabs):
+                z0, z1 = sl * slab_nz, (sl + 1) * slab_nz
+                run = timed if sl == 0 else (lambda name, fn: fn())
+                if k == 0 or n_slabs > 1:
+                    run("gas", lambda: ctx.gas_from_density(p, delta[z0:z1], n_hi, b))
+                run("tau", lambda: ctx.tau_sightlines(p, ax, n_hi, b, vels[k][z0:z1], tau[z0:z1]))
             if world == 1:
-                A, f, it, _ = ctx.normalize_mean_flux(tau, w.f_target, rel_tol=1e-7, max_iter=60)
+                A, f, it, _ = timed("normalize", lambda: ctx.normalize_mean_flux(tau, w.f_target, rel_tol=1e-7,
+                                                                                 max_iter=60))
             else:
-                A, f, it = lya.normalize_mean_flux_sharded(ctx, tau, w.f_target, n_cells * world, rel_tol=1e-7)
-            if t: t[3 + 3 * k].record()
-            ctx.flux(tau, A, flux)
-            if t: t[4 + 3 * k].record()
+                A, f, it = timed("normalize", lambda: lya.normalize_mean_flux_sharded(
+                    ctx, tau, w.f_target, n_cells * world, rel_tol=1e-7))
+            timed("flux", lambda: ctx.flux(tau, A, flux))
             results.update(A=A, f=f, passes=it)
         if timers is not None:
             timers.append(t)
+
+    # the oracle's sample for the cpu_baseline leg: the first >= 65536 sightlines (whole planes), copied now
+    nz_cpu = min(n, max(1, 65536 // n))
+    cpu_rows = (delta[:nz_cpu].reshape(-1, n).cpu().numpy(), vels[0][:nz_cpu].reshape(-1, n).cpu().numpy())
 
     for _ in range(max(args.warmup, 3)):
         step()
@@ -181,26 +212,24 @@ def bench_ours(args) -> dict:
     pairs_per_step = float(n) ** 4 * n_ax * world
     pix_per_step = float(n) ** 3 * n_ax * world
 
-    # per-kernel means (rank 0): gas | tau | normalize | flux
-    k_ms = {"gas": 0.0, "tau": 0.0, "normalize": 0.0, "flux": 0.0}
-    for t in timers:
-        k_ms["gas"] += t[0].elapsed_time(t[1])
-        for k in range(n_ax):
-            prev = t[1] if k == 0 else t[4 + 3 * (k - 1)]
-            k_ms["tau"] += prev.elapsed_time(t[2 + 3 * k])
-            k_ms["normalize"] += t[2 + 3 * k].elapsed_time(t[3 + 3 * k])
-            k_ms["flux"] += t[3 + 3 * k].elapsed_time(t[4 + 3 * k])
-    k_ms["gas"] /= args.steps
-    for k in ("tau", "normalize", "flux"):
-        k_ms[k] /= args.steps * n_ax                    # per launch (per axis pass)
+    # per-launch means (rank 0): gas and tau launches cover one slab (= the whole grid unless config 5)
+    k_ms = {}
+    for name in ("gas", "tau", "normalize", "flux"):
+        spans = [e0.elapsed_time(e1) for t in timers for e0, e1 in t[name]]
+        k_ms[name] = sum(spans) / len(spans)
+    slab_cells = slab_nz * n * n
 
     # ---- end to end through lya_forest_host: pinned host inputs, F read back, every step
     e2e = None
     if not args.no_e2e:
-        dh = delta.cpu().pin_memory()
-        vh = [v.cpu().pin_memory() for v in vels]
-        fh = torch.empty_like(dh).pin_memory()
-        for _ in range(2):
+        pinned = lambda src: torch.empty(src.shape, dtype=src.dtype, pin_memory=True).copy_(src)
+        dh = pinned(delta)
+        vh = [pinned(v) for v in vels]
+        fh = torch.empty(dh.shape, dtype=dh.dtype, pin_memory=True)
+        if w.cfg == 5:                                  # lya_forest_host keeps its own tau + slab workspace
+            del delta, vels, tau, flux, n_hi, b
+            torch.cuda.empty_cache()
+        for _ in range(1 if w.cfg == 5 else 2):
             ctx.forest_host(p, w.axes[0], dh, vh[0], w.f_target, flux_h=fh)
         if world > 1:
             dist.barrier()
@@ -224,7 +253,7 @@ def bench_ours(args) -> dict:
     clocks = sampler.summary(pk["sm_max_mhz"])
     mufu_measured = ctx.measure_mufu_peak()                                   # pure ex2 micro-kernel, this device
     f_peak = MUFU_PER_CLK_SM * ctx.sm_count * pk["sm_max_mhz"] * 1e6          # pair-evals/s at max SM clock
-    tau_rate = float(n) ** 4 / (k_ms["tau"] * 1e-3)
+    tau_rate = float(slab_cells) * n / (k_ms["tau"] * 1e-3)      # pairs of one launch / its duration
     hbm = pk["hbm_gbs"]
     gbs = lambda bytes_, ms: bytes_ / (ms * 1e-3) / 1e9
     passes = results["passes"]
@@ -233,12 +262,12 @@ def bench_ours(args) -> dict:
         "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step,
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": w.name, "grid": [n, n, n * world], "sightlines": n * n * world * n_ax,
-                   "pixels_per_sightline": n, "axes": list(w.axes), "f_target": w.f_target,
+                   "pixels_per_sightline": n, "axes": list(w.axes), "f_target": w.f_target, "slab_nz": slab_nz,
                    "l2": "256 MiB memset between steps (outside the event spans); working set %d MiB" %
                          (6 * 4 * n_cells >> 20),
                    "parallelism": "z-slabs per rank; S4 all-reduce of 2 doubles per pass" if world > 1 else "1 GPU"},
         "sightline_pixels_per_s": pix_per_step / (ms_per_step * 1e-3),
-        "tau_kernel_pixels_per_s": float(n) ** 3 / (k_ms["tau"] * 1e-3),
+        "tau_kernel_pixels_per_s": float(slab_cells) / (k_ms["tau"] * 1e-3),
         "A": results["A"], "mean_flux": results["f"], "normalize_passes": passes,
         "kernel_ms": k_ms, "wall_s_timed_region_incl_flush": wall,
         "roofline": {"bound": "alu", "kernel": "tau_kernel", "achieved": tau_rate / 1e9, "peak": f_peak / 1e9,
@@ -251,7 +280,7 @@ def bench_ours(args) -> dict:
                      if clocks["sm_mhz"] else None},
         "roofline_hbm": {
             "peak_gbs": hbm, "peak_src": pk["src"],
-            "gas": {"bytes": 12 * n_cells, "gbs": gbs(12 * n_cells, k_ms["gas"]), "frac": gbs(12 * n_cells, k_ms["gas"]) / hbm},
+            "gas": {"bytes": 12 * slab_cells, "gbs": gbs(12 * slab_cells, k_ms["gas"]), "frac": gbs(12 * slab_cells, k_ms["gas"]) / hbm},
             "normalize": {"bytes": 4 * n_cells * passes, "passes": passes,
                           "gbs": gbs(4 * n_cells * passes, k_ms["normalize"]),
                           "frac": gbs(4 * n_cells * passes, k_ms["normalize"]) / hbm},
@@ -259,7 +288,7 @@ def bench_ours(args) -> dict:
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "sm_count": ctx.sm_count,
     }
     if rank == 0 and world == 1 and not args.no_cpu:
-        out["cpu_baseline"] = cpu_baseline(w, delta, vels[0], budget_s=args.cpu_seconds)
+        out["cpu_baseline"] = cpu_baseline(w, cpu_rows[0], cpu_rows[1], budget_s=args.cpu_seconds)
     ctx.close()
     if world > 1:
         dist.destroy_process_group()
@@ -286,17 +315,16 @@ def _calibrated_rows(orc, w, d, v, seconds):
     return int(max(probe, min(d.shape[0], rate * seconds)))
 
 
-def cpu_baseline(w, delta, v, budget_s=12.0) -> dict:
+def cpu_baseline(w, d, vv, budget_s=12.0) -> dict:
+    """d, vv: [rows, n] numpy arrays of delta and v_pec (the first planes of the bench's own fields)."""
     from oracle import lya_oracle as orc
     n = w.n
-    d = delta.reshape(-1, n).cpu().numpy()
-    vv = v.reshape(-1, n).cpu().numpy()
     rows = _calibrated_rows(orc, w, d, vv, budget_s)
     t0 = time.perf_counter()
     _oracle_sample(orc, w, d[:rows], vv[:rows])
     dt = time.perf_counter() - t0
     return {"value": rows * float(n) ** 2 / dt, "unit": UNIT, "cores": orc.threads(), "kind": "oracle",
-            "sample": f"first {rows} of {d.shape[0]} sightlines of {w.name}, whole path S1..S5 in double, "
+            "sample": f"first {rows} of {n * n} sightlines of {w.name}, whole path S1..S5 in double, "
                       f"plain mode, {dt:.1f} s"}
 
 
@@ -334,7 +362,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--cfg", type=int, default=2, choices=[1, 2, 3, 4])
+    ap.add_argument("--cfg", type=int, default=2, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
