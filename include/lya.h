@@ -143,6 +143,47 @@ lya_status lya_forest_host(lya_ctx *ctx, const lya_params *p, int axis, int32_t 
                            float *tau_h, float *flux_h,
                            double *a_out, double *f_achieved, int *iters);
 
+/* ---------------------------------------------------------------------------------------------------------
+ * After F: the paper's instrument model and its two validation statistics.
+ * Spectra are ROWS: n_rows sightlines of n_pix contiguous fp32 pixels of velocity width dv_kms (sightlines
+ * along x of a [nz][ny][nx] grid are already in this form), periodic in velocity.
+ * --------------------------------------------------------------------------------------------------------- */
+
+/* "convolve the spectra with a Gaussian with a FWHM = 7 km/s, and resample our spectra onto 0.05 A bins ...
+ * add Gaussian distributed noise assuming S/N ~ 50 per pixel" (224 km/s, 1.0375 A, S/N 5:
+ * PAPER.md:130; 170 km/s, ~1 A, S/N 3.8: PAPER.md:166).  DESIGN.md readings O1-O3. */
+typedef struct {
+    double fwhm_kms;    /* Gaussian FWHM [km/s]; <= 0: no convolution                                          */
+    double bin_kms;     /* output bin width [km/s] (see lya_bin_kms_from_angstrom); <= 0: keep the pixels      */
+    double snr;         /* continuum signal-to-noise per output bin; <= 0: no noise                            */
+} lya_instrument;
+
+/* c dlambda / (1215.67 A (1+z)): velocity width of a wavelength bin at observed Lyman-alpha.  Host only. */
+double     lya_bin_kms_from_angstrom(double z, double dlambda_angstrom);
+/* floor(n_pix dv / bin) output bins per row (n_pix if bin_kms <= 0); a ragged last bin is dropped.  Host only. */
+int32_t    lya_instrument_bins(int32_t n_pix, double dv_kms, const lya_instrument *inst);
+
+/* flux: DEVICE [n_rows][n_pix].  unit_noise: DEVICE [n_rows][n_bins] N(0,1) draws supplied by the caller, or
+ * NULL (then snr must be <= 0).  out: DEVICE [n_rows][n_bins], n_bins = lya_instrument_bins(); may not alias
+ * flux.  out = rebin(G * flux) + unit_noise / snr.  LYA_EINVAL if the Gaussian needs more than 4096 taps a
+ * side or a row does not fit in shared memory.  Asynchronous on ctx's stream. */
+lya_status lya_observe_rows(lya_ctx *ctx, size_t n_rows, int32_t n_pix, double dv_kms, const lya_instrument *inst,
+                            const float *flux, const float *unit_noise, float *out);
+
+/* Flux PDF (21 bins of width 0.05, the first -0.025 <= F < 0.025): counts of n fp32 fluxes in
+ * n_bins (<= 256) bins [f_lo + b width, f_lo + (b+1) width); fluxes outside fall into the first / last bin
+ * (reading O4).  flux DEVICE; counts (uint64) and pdf (counts / (n width)) HOST, either may be NULL.
+ * Synchronises the stream. */
+lya_status lya_flux_pdf(lya_ctx *ctx, const float *flux, size_t n, int32_t n_bins, double f_lo, double width,
+                        uint64_t *counts, double *pdf);
+
+/* 1D flux power spectrum: P(k_m) = (V/N^2) <|sum_i dF_i exp(-2 pi i m i/N)|^2> over the
+ * rows, dF = F/mean_flux - 1, V = n_pix dv, k_m = 2 pi m / V [s/km], m = 0 .. n_pix/2.  n_pix must be a power
+ * of two between 8 and 8192 (a radix-2 FFT per row in shared memory).  flux DEVICE [n_rows][n_pix];
+ * power HOST, n_pix/2 + 1 doubles [km/s].  Synchronises the stream. */
+lya_status lya_flux_power_rows(lya_ctx *ctx, size_t n_rows, int32_t n_pix, double dv_kms, const float *flux,
+                               double mean_flux, double *power);
+
 /* Roofline denominator of the tau kernel (BASELINE.json: "MUFU.EX2 ... issue rate from SM count x clock"):
  * runs a pure ex2.approx micro-kernel on every SM of ctx's device and returns MUFU.EX2 results per second
  * (HOST double; best of 3 after a warm-up).  Synchronises the stream.  16 / clk / SM on B200. */

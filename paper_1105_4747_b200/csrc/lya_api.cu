@@ -81,6 +81,7 @@ lya_status lya_create(lya_ctx **out, int device, void *cuda_stream)
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->d_partials, part_bytes);
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->d_root, 64 * sizeof(double));
     if (e == cudaSuccess) e = cudaMallocHost((void **)&ctx->h_pinned, 64 * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->d_stats, LYA_STATS_DOUBLES * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->d_sched, 4 * sizeof(unsigned int));
     if (e == cudaSuccess) e = cudaMemset(ctx->d_sched, 0, 4 * sizeof(unsigned int));
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking);
@@ -104,6 +105,9 @@ void lya_destroy(lya_ctx *ctx)
     if (ctx->d_partials) cudaFree(ctx->d_partials);
     if (ctx->d_root) cudaFree(ctx->d_root);
     if (ctx->d_sched) cudaFree(ctx->d_sched);
+    if (ctx->d_stats) cudaFree(ctx->d_stats);
+    if (ctx->d_taps) cudaFree(ctx->d_taps);
+    free(ctx->h_taps);
     if (ctx->h_pinned) cudaFreeHost(ctx->h_pinned);
     for (int i = 0; i < 2; ++i) {
         if (ctx->ev_copy[i]) cudaEventDestroy(ctx->ev_copy[i]);

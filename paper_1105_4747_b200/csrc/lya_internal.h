@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include "../../include/lya.h"
@@ -21,6 +22,9 @@ struct lya_ctx {
     double       *d_root;         // device copy of the root-iteration result (see normalize.cu)
     double       *h_pinned;       // small pinned host mirror
     unsigned int *d_sched;        // tau_x_kernel row counter {next row, groups finished}; zero between launches
+    double       *d_stats;        // 8192 doubles: flux-PDF counts (as uint64) / power-spectrum accumulators
+    float        *d_taps, *h_taps; // lya_observe_rows: Gaussian taps (device / host staging), grown on demand
+    size_t        taps_cap;
     // lya_forest_host workspace (device), grown on demand
     void         *ws;
     size_t        ws_bytes;
@@ -29,6 +33,7 @@ struct lya_ctx {
 
 #define LYA_MAX_RED_BLOCKS 2048
 #define LYA_MAX_TRIALS     8
+#define LYA_STATS_DOUBLES   8192
 
 static inline lya_status lya_fail(lya_ctx *ctx, lya_status s, const char *msg)
 {

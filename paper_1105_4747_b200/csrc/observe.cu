@@ -1,0 +1,268 @@
+// observe.cu -- the paper's instrument model on rows of transmitted flux:
+// circular Gaussian convolution in velocity, flux-conserving resampling onto wider (or narrower) bins,
+// additive noise N(0,1)/(S/N) from caller-supplied unit draws.  DESIGN.md readings O1-O3.
+//
+//   Fc(i)  = sum_k g(k) F(i-k),  g(k) ~ exp(-(k dv)^2 / 2 sigma^2) over the nearest periodic image,
+//            normalised by the discrete sum; taps below 1e-10 of the peak are dropped (6.8 sigma)
+//   Fb(m)  = (1/B) integral over [m B, (m+1) B) of the piecewise-constant Fc       (B = bin / dv in pixels)
+//   out    = Fb + unit_noise / snr
+//
+// HBM-bound: 4 B read per pixel, 4 (+4 noise) B per output bin.  One CTA stages one row (with its periodic
+// halo) in shared memory; the convolution is register-tiled -- a thread owns 4 consecutive outputs, walks the
+// inputs with one conflict-free LDS.128 per 4 inputs and two broadcast LDS.128 of taps, 16 FFMA per step --
+// so even a 60-tap kernel stays near the memory roofline; the rebinning reads the convolved row from shared
+// memory with bin edges in double.
+#include <math.h>
+
+#include "lya_internal.h"
+
+namespace {
+
+struct ObsArgs {
+    const float *flux, *noise, *taps;     // taps: device, wp[0 .. L+10], wp[t+3] = g(Kr - t), zero padded
+    float       *out;
+    size_t       n_rows;
+    int          n, n4;                   // pixels per row; rounded up to a multiple of 4
+    int          Kl, Kr, L;               // taps on either side; L = Kl + Kr (L < 0: no convolution)
+    int          nb;                      // output bins per row
+    int          rebin;                   // 0: out has n pixels, no resampling
+    double       bin_px, inv_bin_px;      // B = bin / dv [pixels]
+    float        inv_snr;                 // 0: no noise
+};
+
+__global__ void __launch_bounds__(256) observe_rows_kernel(const ObsArgs a)
+{
+    extern __shared__ __align__(16) float sm[];
+    const int n = a.n, n4 = a.n4;
+    const int halo = a.L >= 0 ? a.L : 0;
+    const int in_len = n4 + ((halo + 3) & ~3) + 8;       // staged inputs incl. halo and zero padding
+    float *s_in = sm;                                    // s_in[h] = F[(h - Kr) mod n]
+    float *s_c  = sm + in_len;                           // convolved row, n4 floats
+    float *s_w  = s_c + n4;                              // taps, L + 11 floats rounded up to 4
+    const int w_len = ((halo + 11) + 3) & ~3;
+
+    if (a.L >= 0)
+        for (int t = threadIdx.x; t < w_len; t += blockDim.x) s_w[t] = t < halo + 11 ? a.taps[t] : 0.0f;
+
+    for (size_t row = blockIdx.x; row < a.n_rows; row += gridDim.x) {
+        const float *src = a.flux + row * (size_t)n;
+        __syncthreads();                                 // previous row's s_c / s_in consumed
+        if (a.L >= 0) {
+            for (int h = threadIdx.x; h < in_len; h += blockDim.x) {
+                float v = 0.0f;
+                if (h < n + halo) {
+                    int i = h - a.Kr;
+                    i = i < 0 ? i + n : (i >= n ? i - n : i);     // halo <= n - 1: one wrap is enough
+                    v = __ldcs(src + i);
+                }
+                s_in[h] = v;
+            }
+            __syncthreads();
+            for (int i0 = 4 * threadIdx.x; i0 < n4; i0 += 4 * blockDim.x) {
+                float acc0 = 0.f, acc1 = 0.f, acc2 = 0.f, acc3 = 0.f;
+                // out(i0 + r) = sum_t wt[t] s_in[i0 + r + t]; with u = r + t the weight of input u is wp[u - r + 3]
+                for (int u = 0; u <= a.L + 3; u += 4) {
+                    const float4 x  = *reinterpret_cast<const float4 *>(s_in + i0 + u);
+                    const float4 wa = *reinterpret_cast<const float4 *>(s_w + u);       // wp[u .. u+3]
+                    const float4 wb = *reinterpret_cast<const float4 *>(s_w + u + 4);   // wp[u+4 .. u+7]
+                    // input c (= x.c) and output r use wp[u + c - r + 3]
+                    acc0 = fmaf(wa.w, x.x, acc0); acc0 = fmaf(wb.x, x.y, acc0); acc0 = fmaf(wb.y, x.z, acc0); acc0 = fmaf(wb.z, x.w, acc0);
+                    acc1 = fmaf(wa.z, x.x, acc1); acc1 = fmaf(wa.w, x.y, acc1); acc1 = fmaf(wb.x, x.z, acc1); acc1 = fmaf(wb.y, x.w, acc1);
+                    acc2 = fmaf(wa.y, x.x, acc2); acc2 = fmaf(wa.z, x.y, acc2); acc2 = fmaf(wa.w, x.z, acc2); acc2 = fmaf(wb.x, x.w, acc2);
+                    acc3 = fmaf(wa.x, x.x, acc3); acc3 = fmaf(wa.y, x.y, acc3); acc3 = fmaf(wa.z, x.z, acc3); acc3 = fmaf(wa.w, x.w, acc3);
+                }
+                *reinterpret_cast<float4 *>(s_c + i0) = make_float4(acc0, acc1, acc2, acc3);
+            }
+        } else {
+            for (int i = threadIdx.x; i < n4; i += blockDim.x) s_c[i] = i < n ? __ldcs(src + i) : 0.0f;
+        }
+        __syncthreads();
+
+        float *dst = a.out + row * (size_t)a.nb;
+        const float *nz = a.noise ? a.noise + row * (size_t)a.nb : nullptr;
+        for (int m = threadIdx.x; m < a.nb; m += blockDim.x) {
+            float v;
+            if (a.rebin) {
+                const double lo = (double)m * a.bin_px, hi = lo + a.bin_px;
+                int i = (int)lo;
+                int i_end = (int)ceil(hi);
+                if (i_end > n) i_end = n;
+                float acc = 0.0f;
+                for (; i < i_end; ++i) {
+                    const double l = lo > (double)i ? lo : (double)i;
+                    const double h = hi < (double)(i + 1) ? hi : (double)(i + 1);
+                    if (h > l) acc = fmaf((float)(h - l), s_c[i], acc);
+                }
+                v = acc * (float)a.inv_bin_px;
+            } else {
+                v = s_c[m];
+            }
+            if (nz) v = fmaf(__ldcs(nz + m), a.inv_snr, v);
+            __stcs(dst + m, v);
+        }
+    }
+}
+
+// ---- flux PDF: private per-thread histograms in shared memory (hist[bin][thread]: conflict-free, no atomics)
+constexpr int PDF_THREADS = 128;
+
+__global__ void __launch_bounds__(PDF_THREADS) flux_pdf_kernel(const float *__restrict__ flux, size_t n, int n_bins,
+                                                               float f_lo, float inv_width,
+                                                               unsigned long long *__restrict__ counts)
+{
+    extern __shared__ unsigned int hist[];               // [n_bins][PDF_THREADS]
+    for (int t = threadIdx.x; t < n_bins * PDF_THREADS; t += PDF_THREADS) hist[t] = 0u;
+    __syncthreads();
+    unsigned int *mine = hist + threadIdx.x;
+    const float top = (float)n_bins;
+    auto add = [&](float f) {
+        // the bin decision is taken in fp32 with two separately rounded operations (reading O4)
+        const float t = floorf(__fmul_rn(__fsub_rn(f, f_lo), inv_width));
+        const int b = (t >= top) ? n_bins - 1 : (t > 0.0f ? (int)t : 0);
+        mine[b * PDF_THREADS] += 1u;
+    };
+    const size_t gtid = (size_t)blockIdx.x * PDF_THREADS + threadIdx.x, gsz = (size_t)gridDim.x * PDF_THREADS;
+    size_t head = ((16 - ((uintptr_t)flux & 15)) & 15) >> 2;
+    if (head > n) head = n;
+    const size_t n4 = (n - head) >> 2;
+    const float4 *f4 = reinterpret_cast<const float4 *>(flux + head);
+#pragma unroll 2
+    for (size_t i = gtid; i < n4; i += gsz) {
+        const float4 f = __ldcs(f4 + i);
+        add(f.x); add(f.y); add(f.z); add(f.w);
+    }
+    const size_t tail0 = head + (n4 << 2), n_edge = head + (n - tail0);
+    for (size_t e = gtid; e < n_edge; e += gsz) add(flux[e < head ? e : tail0 + (e - head)]);
+    __syncthreads();
+    // one warp per bin: sum the 128 private counters, one atomic per bin and CTA
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int b = warp; b < n_bins; b += PDF_THREADS / 32) {
+        unsigned int s = 0;
+        for (int t = lane; t < PDF_THREADS; t += 32) s += hist[b * PDF_THREADS + t];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+        if (lane == 0 && s) atomicAdd(counts + b, (unsigned long long)s);
+    }
+}
+
+}  // namespace
+
+extern "C" double lya_bin_kms_from_angstrom(double z, double dlambda_angstrom)
+{
+    return (LYA_C_CGS * 1.0e-5) * dlambda_angstrom / (1215.67 * (1.0 + z));
+}
+
+extern "C" int32_t lya_instrument_bins(int32_t n_pix, double dv_kms, const lya_instrument *inst)
+{
+    if (!inst || n_pix < 1 || !(dv_kms > 0.0)) return 0;
+    if (!(inst->bin_kms > 0.0)) return n_pix;
+    return (int32_t)floor((double)n_pix * dv_kms / inst->bin_kms + 1e-9);
+}
+
+extern "C" lya_status lya_observe_rows(lya_ctx *ctx, size_t n_rows, int32_t n_pix, double dv_kms,
+                                       const lya_instrument *inst, const float *flux, const float *unit_noise,
+                                       float *out)
+{
+    if (!ctx) return LYA_EINVAL;
+    ctx->err[0] = 0;
+    if (!inst || !flux || !out) return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: null pointer");
+    if (n_pix < 1 || !(dv_kms > 0.0)) return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: n_pix >= 1 and dv > 0 required");
+    if ((((uintptr_t)flux | (uintptr_t)out | (uintptr_t)unit_noise) & 3) != 0)
+        return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: pointers must be 4-byte aligned");
+    if (out == flux) return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: out may not alias flux");
+    if (inst->snr > 0.0 && !unit_noise) return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: snr > 0 needs unit_noise");
+    const int32_t nb = lya_instrument_bins(n_pix, dv_kms, inst);
+    if (nb < 1) return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: bin wider than the row");
+    if (n_rows == 0) return LYA_OK;
+    LYA_CUDA(ctx, cudaSetDevice(ctx->device));
+
+    ObsArgs a;
+    memset(&a, 0, sizeof(a));
+    a.flux = flux; a.noise = inst->snr > 0.0 ? unit_noise : nullptr; a.out = out;
+    a.n_rows = n_rows; a.n = n_pix; a.n4 = (n_pix + 3) & ~3; a.nb = nb;
+    a.rebin = inst->bin_kms > 0.0;
+    a.bin_px = a.rebin ? inst->bin_kms / dv_kms : 1.0;
+    a.inv_bin_px = 1.0 / a.bin_px;
+    a.inv_snr = inst->snr > 0.0 ? (float)(1.0 / inst->snr) : 0.0f;
+    a.L = -1;
+    if (inst->fwhm_kms > 0.0) {
+        const double sigma_px = inst->fwhm_kms / (2.0 * sqrt(2.0 * log(2.0))) / dv_kms;
+        const double kd = ceil(6.8 * sigma_px);                         // exp(-6.8^2 / 2) = 9e-11 of the peak
+        if (kd > 4096.0 && kd < 0.5 * n_pix) return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: Gaussian wider than 4096 taps a side");
+        const int K = kd < 1.0 ? 1 : (kd > 1.0e6 ? 1000000 : (int)kd);
+        a.Kl = K < (n_pix - 1) / 2 ? K : (n_pix - 1) / 2;
+        a.Kr = K < n_pix / 2 ? K : n_pix / 2;
+        a.L = a.Kl + a.Kr;
+        if (a.L > 8192) return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: Gaussian wider than 4096 taps a side");
+        const int n_t = a.L + 11;
+        if (ctx->taps_cap < (size_t)n_t) {
+            if (ctx->d_taps) cudaFree(ctx->d_taps);
+            ctx->d_taps = nullptr; ctx->taps_cap = 0;
+            free(ctx->h_taps);
+            ctx->h_taps = (float *)malloc((size_t)(n_t + 64) * sizeof(float));
+            if (!ctx->h_taps) return lya_fail(ctx, LYA_ENOMEM, "lya_observe_rows: host allocation failed");
+            LYA_CUDA(ctx, cudaMalloc((void **)&ctx->d_taps, (size_t)(n_t + 64) * sizeof(float)));
+            ctx->taps_cap = (size_t)n_t + 64;
+        }
+        // the stream may still be reading the previous call's taps: wait before overwriting the host copy
+        LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+        double sum = 0.0;
+        for (int k = -a.Kl; k <= a.Kr; ++k) sum += exp(-0.5 * (double)k * k / (sigma_px * sigma_px));
+        for (int t = 0; t < n_t; ++t) ctx->h_taps[t] = 0.0f;
+        for (int t = 0; t <= a.L; ++t) {
+            const double k = (double)(a.Kr - t);
+            ctx->h_taps[t + 3] = (float)(exp(-0.5 * k * k / (sigma_px * sigma_px)) / sum);
+        }
+        LYA_CUDA(ctx, cudaMemcpyAsync(ctx->d_taps, ctx->h_taps, (size_t)n_t * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+        a.taps = ctx->d_taps;
+    }
+    const int halo = a.L >= 0 ? a.L : 0;
+    const size_t smem = ((size_t)a.n4 + ((halo + 3) & ~3) + 8 + a.n4 + (((halo + 11) + 3) & ~3)) * sizeof(float);
+    if (smem > (size_t)ctx->max_smem_optin) return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: row too long for shared memory");
+    int threads = ((a.n4 / 4 + 31) / 32) * 32;
+    threads = threads < 32 ? 32 : (threads > 256 ? 256 : threads);
+    LYA_CUDA(ctx, cudaFuncSetAttribute(observe_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int per_sm = 0;
+    LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, observe_rows_kernel, threads, smem));
+    if (per_sm < 1) return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: row too long for shared memory");
+    const size_t cap = (size_t)ctx->sm_count * per_sm;
+    const int grid = (int)(n_rows < cap ? n_rows : cap);
+    observe_rows_kernel<<<grid, threads, smem, ctx->stream>>>(a);
+    ctx->launches++;
+    LYA_CUDA(ctx, cudaGetLastError());
+    return LYA_OK;
+}
+
+extern "C" lya_status lya_flux_pdf(lya_ctx *ctx, const float *flux, size_t n, int32_t n_bins, double f_lo,
+                                   double width, uint64_t *counts, double *pdf)
+{
+    if (!ctx) return LYA_EINVAL;
+    ctx->err[0] = 0;
+    if (!flux || ((uintptr_t)flux & 3)) return lya_fail(ctx, LYA_EINVAL, "lya_flux_pdf: bad flux pointer");
+    if (n_bins < 1 || n_bins > 256 || !(width > 0.0)) return lya_fail(ctx, LYA_EINVAL, "lya_flux_pdf: 1 <= n_bins <= 256 and width > 0 required");
+    LYA_CUDA(ctx, cudaSetDevice(ctx->device));
+    unsigned long long *d_counts = reinterpret_cast<unsigned long long *>(ctx->d_stats);
+    LYA_CUDA(ctx, cudaMemsetAsync(d_counts, 0, (size_t)n_bins * sizeof(unsigned long long), ctx->stream));
+    if (n > 0) {
+        const size_t smem = (size_t)n_bins * PDF_THREADS * sizeof(unsigned int);
+        LYA_CUDA(ctx, cudaFuncSetAttribute(flux_pdf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int per_sm = 0;
+        LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, flux_pdf_kernel, PDF_THREADS, smem));
+        if (per_sm < 1) return lya_fail(ctx, LYA_EINVAL, "lya_flux_pdf: too many bins for shared memory");
+        size_t want = (n / 4 + PDF_THREADS - 1) / PDF_THREADS;
+        if (want < 1) want = 1;
+        const size_t cap = (size_t)ctx->sm_count * per_sm;
+        flux_pdf_kernel<<<(int)(want < cap ? want : cap), PDF_THREADS, smem, ctx->stream>>>(
+            flux, n, n_bins, (float)f_lo, (float)(1.0 / width), d_counts);
+        ctx->launches++;
+        LYA_CUDA(ctx, cudaGetLastError());
+    }
+    uint64_t host[256];
+    LYA_CUDA(ctx, cudaMemcpyAsync(host, d_counts, (size_t)n_bins * sizeof(uint64_t), cudaMemcpyDeviceToHost, ctx->stream));
+    LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    for (int b = 0; b < n_bins; ++b) {
+        if (counts) counts[b] = host[b];
+        if (pdf) pdf[b] = n ? (double)host[b] / ((double)n * width) : 0.0;
+    }
+    return LYA_OK;
+}

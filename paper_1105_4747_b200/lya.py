@@ -36,6 +36,10 @@ class CScalars(C.Structure):
                 ("Ez", "Hz", "dR_cm", "dv_kms", "V_kms", "b0_kms", "nbarH", "nbarHI", "K", "tau0", "tauGP")]
 
 
+class CInstrument(C.Structure):
+    _fields_ = [("fwhm_kms", C.c_double), ("bin_kms", C.c_double), ("snr", C.c_double)]
+
+
 class CRootState(C.Structure):
     _fields_ = [("f_target", C.c_double), ("rel_tol", C.c_double), ("n_pix", C.c_double),
                 ("lo", C.c_double), ("hi", C.c_double), ("a", C.c_double), ("f_at_a", C.c_double),
@@ -73,7 +77,9 @@ class Params:
 EXPORTS = ("lya_version", "lya_status_string", "lya_scalars_from_params", "lya_create", "lya_destroy",
            "lya_last_error", "lya_sm_count", "lya_gas_from_density", "lya_tau_sightlines",
            "lya_normalize_mean_flux", "lya_flux_partial_sums", "lya_root_init", "lya_root_update",
-           "lya_flux", "lya_forest_host", "lya_launch_count", "lya_measure_mufu_peak")
+           "lya_flux", "lya_forest_host", "lya_launch_count", "lya_measure_mufu_peak",
+           "lya_bin_kms_from_angstrom", "lya_instrument_bins", "lya_observe_rows", "lya_flux_pdf",
+           "lya_flux_power_rows")
 
 _lib = None
 
@@ -109,8 +115,19 @@ def lib() -> C.CDLL:
     L.lya_forest_host.argtypes = [vp, pp, C.c_int, C.c_int32, fp, fp, C.c_double, C.c_double, C.c_int,
                                   fp, fp, dp, dp, ip]
     L.lya_measure_mufu_peak.argtypes = [vp, dp]
+    L.lya_bin_kms_from_angstrom.argtypes = [C.c_double, C.c_double]
+    L.lya_bin_kms_from_angstrom.restype = C.c_double
+    L.lya_instrument_bins.argtypes = [C.c_int32, C.c_double, C.POINTER(CInstrument)]
+    L.lya_instrument_bins.restype = C.c_int32
+    L.lya_observe_rows.argtypes = [vp, C.c_size_t, C.c_int32, C.c_double, C.POINTER(CInstrument), fp, fp, fp]
+    L.lya_flux_pdf.argtypes = [vp, fp, C.c_size_t, C.c_int32, C.c_double, C.c_double, C.POINTER(C.c_uint64), dp]
+    L.lya_flux_power_rows.argtypes = [vp, C.c_size_t, C.c_int32, C.c_double, fp, C.c_double, dp]
     _lib = L
     return L
+
+
+def bin_kms_from_angstrom(z: float, dlambda: float) -> float:
+    return float(lib().lya_bin_kms_from_angstrom(z, dlambda))
 
 
 def scalars(p: Params, axis: int = 0) -> dict:
@@ -217,6 +234,39 @@ class Context:
         out = torch.empty_like(tau) if out is None else out
         self._check(lib().lya_flux(self._h, _dev(tau, "tau"), tau.numel(), a, _dev(out, "flux")))
         return out
+
+    # after F: instrument model, flux PDF, 1D flux power
+    def observe_rows(self, flux, dv_kms: float, fwhm_kms: float = 0.0, bin_kms: float = 0.0, snr: float = 0.0,
+                     unit_noise=None, out=None):
+        """flux: [..., n_pix] rows.  Returns [n_rows, n_bins]."""
+        n_pix = flux.shape[-1]
+        n_rows = flux.numel() // n_pix
+        inst = CInstrument(fwhm_kms, bin_kms, snr)
+        nb = lib().lya_instrument_bins(n_pix, dv_kms, C.byref(inst))
+        if nb < 1:
+            raise LyaError(EINVAL, "observe_rows: bin wider than the row")
+        out = torch.empty((n_rows, nb), dtype=torch.float32, device=flux.device) if out is None else out
+        if out.numel() != n_rows * nb or (unit_noise is not None and unit_noise.numel() != n_rows * nb):
+            raise ValueError("observe_rows: out / unit_noise must be [n_rows][n_bins]")
+        self._check(lib().lya_observe_rows(self._h, n_rows, n_pix, dv_kms, C.byref(inst), _dev(flux, "flux"),
+                                           None if unit_noise is None else _dev(unit_noise, "unit_noise"),
+                                           _dev(out, "out")))
+        return out
+
+    def flux_pdf(self, flux, n_bins: int = 21, f_lo: float = -0.025, width: float = 0.05):
+        import numpy as np
+        counts = (C.c_uint64 * n_bins)()
+        pdf = (C.c_double * n_bins)()
+        self._check(lib().lya_flux_pdf(self._h, _dev(flux, "flux"), flux.numel(), n_bins, f_lo, width, counts, pdf))
+        return np.array(counts, dtype=np.uint64), np.array(pdf, dtype=np.float64)
+
+    def flux_power_rows(self, flux, dv_kms: float, mean_flux: float):
+        import numpy as np
+        n_pix = flux.shape[-1]
+        P = (C.c_double * (n_pix // 2 + 1))()
+        self._check(lib().lya_flux_power_rows(self._h, flux.numel() // n_pix, n_pix, dv_kms, _dev(flux, "flux"),
+                                              mean_flux, P))
+        return np.array(P, dtype=np.float64)
 
     # S1..S5 from host buffers
     def forest_host(self, p: Params, axis: int, delta_h, v_pec_h, f_target: float, rel_tol: float = 1e-7,

@@ -1,0 +1,119 @@
+"""GPU parity of the instrument model, flux PDF and 1D flux power against
+oracle/lya_obs_oracle.c, through the C ABI.  Tolerances: observed flux 1e-5 absolute (the north_star's bar for
+F); PDF counts bit-exact (the bin decision is taken in fp32 on both sides); power 1e-4 relative plus 1e-9 of
+the largest mode (fp32 FFT of dF)."""
+import numpy as np
+import pytest
+import torch
+
+from paper_1105_4747_b200 import inputs, lya
+from paper_1105_4747_b200.workloads import WORKLOADS
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def ctx():
+    c = lya.Context(0)
+    yield c
+    c.close()
+
+
+@pytest.fixture(scope="module")
+def obs():
+    from oracle import lya_obs_oracle
+    lya_obs_oracle.build()
+    return lya_obs_oracle
+
+
+@pytest.fixture(scope="module")
+def flux_rows(ctx):
+    """F of the first 4 planes of config 2 (1024 rows of 256 pixels) through the library's own S1-S5."""
+    w = WORKLOADS[2]
+    f = inputs.make_fields(w, device="cuda", z0=0, z1=4)
+    p = lya.Params.from_workload(w)
+    n_hi, b = ctx.gas_from_density(p, f["delta"])
+    tau = ctx.tau_sightlines(p, 0, n_hi, b, f["v_pec"][0], nz_local=4)
+    A, _, _, _ = ctx.normalize_mean_flux(tau, w.f_target)
+    F = ctx.flux(tau, A).reshape(-1, w.n)
+    return F, lya.scalars(p, 0)["dv_kms"], w
+
+
+# the paper's three instruments + pure cases
+@pytest.mark.parametrize("fwhm,dlam,snr", [(7.0, 0.05, 50.0), (170.0, 1.0, 3.8), (224.0, 1.0375, 5.0),
+                                           (120.0, 0.0, 0.0), (0.0, 1.0375, 0.0), (0.0, 0.0, 5.0)])
+def test_observe_rows_parity(ctx, obs, flux_rows, fwhm, dlam, snr):
+    F, dv, w = flux_rows
+    bin_kms = lya.bin_kms_from_angstrom(w.z, dlam) if dlam > 0 else 0.0
+    assert bin_kms == pytest.approx(obs.bin_kms_from_angstrom(w.z, dlam), rel=1e-12)
+    nb = obs.n_bins(w.n, dv, bin_kms)
+    g = torch.Generator(device="cuda").manual_seed(7)
+    noise = torch.randn((F.shape[0], nb), device="cuda", generator=g) if snr > 0 else None
+    out = ctx.observe_rows(F, dv, fwhm, bin_kms, snr, noise)
+    torch.cuda.synchronize()
+    rows = slice(0, 192)
+    ref = obs.observe_rows(F[rows].cpu().numpy(), dv, fwhm, bin_kms, snr,
+                           None if noise is None else noise[rows].cpu().numpy())
+    assert out.shape == (F.shape[0], nb) and ref.shape[1] == nb
+    err = np.abs(out[rows].cpu().numpy() - ref).max()
+    assert err < 1e-5, f"observed flux max abs err {err:.2e}"
+
+
+@pytest.mark.parametrize("n,fwhm", [(5, 3.0), (13, 40.0), (100, 9.0), (257, 300.0), (1000, 55.0), (4096, 224.0)])
+def test_observe_rows_ragged_and_wide_kernels(ctx, obs, n, fwhm):
+    """Ragged row lengths, a Gaussian as wide as the row (every nearest image contributes), bins that do not
+    divide the row."""
+    rng = np.random.default_rng(n)
+    F = torch.from_numpy(rng.uniform(0, 1, (7, n)).astype(np.float32)).cuda()
+    dv, bin_kms = 6.5, 17.3 if n > 5 else 0.0
+    out = ctx.observe_rows(F, dv, fwhm, bin_kms)
+    ref = obs.observe_rows(F.cpu().numpy(), dv, fwhm, bin_kms, 0.0)
+    assert out.shape == ref.shape
+    assert np.abs(out.cpu().numpy() - ref).max() < 1e-5
+
+
+def test_observe_rows_errors(ctx):
+    F = torch.rand((4, 64), device="cuda")
+    with pytest.raises(lya.LyaError):
+        ctx.observe_rows(F, 5.0, 10.0, 1000.0)                     # bin wider than the row
+    with pytest.raises(lya.LyaError):
+        ctx.observe_rows(F, 5.0, 10.0, 0.0, snr=5.0)               # noise requested, no draws given
+    with pytest.raises(lya.LyaError):
+        ctx.observe_rows(F, 5.0, 10.0, 0.0, out=F)                 # aliasing
+
+
+def test_flux_pdf_bit_exact(ctx, obs, flux_rows):
+    F, dv, w = flux_rows
+    g = torch.Generator(device="cuda").manual_seed(11)
+    noisy = (F + 0.2 * torch.randn(F.shape, device="cuda", generator=g)).contiguous()    # spills over both ends
+    for arr in (F, noisy, noisy.reshape(-1)[3:100_002]):            # the last one: unaligned base, ragged length
+        arr = arr.contiguous() if arr.dim() == 2 else arr
+        counts, pdf = ctx.flux_pdf(arr)
+        c_ref, p_ref = obs.flux_pdf(arr.cpu().numpy())
+        assert np.array_equal(counts, c_ref)
+        assert np.allclose(pdf, p_ref, rtol=1e-14)
+        assert counts.sum() == arr.numel()
+    counts, _ = ctx.flux_pdf(noisy, n_bins=100, f_lo=-0.5, width=0.02)
+    assert np.array_equal(counts, obs.flux_pdf(noisy.cpu().numpy(), 100, -0.5, 0.02)[0])
+
+
+@pytest.mark.parametrize("n_rows", [1, 2, 333])
+def test_flux_power_parity(ctx, obs, flux_rows, n_rows):
+    F, dv, w = flux_rows
+    Fr = F[:n_rows].contiguous()
+    fbar = float(Fr.double().mean())
+    P = ctx.flux_power_rows(Fr, dv, fbar)
+    ref = obs.flux_power(Fr.cpu().numpy(), dv, fbar)
+    assert P.shape == ref.shape == (w.n // 2 + 1,)
+    assert np.all(np.abs(P - ref) <= 1e-4 * ref + 1e-9 * ref.max()), np.abs(P / ref - 1).max()
+
+
+@pytest.mark.parametrize("n", [8, 64, 2048, 8192])
+def test_flux_power_lengths_and_errors(ctx, obs, n):
+    rng = np.random.default_rng(n)
+    F = torch.from_numpy(rng.uniform(0.05, 1, (5, n)).astype(np.float32)).cuda()
+    P = ctx.flux_power_rows(F, 2.0, 0.5)
+    ref = obs.flux_power(F.cpu().numpy(), 2.0, 0.5)
+    assert np.all(np.abs(P - ref) <= 1e-4 * ref + 1e-9 * ref.max())
+    with pytest.raises(lya.LyaError):
+        ctx.flux_power_rows(F[:, : n - 1].contiguous(), 2.0, 0.5)   # not a power of two
