@@ -219,6 +219,42 @@ def bench_ours(args) -> dict:
         k_ms[name] = sum(spans) / len(spans)
     slab_cells = slab_nz * n * n
 
+    # ---- the rows after F, timed per kernel on this workload's F; not part of `value`
+    next_rows = None
+    if not args.no_next and w.cfg != 5 and (n & (n - 1)) == 0:
+        dv = lya.scalars(p, 0)["dv_kms"]
+        Frows = flux.reshape(-1, n)
+        bin_kms = lya.bin_kms_from_angstrom(w.z, 1.0375)                   # BOSS-like instrument
+        nb = lya.lib().lya_instrument_bins(n, dv, lya.C.byref(lya.CInstrument(224.0, bin_kms, 5.0)))
+        noise = torch.randn((Frows.shape[0], nb), device="cuda")
+        obs_out = torch.empty_like(noise)
+
+        def timed_ms(fn, reps=5):
+            spans = []
+            for _ in range(reps + 1):
+                flush.zero_()
+                e0, e1 = ev(), ev()
+                e0.record()
+                fn()
+                e1.record()
+                torch.cuda.synchronize()
+                spans.append(e0.elapsed_time(e1))
+            return sum(spans[1:]) / reps
+
+        t_obs = timed_ms(lambda: ctx.observe_rows(Frows, dv, 224.0, bin_kms, 5.0, noise, obs_out))
+        t_pdf = timed_ms(lambda: ctx.flux_pdf(flux))
+        t_pow = timed_ms(lambda: ctx.flux_power_rows(Frows, dv, results["f"]))
+        b_obs = 4 * n_cells + 8 * obs_out.numel()
+        next_rows = {
+            "observe_rows": {"instrument": "FWHM 224 km/s, 1.0375 A bins, S/N 5 (PAPER.md:130)", "bins_per_row": int(nb),
+                             "ms": t_obs, "bytes": int(b_obs), "gbs": b_obs / t_obs / 1e6, "frac_hbm": b_obs / t_obs / 1e6 / pk["hbm_gbs"]},
+            "flux_pdf": {"ms": t_pdf, "bytes": int(4 * n_cells), "gbs": 4 * n_cells / t_pdf / 1e6,
+                         "frac_hbm": 4 * n_cells / t_pdf / 1e6 / pk["hbm_gbs"]},
+            "flux_power_rows": {"ms": t_pow, "bytes": int(4 * n_cells), "gbs": 4 * n_cells / t_pow / 1e6,
+                                "frac_hbm": 4 * n_cells / t_pow / 1e6 / pk["hbm_gbs"],
+                                "note": "radix-2 FFT in shared memory: shared-memory bound, not HBM bound"}}
+        del noise, obs_out
+
     # ---- end to end through lya_forest_host: pinned host inputs, F read back, every step
     e2e = None
     if not args.no_e2e:
@@ -285,7 +321,7 @@ def bench_ours(args) -> dict:
                           "gbs": gbs(4 * n_cells * passes, k_ms["normalize"]),
                           "frac": gbs(4 * n_cells * passes, k_ms["normalize"]) / hbm},
             "flux": {"bytes": 8 * n_cells, "gbs": gbs(8 * n_cells, k_ms["flux"]), "frac": gbs(8 * n_cells, k_ms["flux"]) / hbm}},
-        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches), "sm_count": ctx.sm_count,
+        "clocks": clocks, "e2e": e2e, "next_rows": next_rows, "gpu_launches": int(launches), "sm_count": ctx.sm_count,
     }
     if rank == 0 and world == 1 and not args.no_cpu:
         out["cpu_baseline"] = cpu_baseline(w, cpu_rows[0], cpu_rows[1], budget_s=args.cpu_seconds)
@@ -366,6 +402,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-next", action="store_true", help="skip the per-kernel timing of the rows after F")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     args = ap.parse_args()
     out = bench_reference(args) if args.impl == "reference" else bench_ours(args)

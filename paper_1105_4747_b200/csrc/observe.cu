@@ -3,7 +3,7 @@
 // additive noise N(0,1)/(S/N) from caller-supplied unit draws.  DESIGN.md readings O1-O3.
 //
 //   Fc(i)  = sum_k g(k) F(i-k),  g(k) ~ exp(-(k dv)^2 / 2 sigma^2) over the nearest periodic image,
-//            normalised by the discrete sum; taps below 1e-10 of the peak are dropped (6.8 sigma)
+//            normalised by the discrete sum; taps below 9e-8 of the peak are dropped (5.7 sigma)
 //   Fb(m)  = (1/B) integral over [m B, (m+1) B) of the piecewise-constant Fc       (B = bin / dv in pixels)
 //   out    = Fb + unit_noise / snr
 //
@@ -23,46 +23,123 @@ struct ObsArgs {
     float       *out;
     size_t       n_rows;
     int          n, n4;                   // pixels per row; rounded up to a multiple of 4
-    int          Kl, Kr, L;               // taps on either side; L = Kl + Kr (L < 0: no convolution)
+    int          Kl, Kr, KO, L;           // taps on either side, left halo KO >= Kr; L = KO + Kl (< 0: no convolution)
     int          nb;                      // output bins per row
     int          rebin;                   // 0: out has n pixels, no resampling
-    double       bin_px, inv_bin_px;      // B = bin / dv [pixels]
+    unsigned long long bin_fx;            // B = bin / dv [pixels] in 32.32 fixed point
+    float        inv_bin_f;               // 1 / B
     float        inv_snr;                 // 0: no noise
 };
 
+// A CTA works on batches of D rows.  NV = float4 loads per thread and row (n4 <= 4 * NV * blockDim.x).  The
+// NEXT batch is fetched into registers, and the CURRENT batch's noise draws are, before the current batch is
+// convolved, so D * NV 128-bit loads per thread are in flight during all the arithmetic (HBM latency x
+// bandwidth needs ~10 MB in flight on B200).
+// s_in[d][h] = F_d[(h - KO) mod n], h < n + L, with KO >= Kr the left halo (a multiple of 4 in FAST mode, so
+// that a thread's four pixels go to shared memory as one aligned STS.128 and the halo pixels -- at most one
+// per thread and row -- are fetched separately); taps wp[t + 3] = g(KO - t), zero where KO - t is outside
+// [-Kl, Kr].
+constexpr int OBS_NBR = 4;                               // noise draws per thread and row held in registers
+
+template <int NV, int D, bool FAST>
 __global__ void __launch_bounds__(256) observe_rows_kernel(const ObsArgs a)
 {
     extern __shared__ __align__(16) float sm[];
     const int n = a.n, n4 = a.n4;
     const int halo = a.L >= 0 ? a.L : 0;
     const int in_len = n4 + ((halo + 3) & ~3) + 8;       // staged inputs incl. halo and zero padding
-    float *s_in = sm;                                    // s_in[h] = F[(h - Kr) mod n]
-    float *s_c  = sm + in_len;                           // convolved row, n4 floats
-    float *s_w  = s_c + n4;                              // taps, L + 11 floats rounded up to 4
+    float *s_in = sm;                                    // [D][in_len]
+    float *s_c  = sm + D * in_len;                       // [D][n4] convolved rows
+    float *s_w  = s_c + D * n4;                          // taps, L + 11 floats rounded up to 4
     const int w_len = ((halo + 11) + 3) & ~3;
+    const bool conv = a.L >= 0;
+    const int T = blockDim.x, tid = threadIdx.x;
 
-    if (a.L >= 0)
-        for (int t = threadIdx.x; t < w_len; t += blockDim.x) s_w[t] = t < halo + 11 ? a.taps[t] : 0.0f;
+    if (conv)
+        for (int t = tid; t < w_len; t += T) s_w[t] = t < halo + 11 ? a.taps[t] : 0.0f;
+    for (int h = tid; h < D * in_len; h += T) s_in[h] = 0.0f;       // zero padding beyond n + halo
+    if (!conv)
+        for (int h = tid; h < D * n4; h += T) s_c[h] = 0.0f;
 
-    for (size_t row = blockIdx.x; row < a.n_rows; row += gridDim.x) {
-        const float *src = a.flux + row * (size_t)n;
-        __syncthreads();                                 // previous row's s_c / s_in consumed
-        if (a.L >= 0) {
-            for (int h = threadIdx.x; h < in_len; h += blockDim.x) {
-                float v = 0.0f;
-                if (h < n + halo) {
-                    int i = h - a.Kr;
-                    i = i < 0 ? i + n : (i >= n ? i - n : i);     // halo <= n - 1: one wrap is enough
-                    v = __ldcs(src + i);
+    float4 reg[D][NV];
+    float hreg[D];                                       // FAST: this thread's halo pixel (tid < L)
+    float nzr[D][OBS_NBR];
+    auto fetch = [&](size_t row0) {                      // rows row0 .. row0+D-1 -> registers
+#pragma unroll
+        for (int d = 0; d < D; ++d) {
+            const size_t row = row0 + d;
+            hreg[d] = 0.0f;
+#pragma unroll
+            for (int q = 0; q < NV; ++q) reg[d][q] = make_float4(0.f, 0.f, 0.f, 0.f);
+            if (row >= a.n_rows) continue;
+            const float *src = a.flux + row * (size_t)n;
+#pragma unroll
+            for (int q = 0; q < NV; ++q) {
+                const int p = 4 * (tid + q * T);
+                if (p < n) {
+                    if (FAST) reg[d][q] = __ldcs(reinterpret_cast<const float4 *>(src + p));
+                    else {
+                        float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+                        v.x = __ldcs(src + p);
+                        if (p + 1 < n) v.y = __ldcs(src + p + 1);
+                        if (p + 2 < n) v.z = __ldcs(src + p + 2);
+                        if (p + 3 < n) v.w = __ldcs(src + p + 3);
+                        reg[d][q] = v;
+                    }
                 }
-                s_in[h] = v;
             }
-            __syncthreads();
-            for (int i0 = 4 * threadIdx.x; i0 < n4; i0 += 4 * blockDim.x) {
+            if (FAST && conv && tid < a.L)               // left halo h < KO: F[n - KO + h]; right: F[h - KO]
+                hreg[d] = __ldg(src + (tid < a.KO ? n - a.KO + tid : tid - a.KO));
+        }
+    };
+    auto put = [&](float *si, float *sc, int i, float v) {   // generic: pixel i -> body and halo copies
+        if (i >= n) return;
+        if (!conv) { sc[i] = v; return; }
+        si[i + a.KO] = v;
+        if (i < a.Kl) si[n + a.KO + i] = v;
+        if (i >= n - a.KO) si[i - (n - a.KO)] = v;
+    };
+
+    size_t row0 = (size_t)blockIdx.x * D;
+    if (row0 < a.n_rows) fetch(row0);
+    for (; row0 < a.n_rows; row0 += (size_t)gridDim.x * D) {
+        __syncthreads();                                 // previous batch's s_in / s_c consumed
+#pragma unroll
+        for (int d = 0; d < D; ++d) {
+            float *si = s_in + d * in_len, *sc = s_c + d * n4;
+#pragma unroll
+            for (int q = 0; q < NV; ++q) {
+                const int p = 4 * (tid + q * T);
+                if (FAST) {
+                    if (p < n) *reinterpret_cast<float4 *>((conv ? si + a.KO : sc) + p) = reg[d][q];
+                } else {
+                    put(si, sc, p, reg[d][q].x); put(si, sc, p + 1, reg[d][q].y);
+                    put(si, sc, p + 2, reg[d][q].z); put(si, sc, p + 3, reg[d][q].w);
+                }
+            }
+            if (FAST && conv && tid < a.L) si[tid < a.KO ? tid : n + tid] = hreg[d];
+        }
+        // loads issued now stay in flight during the convolution: the next batch, and this batch's noise
+        if (row0 + (size_t)gridDim.x * D < a.n_rows) fetch(row0 + (size_t)gridDim.x * D);
+        if (a.noise) {
+#pragma unroll
+            for (int d = 0; d < D; ++d)
+#pragma unroll
+                for (int k = 0; k < OBS_NBR; ++k) {
+                    const int m = tid + k * T;
+                    nzr[d][k] = (row0 + d < a.n_rows && m < a.nb) ? __ldcs(a.noise + (row0 + d) * (size_t)a.nb + m) : 0.0f;
+                }
+        }
+        __syncthreads();
+        if (conv) {
+            for (int item = tid; item < D * (n4 >> 2); item += T) {
+                const int d = item / (n4 >> 2), i0 = 4 * (item - d * (n4 >> 2));
+                const float *si = s_in + d * in_len + i0;
                 float acc0 = 0.f, acc1 = 0.f, acc2 = 0.f, acc3 = 0.f;
                 // out(i0 + r) = sum_t wt[t] s_in[i0 + r + t]; with u = r + t the weight of input u is wp[u - r + 3]
+#pragma unroll 2
                 for (int u = 0; u <= a.L + 3; u += 4) {
-                    const float4 x  = *reinterpret_cast<const float4 *>(s_in + i0 + u);
+                    const float4 x  = *reinterpret_cast<const float4 *>(si + u);
                     const float4 wa = *reinterpret_cast<const float4 *>(s_w + u);       // wp[u .. u+3]
                     const float4 wb = *reinterpret_cast<const float4 *>(s_w + u + 4);   // wp[u+4 .. u+7]
                     // input c (= x.c) and output r use wp[u + c - r + 3]
@@ -71,34 +148,53 @@ __global__ void __launch_bounds__(256) observe_rows_kernel(const ObsArgs a)
                     acc2 = fmaf(wa.y, x.x, acc2); acc2 = fmaf(wa.z, x.y, acc2); acc2 = fmaf(wa.w, x.z, acc2); acc2 = fmaf(wb.x, x.w, acc2);
                     acc3 = fmaf(wa.x, x.x, acc3); acc3 = fmaf(wa.y, x.y, acc3); acc3 = fmaf(wa.z, x.z, acc3); acc3 = fmaf(wa.w, x.w, acc3);
                 }
-                *reinterpret_cast<float4 *>(s_c + i0) = make_float4(acc0, acc1, acc2, acc3);
+                *reinterpret_cast<float4 *>(s_c + d * n4 + i0) = make_float4(acc0, acc1, acc2, acc3);
             }
-        } else {
-            for (int i = threadIdx.x; i < n4; i += blockDim.x) s_c[i] = i < n ? __ldcs(src + i) : 0.0f;
+            __syncthreads();
         }
-        __syncthreads();
 
-        float *dst = a.out + row * (size_t)a.nb;
-        const float *nz = a.noise ? a.noise + row * (size_t)a.nb : nullptr;
-        for (int m = threadIdx.x; m < a.nb; m += blockDim.x) {
-            float v;
-            if (a.rebin) {
-                const double lo = (double)m * a.bin_px, hi = lo + a.bin_px;
-                int i = (int)lo;
-                int i_end = (int)ceil(hi);
-                if (i_end > n) i_end = n;
-                float acc = 0.0f;
-                for (; i < i_end; ++i) {
-                    const double l = lo > (double)i ? lo : (double)i;
-                    const double h = hi < (double)(i + 1) ? hi : (double)(i + 1);
-                    if (h > l) acc = fmaf((float)(h - l), s_c[i], acc);
+#pragma unroll
+        for (int d = 0; d < D; ++d) {
+            if (row0 + d >= a.n_rows) break;
+            const float *sc = s_c + d * n4;
+            float *dst = a.out + (row0 + d) * (size_t)a.nb;
+            int k = 0;
+            for (int m = tid; m < a.nb; m += T, ++k) {
+                float v;
+                if (a.rebin) {
+                    // bin [lo, hi) in pixel units as 32.32 fixed point (bin_fx = B 2^32 rounded: the edges are
+                    // off by < m 2^-33 pixels): partial first and last pixel, whole pixels in between
+                    const unsigned long long lo = (unsigned long long)m * a.bin_fx, hi1 = lo + a.bin_fx - 1ull;
+                    const int i0 = (int)(lo >> 32);
+                    int i1 = (int)(hi1 >> 32);                                   // ceil(hi) - 1
+                    if (i1 > n - 1) i1 = n - 1;
+                    const float f_lo = (float)(unsigned int)lo * 2.3283064365386963e-10f;           // frac(lo)
+                    const float f_hi = ((float)(unsigned int)hi1 + 1.0f) * 2.3283064365386963e-10f; // hi - i1
+                    float acc;
+                    if (i1 <= i0) {
+                        acc = (f_hi - f_lo) * sc[i0];
+                    } else {
+                        acc = (1.0f - f_lo) * sc[i0];
+#pragma unroll 1
+                        for (int i = i0 + 1; i < i1; ++i) acc += sc[i];
+                        acc = fmaf(f_hi, sc[i1], acc);
+                    }
+                    v = acc * a.inv_bin_f;
+                } else {
+                    v = sc[m];
                 }
-                v = acc * (float)a.inv_bin_px;
-            } else {
-                v = s_c[m];
+                if (a.noise) {
+                    float z = 0.0f;
+                    if (k < OBS_NBR) {
+#pragma unroll
+                        for (int kk = 0; kk < OBS_NBR; ++kk) if (kk == k) z = nzr[d][kk];
+                    } else {
+                        z = __ldcs(a.noise + (row0 + d) * (size_t)a.nb + m);
+                    }
+                    v = fmaf(z, a.inv_snr, v);
+                }
+                __stcs(dst + m, v);
             }
-            if (nz) v = fmaf(__ldcs(nz + m), a.inv_snr, v);
-            __stcs(dst + m, v);
         }
     }
 }
@@ -181,18 +277,25 @@ extern "C" lya_status lya_observe_rows(lya_ctx *ctx, size_t n_rows, int32_t n_pi
     a.flux = flux; a.noise = inst->snr > 0.0 ? unit_noise : nullptr; a.out = out;
     a.n_rows = n_rows; a.n = n_pix; a.n4 = (n_pix + 3) & ~3; a.nb = nb;
     a.rebin = inst->bin_kms > 0.0;
-    a.bin_px = a.rebin ? inst->bin_kms / dv_kms : 1.0;
-    a.inv_bin_px = 1.0 / a.bin_px;
+    const double bin_px = a.rebin ? inst->bin_kms / dv_kms : 1.0;
+    if (bin_px < 1.0e-6) return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: bin narrower than 1e-6 pixel");
+    a.bin_fx = (unsigned long long)llrint(bin_px * 4294967296.0);
+    a.inv_bin_f = (float)(1.0 / bin_px);
     a.inv_snr = inst->snr > 0.0 ? (float)(1.0 / inst->snr) : 0.0f;
+    int threads = ((a.n4 / 4 + 31) / 32) * 32;
+    threads = threads < 32 ? 32 : (threads > 256 ? 256 : threads);
+    bool fast = (n_pix % 4 == 0) && (((uintptr_t)flux & 15) == 0);
     a.L = -1;
     if (inst->fwhm_kms > 0.0) {
         const double sigma_px = inst->fwhm_kms / (2.0 * sqrt(2.0 * log(2.0))) / dv_kms;
-        const double kd = ceil(6.8 * sigma_px);                         // exp(-6.8^2 / 2) = 9e-11 of the peak
-        if (kd > 4096.0 && kd < 0.5 * n_pix) return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: Gaussian wider than 4096 taps a side");
+        const double kd = ceil(5.7 * sigma_px);                         // taps below exp(-5.7^2/2) = 9e-8 of the peak dropped
         const int K = kd < 1.0 ? 1 : (kd > 1.0e6 ? 1000000 : (int)kd);
         a.Kl = K < (n_pix - 1) / 2 ? K : (n_pix - 1) / 2;
         a.Kr = K < n_pix / 2 ? K : n_pix / 2;
-        a.L = a.Kl + a.Kr;
+        const int ko4 = (a.Kr + 3) & ~3;
+        fast = fast && ko4 <= n_pix && ko4 + a.Kl <= threads;
+        a.KO = fast ? ko4 : a.Kr;
+        a.L = a.KO + a.Kl;
         if (a.L > 8192) return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: Gaussian wider than 4096 taps a side");
         const int n_t = a.L + 11;
         if (ctx->taps_cap < (size_t)n_t) {
@@ -209,25 +312,33 @@ extern "C" lya_status lya_observe_rows(lya_ctx *ctx, size_t n_rows, int32_t n_pi
         double sum = 0.0;
         for (int k = -a.Kl; k <= a.Kr; ++k) sum += exp(-0.5 * (double)k * k / (sigma_px * sigma_px));
         for (int t = 0; t < n_t; ++t) ctx->h_taps[t] = 0.0f;
-        for (int t = 0; t <= a.L; ++t) {
-            const double k = (double)(a.Kr - t);
+        for (int t = a.KO - a.Kr; t <= a.L; ++t) {                      // offset k = KO - t in [-Kl, Kr]
+            const double k = (double)(a.KO - t);
             ctx->h_taps[t + 3] = (float)(exp(-0.5 * k * k / (sigma_px * sigma_px)) / sum);
         }
         LYA_CUDA(ctx, cudaMemcpyAsync(ctx->d_taps, ctx->h_taps, (size_t)n_t * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
         a.taps = ctx->d_taps;
     }
+    const int nv = (a.n4 / 4 + threads - 1) / threads;                 // float4 per thread and row
+    void (*kern)(const ObsArgs) = nullptr;
+    int D = 1;
+    if (nv <= 1)       kern = fast ? observe_rows_kernel<1, 1, true> : observe_rows_kernel<1, 1, false>;
+    else if (nv <= 2)  kern = fast ? observe_rows_kernel<2, 1, true> : observe_rows_kernel<2, 1, false>;
+    else if (nv <= 4)  kern = fast ? observe_rows_kernel<4, 1, true> : observe_rows_kernel<4, 1, false>;
+    else if (nv <= 8)  kern = fast ? observe_rows_kernel<8, 1, true> : observe_rows_kernel<8, 1, false>;
+    else if (nv <= 16) kern = fast ? observe_rows_kernel<16, 1, true> : observe_rows_kernel<16, 1, false>;
+    else return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: more than 16384 pixels per row");
     const int halo = a.L >= 0 ? a.L : 0;
-    const size_t smem = ((size_t)a.n4 + ((halo + 3) & ~3) + 8 + a.n4 + (((halo + 11) + 3) & ~3)) * sizeof(float);
+    const size_t smem = ((size_t)D * (a.n4 + ((halo + 3) & ~3) + 8) + (size_t)D * a.n4 + (((halo + 11) + 3) & ~3)) * sizeof(float);
     if (smem > (size_t)ctx->max_smem_optin) return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: row too long for shared memory");
-    int threads = ((a.n4 / 4 + 31) / 32) * 32;
-    threads = threads < 32 ? 32 : (threads > 256 ? 256 : threads);
-    LYA_CUDA(ctx, cudaFuncSetAttribute(observe_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    LYA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
-    LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, observe_rows_kernel, threads, smem));
+    LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
     if (per_sm < 1) return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: row too long for shared memory");
     const size_t cap = (size_t)ctx->sm_count * per_sm;
-    const int grid = (int)(n_rows < cap ? n_rows : cap);
-    observe_rows_kernel<<<grid, threads, smem, ctx->stream>>>(a);
+    const size_t n_batches = (n_rows + D - 1) / D;
+    const int grid = (int)(n_batches < cap ? n_batches : cap);
+    kern<<<grid, threads, smem, ctx->stream>>>(a);
     ctx->launches++;
     LYA_CUDA(ctx, cudaGetLastError());
     return LYA_OK;
