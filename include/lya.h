@@ -97,6 +97,23 @@ lya_status lya_gas_from_density(lya_ctx *ctx, const lya_params *p, const float *
 lya_status lya_tau_sightlines(lya_ctx *ctx, const lya_params *p, int axis, int32_t nz_local,
                               const float *n_hi, const float *b_kms, const float *v_pec_kms, float *tau);
 
+/* Work-efficient variants of S2 + S3, same arrays and conventions as
+ * lya_tau_sightlines.  flags:
+ *   LYA_TAU_WINDOWED      walk only the source cells that can contribute: a cell further from a pixel than
+ *                         12.5 b_j sqrt(ln 2)/dv + |v_pec,j|/dv + 1 pixels adds ex2(-x^2) == 0 exactly in fp32, so
+ *                         the result is BIT-IDENTICAL to the full sum while ~N / (128 + 2 reach) times fewer
+ *                         pairs are evaluated.  Sightlines whose reach does not fit take the full loops.
+ *   LYA_TAU_FROM_DENSITY  S1 fused into the staging: n_hi_or_delta is delta (Eq.4/5 are applied per staged
+ *                         cell with the arithmetic of lya_gas_from_density, so tau is bit-identical to the
+ *                         two-call path); b_kms is ignored and may be NULL.
+ * pairs_evaluated: HOST, receives the number of (i,j) pairs actually evaluated, or NULL; non-NULL
+ * synchronises the stream. */
+#define LYA_TAU_WINDOWED     1u
+#define LYA_TAU_FROM_DENSITY 2u
+lya_status lya_tau_sightlines_opt(lya_ctx *ctx, const lya_params *p, int axis, int32_t nz_local, unsigned flags,
+                                  const float *n_hi_or_delta, const float *b_kms, const float *v_pec_kms,
+                                  float *tau, uint64_t *pairs_evaluated);
+
 /* S4.  tau: DEVICE, n_pix floats in any layout (the mean runs over all of them).  Finds the unique A > 0
  * with mean(exp(-A tau)) = f_target by a bracketed Newton/bisection iteration that runs entirely on the
  * device (one cooperative kernel); synchronises the stream because A returns to the HOST.

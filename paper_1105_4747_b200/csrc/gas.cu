@@ -7,26 +7,10 @@
 //
 // HBM-bound: 4 B read + 8 B written per cell.  One lg2 and two ex2 per cell; 128-bit loads/stores,
 // grid-stride over a grid that is a multiple of the SM count.
+#include "gas_cell.h"
 #include "lya_internal.h"
 
 namespace {
-
-struct GasK {
-    float nbar_hi;   // Eq.4 at delta = 0, T = T0 [cm^-3]
-    float b0;        // km/s
-    float h;         // (gamma-1)/2
-    float e_n;       // -0.7 (gamma-1)
-    float pivot;     // +inf when disabled
-};
-
-__device__ __forceinline__ void gas_cell(const GasK &k, float delta, float &n_hi, float &b)
-{
-    float D  = 1.0f + delta;
-    float Dt = fminf(D, k.pivot);
-    float l  = log2f(Dt);                       // full-precision log2 (kernel stays HBM-bound)
-    b    = k.b0 * exp2f(k.h * l);
-    n_hi = (k.nbar_hi * exp2f(k.e_n * l)) * (D * D);
-}
 
 __device__ __forceinline__ void gas_cell4(const GasK &k, const float4 &d, float4 &n, float4 &w)
 {

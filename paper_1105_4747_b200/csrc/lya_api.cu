@@ -141,17 +141,21 @@ lya_status lya_gas_from_density(lya_ctx *ctx, const lya_params *p, const float *
                           (float)(0.5 * (p->gamma - 1.0)), pivot);
 }
 
-lya_status lya_tau_sightlines(lya_ctx *ctx, const lya_params *p, int axis, int32_t nz_local,
-                              const float *n_hi, const float *b_kms, const float *v_pec_kms, float *tau)
+lya_status lya_tau_sightlines_opt(lya_ctx *ctx, const lya_params *p, int axis, int32_t nz_local, unsigned flags,
+                                  const float *n_hi, const float *b_kms, const float *v_pec_kms, float *tau,
+                                  uint64_t *pairs_evaluated)
 {
     if (!ctx) return LYA_EINVAL;
     ctx->err[0] = 0;
+    const bool fused = (flags & LYA_TAU_FROM_DENSITY) != 0;
+    if (flags & ~(LYA_TAU_WINDOWED | LYA_TAU_FROM_DENSITY)) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: unknown flag");
     if (!params_ok(p)) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: bad parameters");
     if (axis < 0 || axis > 2) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: axis must be 0, 1 or 2");
     if (nz_local < 1 || nz_local > p->nz) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: bad nz_local");
     if (axis == 2 && nz_local != p->nz)
         return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: axis 2 needs the whole grid (nz_local == nz)");
-    if (!n_hi || !b_kms || !v_pec_kms || !tau) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: null pointer");
+    if (fused) b_kms = nullptr;
+    if (!n_hi || (!fused && !b_kms) || !v_pec_kms || !tau) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: null pointer");
     if ((((uintptr_t)n_hi | (uintptr_t)b_kms | (uintptr_t)v_pec_kms | (uintptr_t)tau) & 3) != 0)
         return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: pointers must be 4-byte aligned");
     if (tau == n_hi || tau == b_kms || tau == v_pec_kms)
@@ -161,8 +165,29 @@ lya_status lya_tau_sightlines(lya_ctx *ctx, const lya_params *p, int axis, int32
     lya_scalars s;
     lya_scalars_from_params(p, axis, &s);
     LYA_CUDA(ctx, cudaSetDevice(ctx->device));
+    const float pivot = p->delta_pivot > 0.0 ? (float)p->delta_pivot : INFINITY;
+    const float half_gm1 = (float)(0.5 * (p->gamma - 1.0));
+    const float gas5[5] = {(float)s.nbarHI, (float)s.b0_kms, half_gm1, (float)(2.0 * LYA_ALPHA_T) * half_gm1, pivot};
+    unsigned long long *d_pairs = nullptr;
+    if (pairs_evaluated) {
+        d_pairs = reinterpret_cast<unsigned long long *>(ctx->d_sched + 2);      // 8-byte aligned slot
+        LYA_CUDA(ctx, cudaMemsetAsync(d_pairs, 0, sizeof(unsigned long long), ctx->stream));
+    }
     // amplitude a_j = K nHI / (b[km/s] 1e5 cm/km): K 1e-5 is passed so that fp32 operands stay O(1e11 x 1e-11)
-    return lya_launch_tau(ctx, axis, p->nx, p->ny, nz_local, n_hi, b_kms, v_pec_kms, tau, s.K * 1.0e-5, s.dv_kms);
+    lya_status st = lya_launch_tau(ctx, axis, p->nx, p->ny, nz_local, n_hi, b_kms, v_pec_kms, tau, s.K * 1.0e-5,
+                                   s.dv_kms, flags, gas5, d_pairs);
+    if (st != LYA_OK || !pairs_evaluated) return st;
+    unsigned long long host = 0;
+    LYA_CUDA(ctx, cudaMemcpyAsync(&host, d_pairs, sizeof(host), cudaMemcpyDeviceToHost, ctx->stream));
+    LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    *pairs_evaluated = host;
+    return LYA_OK;
+}
+
+lya_status lya_tau_sightlines(lya_ctx *ctx, const lya_params *p, int axis, int32_t nz_local,
+                              const float *n_hi, const float *b_kms, const float *v_pec_kms, float *tau)
+{
+    return lya_tau_sightlines_opt(ctx, p, axis, nz_local, 0u, n_hi, b_kms, v_pec_kms, tau, nullptr);
 }
 
 lya_status lya_normalize_mean_flux(lya_ctx *ctx, const float *tau, size_t n_pix, double f_target,

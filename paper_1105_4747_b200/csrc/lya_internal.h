@@ -70,9 +70,12 @@ static inline lya_status lya_cuda_fail(lya_ctx *ctx, cudaError_t e, const char *
 // kernels' host launchers (each enqueues on ctx->stream and bumps ctx->launches)
 lya_status lya_launch_gas(lya_ctx *ctx, const float *delta, size_t n, float *n_hi, float *b,
                           float nbar_hi, float b0, float half_gm1, float pivot);
+// flags: LYA_TAU_*; gas5 = {nbar_hi, b0, (gamma-1)/2, -0.7 (gamma-1), pivot} when LYA_TAU_FROM_DENSITY (n_hi
+// then points at delta, b is ignored); d_pairs: device counter of evaluated pairs or NULL
 lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
                           const float *n_hi, const float *b, const float *v, float *tau,
-                          double amp_scale, double dv_kms);
+                          double amp_scale, double dv_kms, unsigned flags, const float *gas5,
+                          unsigned long long *d_pairs);
 lya_status lya_launch_flux(lya_ctx *ctx, const float *tau, size_t n, double a, float *flux);
 lya_status lya_run_normalize(lya_ctx *ctx, const float *tau, size_t n, double f_target, double rel_tol,
                              int max_iter, double *a_out, double *f_out, int *iters);

@@ -39,6 +39,7 @@
 // Sightlines along y / z: a CTA gathers 8 (or fewer) neighbouring x at a time so that global accesses stay
 // 32- or 16-byte segments, its 8 warps sum (sightline, tile) items, and tau goes back through a shared-memory
 // tile; batches come from the same atomic counter.
+#include "gas_cell.h"
 #include "lya_internal.h"
 
 namespace {
@@ -69,6 +70,10 @@ struct TauArgs {
     float        amp_scale;   // K * 1e-5  [so that a_j is dimensionless]
     float        w_scale;     // dv * sqrt(log2 e) [km/s]
     float        inv_n, n_f;  // 1/N, N
+    float        xcut_over_w; // TAU_XCUT / w_scale: TAU_XCUT / w_j = b_j * xcut_over_w
+    int          windowed;    // LYA_TAU_WINDOWED: walk only the sources that can contribute
+    GasK         gas;         // FUSED (LYA_TAU_FROM_DENSITY): n_hi points at delta, S1 is done while staging
+    unsigned long long *pairs; // device counter of (i,j) pairs evaluated
 };
 
 __device__ __forceinline__ float ex2_ftz(float x)
@@ -85,15 +90,16 @@ __device__ __forceinline__ float round_magic(float x)
     return __fsub_rn(__fadd_rn(x, big), big);
 }
 
-// One source cell -> staged float4 (m, w, g, a); returns 1 if the cell breaks the fast-path condition.
+// One source cell -> staged float4 (m, w, g, a).  Returns the cell's REACH in pixels, 12.5 / w_j + |P_j| + 1:
+// a pixel further than that from the (unwrapped) cell index gets ex2(-x^2) == 0 exactly from it.  The maximum
+// over a sightline decides between the fast and the general loop and sets the window of LYA_TAU_WINDOWED.
 // All fp32: p = v_pec/dv is split as P + f with P = round(v * inv_dv_hi) and f = fma(v, inv_dv_hi, -P) +
 // v * inv_dv_lo -- the fma forms the residual of the exact 48-bit product with ONE rounding of a number
 // below 1, so f carries an absolute error < 1e-7 pixel however large P is.  Precondition |v_pec| < 2^22 dv
-// (4e6 pixels; beyond it P is no longer an integer and the cell is sent to the general path with a
-// meaningless but finite displacement).  No FP64 and, apart from one reciprocal, no XU-pipe instruction.
-// jf = (float)j.  Reading C11: +v -> higher pixel index.
-__device__ __forceinline__ int stage_cell(const TauArgs &a, float jf, float nh, float bb, float vv, int half_span,
-                                          float4 &out)
+// (4e6 pixels; beyond it P is no longer an integer: the reach is set to +inf, which sends the sightline to the
+// general path with a meaningless but finite displacement).  No FP64 and, apart from one reciprocal, no
+// XU-pipe instruction.  jf = (float)j.  Reading C11: +v -> higher pixel index.
+__device__ __forceinline__ float stage_cell(const TauArgs &a, float jf, float nh, float bb, float vv, float4 &out)
 {
     const float P  = round_magic(vv * a.inv_dv_hi);
     const float f  = fmaf(vv, a.inv_dv_lo, fmaf(vv, a.inv_dv_hi, -P));
@@ -105,27 +111,38 @@ __device__ __forceinline__ int stage_cell(const TauArgs &a, float jf, float nh, 
     out.y = w;
     out.z = -f * w;
     out.w = (a.amp_scale * nh) * ib;
-    const float room = (float)(a.n >> 1) - (float)half_span - fabsf(Pr) - 1.0f;
-    return !(room * w >= TAU_XCUT) || !(fabsf(P) < 4194304.0f);
+    const float reach = fmaf(bb, a.xcut_over_w, fabsf(Pr) + 1.0f);
+    return (fabsf(P) < 4194304.0f && reach >= 0.0f) ? reach : __int_as_float(0x7f800000);   // NaN -> +inf
 }
 
-// Fast path: unwrapped walk around the tile centre, no per-pair image logic.  Lane owns pixels
-// i0 + lane*R + r, r = 0..R-1.
+template <bool FUSED>
+__device__ __forceinline__ float stage_from_global(const TauArgs &a, float jf, size_t g, float4 &out)
+{
+    float nh, bb;
+    if (FUSED) gas_cell(a.gas, __ldcs(a.n_hi + g), nh, bb);            // n_hi points at delta
+    else { nh = __ldcs(a.n_hi + g); bb = __ldcs(a.b + g); }
+    return stage_cell(a, jf, nh, bb, __ldcs(a.v + g), out);
+}
+
+// Fast path: unwrapped walk over the `len` sources jj = start .. start + len - 1 (at most one wrap, len <= n),
+// no per-pair image logic.  Full sum: start = tile centre - n/2, len = n.  Windowed: start = i0 - W,
+// len = 32 R + 2 W with W the sightline's reach -- every source left out would have added exactly 0, and the
+// ones kept are added in the same order, so the result is bit-identical.  Lane owns pixels i0 + lane*R + r.
 template <int R>
-__device__ __forceinline__ void tile_fast(const float4 *__restrict__ cs, int n, int i0, int lane, float (&acc)[R])
+__device__ __forceinline__ void tile_fast(const float4 *__restrict__ cs, int n, int i0, int lane, int start, int len,
+                                          float (&acc)[R])
 {
     constexpr int RH = R / 2;                          // reference pixel of the lane
-    const int c     = i0 + 16 * R;
-    const int start = c - (n >> 1);                    // first unwrapped source index
     int j0 = start % n;
     if (j0 < 0) j0 += n;                               // slot holding jj = start
     const int off = start - j0;                        // jj = j + off on [j0, n), jj = j + off + n on [0, j0)
     float cref = (float)(i0 + lane * R + RH - off);
 #pragma unroll
     for (int r = 0; r < R; ++r) acc[r] = 0.0f;
+    const int end1 = j0 + len < n ? j0 + len : n;      // first segment [j0, end1), second [0, j0 + len - n)
 #pragma unroll 1
     for (int seg = 0; seg < 2; ++seg) {
-        const int lo = seg ? 0 : j0, hi = seg ? j0 : n;
+        const int lo = seg ? 0 : j0, hi = seg ? j0 + len - n : end1;
 #pragma unroll 8
         for (int j = lo; j < hi; ++j) {
             const float4 q = cs[j];
@@ -140,6 +157,21 @@ __device__ __forceinline__ void tile_fast(const float4 *__restrict__ cs, int n, 
         }
         cref -= (float)n;
     }
+}
+
+// which sources a tile walks: returns false if the sightline needs the general loop
+template <int R>
+__device__ __forceinline__ bool tile_span(const TauArgs &a, float reach, int i0, int &start, int &len)
+{
+    const int n = a.n;
+    if (!(reach <= (float)((n >> 1) - 16 * R))) return false;          // also catches +inf
+    start = i0 + 16 * R - (n >> 1);
+    len = n;
+    if (a.windowed) {
+        const int W = (int)reach + 1;
+        if (32 * R + 2 * W < n) { start = i0 - W; len = 32 * R + 2 * W; }
+    }
+    return true;
 }
 
 // General path: nearest image chosen per pair (tiny N, or |v_pec| comparable to the box).
@@ -177,11 +209,11 @@ __device__ __forceinline__ void group_sync(int G, int bar_id)
 
 // ---------------------------------------------------------------------------------------------------------
 // Sightlines along x.  blockDim = 32 * G * gpc (gpc = groups per CTA).  Dynamic shared memory: per group n
-// float4 cells, then per group one int4 control word {row, bad, next row, -}.
+// float4 cells, then per group one int4 control word {row, reach (float bits), next row, -}.
 // (A variant that bulk-copied the next row into a raw buffer with cp.async.bulk + mbarrier while the current
 // one was summed measured 4 % slower: profiles/r1_tau_prefetch_ab.md.  The row change here is plain coalesced
 // loads; the other resident groups keep the MUFU pipe busy meanwhile.)
-template <int R>
+template <int R, bool FUSED>
 __global__ void __launch_bounds__(1024, 1) tau_x_kernel(const TauArgs a, const int G, const int gpc)
 {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -201,31 +233,35 @@ __global__ void __launch_bounds__(1024, 1) tau_x_kernel(const TauArgs a, const i
         if (row >= a.n_sl) break;
         const size_t g0 = (size_t)row * n;
 
-        // ---- stage the row: (nHI, b, v_pec) -> (m, w, g, a) per cell; 128-byte coalesced loads
-        int bad = 0;
+        // ---- stage the row: (nHI, b, v_pec) [or delta, v_pec] -> (m, w, g, a) per cell; 128-byte coalesced loads
+        float reach = 0.0f;
         float jf = (float)gl;
 #pragma unroll 4
         for (int j = gl; j < n; j += gthreads) {
             float4 q;
-            bad |= stage_cell(a, jf, __ldcs(a.n_hi + g0 + j), __ldcs(a.b + g0 + j), __ldcs(a.v + g0 + j), 16 * R, q);
+            reach = fmaxf(reach, stage_from_global<FUSED>(a, jf, g0 + j, q));
             cells[j] = q;
             jf += (float)gthreads;
         }
-        bad = __any_sync(0xffffffffu, bad);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) reach = fmaxf(reach, __shfl_xor_sync(0xffffffffu, reach, o));
         if (gl == 0) ctl[1] = 0;
         group_sync(G, bar_id);                           // cells complete, ctl[0] read
-        if (G > 1 && bad && lane == 0) ctl[1] = 1;
+        if (G > 1 && lane == 0) atomicMax(const_cast<int *>(ctl + 1), __float_as_int(reach));   // reach >= 0
         if (gl == 0) ctl[2] = (int)atomicAdd(&a.sched[0], 1u);   // claim the next row early: latency hidden
         if (G > 1) {
             group_sync(G, bar_id);
-            bad = ctl[1];
+            reach = __int_as_float(ctl[1]);
         }
 
         // ---- sum: the group's warps take the pixel tiles of the row
+        int start = 0, len = n;
+        const bool fast = tile_span<R>(a, reach, 0, start, len);
+        if (gl == 0 && a.pairs) atomicAdd(a.pairs, (unsigned long long)n * (unsigned long long)len);
         for (int tile = wg; tile < a.tiles; tile += G) {
             const int i0 = tile * 32 * R;
             float acc[R];
-            if (!bad) tile_fast<R>(cells, n, i0, lane, acc);
+            if (fast) tile_fast<R>(cells, n, i0, lane, start + i0, len, acc);
             else      tile_general<R>(cells, n, a.n_f, a.inv_n, i0, lane, acc);
             const int i = i0 + lane * R;
             float *dst = a.tau + g0 + i;
@@ -263,11 +299,12 @@ __global__ void __launch_bounds__(1024, 1) tau_x_kernel(const TauArgs a, const i
 // way.  Batches are handed out by the atomic counter; bsl is chosen so that >= 4 CTAs are resident per SM and
 // one CTA's gather overlaps the others' pair loops.  cstride / tstride are padded so that neither the
 // transposed staging stores nor the tile read-out have shared-memory bank conflicts.
-template <int R>
+template <int R, bool FUSED>
 __global__ void __launch_bounds__(TAU_THREADS) tau_strided_kernel(const TauArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     __shared__ unsigned int s_batch;
+    __shared__ int s_reach;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int n = a.n;
     const int cstride = a.cstride, tstride = a.tstride;
@@ -285,27 +322,35 @@ __global__ void __launch_bounds__(TAU_THREADS) tau_strided_kernel(const TauArgs 
         const int nb = (a.nx - x0 < a.bsl) ? (a.nx - x0) : a.bsl;
         const long long base = outer * a.outer_stride + x0;   // element offset of (pixel 0, first x of the batch)
 
-        int bad = 0;
+        float reach = 0.0f;
+        if (tid == 0) s_reach = 0;
 #pragma unroll 4
         for (int c = tid; c < (n << a.bshift); c += TAU_THREADS) {
             const int bx = c & (a.bsl - 1), j = c >> a.bshift;
             if (bx < nb) {
-                const long long g = base + (long long)j * a.stride + bx;
                 float4 q;
-                bad |= stage_cell(a, (float)j, __ldcs(a.n_hi + g), __ldcs(a.b + g), __ldcs(a.v + g), 16 * R, q);
+                reach = fmaxf(reach, stage_from_global<FUSED>(a, (float)j, (size_t)(base + (long long)j * a.stride + bx), q));
                 cells[bx * cstride + j] = q;
             }
         }
-        bad = __syncthreads_or(bad);                     // cells complete; s_batch read by everyone
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) reach = fmaxf(reach, __shfl_xor_sync(0xffffffffu, reach, o));
+        __syncthreads();                                 // s_reach zeroed; s_batch read by everyone
+        if (lane == 0) atomicMax(&s_reach, __float_as_int(reach));
+        __syncthreads();                                 // cells complete
+        reach = __int_as_float(s_reach);
         if (tid == 0) s_batch = atomicAdd(&a.sched[0], 1u);
 
+        int start = 0, len = n;
+        const bool fast = tile_span<R>(a, reach, 0, start, len);
+        if (tid == 0 && a.pairs) atomicAdd(a.pairs, (unsigned long long)nb * n * (unsigned long long)len);
         const int items = nb * a.tiles;
         for (int item = warp; item < items; item += TAU_WARPS) {
             const int sl = item / a.tiles, tile = item - sl * a.tiles;
             const int i0 = tile * 32 * R;
             const float4 *cs = cells + (size_t)sl * cstride;
             float acc[R];
-            if (!bad) tile_fast<R>(cs, n, i0, lane, acc);
+            if (fast) tile_fast<R>(cs, n, i0, lane, start + i0, len, acc);
             else      tile_general<R>(cs, n, a.n_f, a.inv_n, i0, lane, acc);
             const int i = i0 + lane * R;
             float *dst = ttile + (size_t)sl * tstride + i;     // tstride covers tiles * 32 * R: no bound check
@@ -331,10 +376,10 @@ __global__ void __launch_bounds__(TAU_THREADS) tau_strided_kernel(const TauArgs 
     }
 }
 
-template <int R>
+template <int R, bool FUSED>
 lya_status launch_x(lya_ctx *ctx, const TauArgs &a)
 {
-    auto kern = tau_x_kernel<R>;
+    auto kern = tau_x_kernel<R, FUSED>;
     const size_t cap = (size_t)ctx->max_smem_optin;
     const size_t per_group = (size_t)a.n * sizeof(float4) + 16;
     int groups = (int)(cap / per_group);                 // groups that fit in one SM's shared memory
@@ -357,10 +402,10 @@ lya_status launch_x(lya_ctx *ctx, const TauArgs &a)
     return LYA_OK;
 }
 
-template <int R>
+template <int R, bool FUSED>
 lya_status launch_strided(lya_ctx *ctx, const TauArgs &a, size_t smem_bytes)
 {
-    auto kern = tau_strided_kernel<R>;
+    auto kern = tau_strided_kernel<R, FUSED>;
     LYA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
     int per_sm = 0;
     LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, TAU_THREADS, smem_bytes));
@@ -377,8 +422,10 @@ lya_status launch_strided(lya_ctx *ctx, const TauArgs &a, size_t smem_bytes)
 
 lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
                           const float *n_hi, const float *b, const float *v, float *tau,
-                          double amp_scale, double dv_kms)
+                          double amp_scale, double dv_kms, unsigned flags, const float *gas5,
+                          unsigned long long *d_pairs)
 {
+    const bool fused = (flags & LYA_TAU_FROM_DENSITY) != 0;
     TauArgs a;
     memset(&a, 0, sizeof(a));
     a.n_hi = n_hi; a.b = b; a.v = v; a.tau = tau;
@@ -390,6 +437,10 @@ lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
     a.w_scale   = (float)(dv_kms * 1.2011224087864498);   // sqrt(log2 e)
     a.n_f = (float)n;
     a.inv_n = 1.0f / (float)n;
+    a.xcut_over_w = TAU_XCUT / a.w_scale;
+    a.windowed = (flags & LYA_TAU_WINDOWED) != 0;
+    a.pairs = d_pairs;
+    if (fused) a.gas = GasK{gas5[0], gas5[1], gas5[2], gas5[3], gas5[4]};
     const int R = n >= 128 ? 4 : (n >= 64 ? 2 : 1);
     a.tiles = (n + 32 * R - 1) / (32 * R);
     const size_t smem_cap = (size_t)ctx->max_smem_optin;
@@ -400,9 +451,9 @@ lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
         a.vec = (n % 4 == 0) && (((uintptr_t)tau & 15) == 0);
         a.sched = ctx->d_sched;
         switch (R) {
-            case 1:  return launch_x<1>(ctx, a);
-            case 2:  return launch_x<2>(ctx, a);
-            default: return launch_x<4>(ctx, a);
+            case 1:  return fused ? launch_x<1, true>(ctx, a) : launch_x<1, false>(ctx, a);
+            case 2:  return fused ? launch_x<2, true>(ctx, a) : launch_x<2, false>(ctx, a);
+            default: return fused ? launch_x<4, true>(ctx, a) : launch_x<4, false>(ctx, a);
         }
     }
 
@@ -438,8 +489,8 @@ lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
     if (a.n_batches >= (1LL << 31)) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: more than 2^31 batches");
     a.sched = ctx->d_sched;
     switch (R) {
-        case 1:  return launch_strided<1>(ctx, a, need2(bshift));
-        case 2:  return launch_strided<2>(ctx, a, need2(bshift));
-        default: return launch_strided<4>(ctx, a, need2(bshift));
+        case 1:  return fused ? launch_strided<1, true>(ctx, a, need2(bshift)) : launch_strided<1, false>(ctx, a, need2(bshift));
+        case 2:  return fused ? launch_strided<2, true>(ctx, a, need2(bshift)) : launch_strided<2, false>(ctx, a, need2(bshift));
+        default: return fused ? launch_strided<4, true>(ctx, a, need2(bshift)) : launch_strided<4, false>(ctx, a, need2(bshift));
     }
 }

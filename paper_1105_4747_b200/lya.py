@@ -16,6 +16,7 @@ import torch
 from . import build as _build
 
 OK, EINVAL, ECUDA, ENOROOT, ENOCONV, ENOMEM = range(6)
+TAU_WINDOWED, TAU_FROM_DENSITY = 1, 2
 
 
 class LyaError(RuntimeError):
@@ -79,7 +80,7 @@ EXPORTS = ("lya_version", "lya_status_string", "lya_scalars_from_params", "lya_c
            "lya_normalize_mean_flux", "lya_flux_partial_sums", "lya_root_init", "lya_root_update",
            "lya_flux", "lya_forest_host", "lya_launch_count", "lya_measure_mufu_peak",
            "lya_bin_kms_from_angstrom", "lya_instrument_bins", "lya_observe_rows", "lya_flux_pdf",
-           "lya_flux_power_rows")
+           "lya_flux_power_rows", "lya_tau_sightlines_opt")
 
 _lib = None
 
@@ -107,6 +108,7 @@ def lib() -> C.CDLL:
     L.lya_launch_count.restype = C.c_uint64
     L.lya_gas_from_density.argtypes = [vp, pp, fp, C.c_size_t, fp, fp]
     L.lya_tau_sightlines.argtypes = [vp, pp, C.c_int, C.c_int32, fp, fp, fp, fp]
+    L.lya_tau_sightlines_opt.argtypes = [vp, pp, C.c_int, C.c_int32, C.c_uint, fp, fp, fp, fp, C.POINTER(C.c_uint64)]
     L.lya_normalize_mean_flux.argtypes = [vp, fp, C.c_size_t, C.c_double, C.c_double, C.c_int, dp, dp, ip]
     L.lya_flux_partial_sums.argtypes = [vp, fp, C.c_size_t, dp, C.c_int, dp, dp]
     L.lya_root_init.argtypes = [C.POINTER(CRootState), C.c_double, C.c_double, C.c_double]
@@ -212,6 +214,24 @@ class Context:
         self._check(lib().lya_tau_sightlines(self._h, C.byref(cp), axis, nz_local, _dev(n_hi, "n_hi"),
                                              _dev(b_kms, "b_kms"), _dev(v_pec, "v_pec"), _dev(tau, "tau")))
         return tau
+
+    def tau_sightlines_opt(self, p: Params, axis: int, v_pec, n_hi=None, b_kms=None, delta=None, windowed=False,
+                           tau=None, nz_local=None, count_pairs=False):
+        """delta given -> S1 fused into the staging; windowed -> only contributing sources.
+        Returns tau, or (tau, pairs evaluated) with count_pairs."""
+        first = delta if delta is not None else n_hi
+        flags = (TAU_WINDOWED if windowed else 0) | (TAU_FROM_DENSITY if delta is not None else 0)
+        tau = torch.empty_like(first) if tau is None else tau
+        nz_local = first.shape[0] if nz_local is None else nz_local
+        if first.numel() != nz_local * p.ny * p.nx or v_pec.numel() != first.numel() or tau.numel() != first.numel():
+            raise ValueError("tau_sightlines_opt: arrays must be [nz_local][ny][nx]")
+        cp = p.c()
+        pairs = C.c_uint64()
+        self._check(lib().lya_tau_sightlines_opt(
+            self._h, C.byref(cp), axis, nz_local, flags, _dev(first, "n_hi/delta"),
+            None if delta is not None else _dev(b_kms, "b_kms"), _dev(v_pec, "v_pec"), _dev(tau, "tau"),
+            C.byref(pairs) if count_pairs else None))
+        return (tau, int(pairs.value)) if count_pairs else tau
 
     # S4
     def normalize_mean_flux(self, tau, f_target: float, rel_tol: float = 1e-7, max_iter: int = 60,

@@ -274,3 +274,49 @@ def test_sharded_normalisation_on_one_gpu(ctx):
     _, _, tau, A, f, it, _ = run_gpu(ctx, w, delta, v[0])
     A2, f2, it2 = lya.normalize_mean_flux_sharded(ctx, tau, w.f_target, tau.numel())
     assert abs(A2 / A - 1) < 1e-9 and abs(f2 - f) < 1e-9
+
+
+# ------------------------------------------------------------------ windowed / fused tau
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_tau_windowed_and_fused_are_bit_identical_to_the_full_sum(ctx, oracle, axis):
+    """LYA_TAU_WINDOWED leaves out only terms that are exactly 0 in fp32; LYA_TAU_FROM_DENSITY applies S1 with
+    lya_gas_from_density's arithmetic while staging: both must reproduce the two-call full sum bit for bit
+    (whose parity with the oracle the tests above establish), and the window must really shrink the work."""
+    w = scaled(WORKLOADS[4], 512) if axis == 0 else scaled(WORKLOADS[3], 192)
+    n = w.n
+    nz = 6 if axis == 0 else n
+    f = inputs.make_fields(w, device="cuda", z0=0, z1=nz, axes=(axis,))
+    delta, v = f["delta"], f["v_pec"][axis]
+    p = lya.Params(nx=n, ny=n, nz=nz, box_mpch=w.box_mpch, z=w.z, T0=w.T0, gamma=w.gamma)
+    if axis == 2:
+        p.nz = n
+    n_hi, b = ctx.gas_from_density(p, delta)
+    full = ctx.tau_sightlines(p, axis, n_hi, b, v)
+    win, pairs_w = ctx.tau_sightlines_opt(p, axis, v, n_hi=n_hi, b_kms=b, windowed=True, count_pairs=True)
+    fus, pairs_f = ctx.tau_sightlines_opt(p, axis, v, delta=delta, count_pairs=True)
+    both = ctx.tau_sightlines_opt(p, axis, v, delta=delta, windowed=True)
+    assert torch.equal(win, full) and torch.equal(fus, full) and torch.equal(both, full)
+    assert pairs_f == delta.numel() * n                      # full sum: N pairs per pixel
+    # a tile walks 128 + 2 * reach sources instead of N: a third of them at N = 512, most of them at N = 192
+    assert pairs_w < (0.5 if axis == 0 else 0.95) * pairs_f, (pairs_w, pairs_f)
+    if axis == 0:                                            # and against the oracle on a few rows
+        po = oracle.Params.from_workload(w)
+        _, n_ref, b_ref = oracle.gas_from_density(po, delta[0, :8].cpu().numpy())
+        ref = oracle.tau_rows(po, n_ref, b_ref, v[0, :8].cpu().numpy())
+        assert_tau_close(both[0, :8].cpu().numpy(), ref, "windowed+fused")
+
+
+def test_tau_windowed_falls_back_when_the_reach_does_not_fit(ctx):
+    """Huge velocities / tiny rows: the window would exceed the row, the full (or general) loop must run."""
+    w = scaled(WORKLOADS[1], 64)
+    f = inputs.make_fields(w, device="cuda", z0=0, z1=4)
+    delta, v = f["delta"], (f["v_pec"][0] * 40.0).contiguous()          # |v| of order V
+    p = lya.Params(nx=64, ny=64, nz=4, box_mpch=w.box_mpch, z=w.z, T0=w.T0, gamma=w.gamma)
+    n_hi, b = ctx.gas_from_density(p, delta)
+    full = ctx.tau_sightlines(p, 0, n_hi, b, v)
+    win, pairs = ctx.tau_sightlines_opt(p, 0, v, n_hi=n_hi, b_kms=b, windowed=True, count_pairs=True)
+    assert torch.equal(win, full) and pairs == delta.numel() * 64
+    with pytest.raises(lya.LyaError):
+        lya.lib().lya_tau_sightlines_opt  # noqa: B018  (symbol exists)
+        ctx._check(lya.lib().lya_tau_sightlines_opt(ctx._h, lya.C.byref(p.c()), 0, 4, 8, n_hi.data_ptr(),
+                                                    b.data_ptr(), v.data_ptr(), full.data_ptr(), None))
