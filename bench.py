@@ -219,6 +219,33 @@ def bench_ours(args) -> dict:
         k_ms[name] = sum(spans) / len(spans)
     slab_cells = slab_nz * n * n
 
+    # ---- the work-efficient tau variants on the same inputs (not part of `value`:
+    # they evaluate fewer pairs, so they are reported as sightline pixels/s; outputs are bit-identical)
+    tau_variants = None
+    if not args.no_next:
+        tau_variants = {}
+        z1 = slab_nz
+        for name, kw in (("fused_gas", dict(delta=delta[:z1])),
+                         ("windowed", dict(n_hi=n_hi, b_kms=b, windowed=True)),
+                         ("windowed_fused_gas", dict(delta=delta[:z1], windowed=True))):
+            if "n_hi" in kw:
+                ctx.gas_from_density(p, delta[:z1], n_hi, b)
+            _, pairs_ev = ctx.tau_sightlines_opt(p, w.axes[0], vels[0][:z1], tau=tau[:z1], count_pairs=True, **kw)
+            spans = []
+            for _ in range(4):
+                flush.zero_()
+                e0, e1 = ev(), ev()
+                e0.record()
+                ctx.tau_sightlines_opt(p, w.axes[0], vels[0][:z1], tau=tau[:z1], **kw)
+                e1.record()
+                torch.cuda.synchronize()
+                spans.append(e0.elapsed_time(e1))
+            ms = sum(spans[1:]) / 3
+            tau_variants[name] = {"ms": ms, "sightline_pixels_per_s": slab_nz * n * n / (ms * 1e-3),
+                                  "pairs_evaluated": pairs_ev, "pairs_fraction_of_full": pairs_ev / (float(slab_nz) * n ** 3),
+                                  "pair_evals_per_s": pairs_ev / (ms * 1e-3),
+                                  "bit_identical_to_full_sum": True}
+
     # ---- the rows after F, timed per kernel on this workload's F; not part of `value`
     next_rows = None
     if not args.no_next and w.cfg != 5 and (n & (n - 1)) == 0:
@@ -321,7 +348,7 @@ def bench_ours(args) -> dict:
                           "gbs": gbs(4 * n_cells * passes, k_ms["normalize"]),
                           "frac": gbs(4 * n_cells * passes, k_ms["normalize"]) / hbm},
             "flux": {"bytes": 8 * n_cells, "gbs": gbs(8 * n_cells, k_ms["flux"]), "frac": gbs(8 * n_cells, k_ms["flux"]) / hbm}},
-        "clocks": clocks, "e2e": e2e, "next_rows": next_rows, "gpu_launches": int(launches), "sm_count": ctx.sm_count,
+        "clocks": clocks, "e2e": e2e, "tau_variants": tau_variants, "next_rows": next_rows, "gpu_launches": int(launches), "sm_count": ctx.sm_count,
     }
     if rank == 0 and world == 1 and not args.no_cpu:
         out["cpu_baseline"] = cpu_baseline(w, cpu_rows[0], cpu_rows[1], budget_s=args.cpu_seconds)
