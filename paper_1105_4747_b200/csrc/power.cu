@@ -2,11 +2,14 @@
 //   P(k_m) = (V/N^2) < |sum_i dF_i exp(-2 pi i m i / N)|^2 >,  dF = F / <F> - 1,  m = 0 .. N/2   (reading O5)
 //
 // One CTA transforms two rows at a time as ONE complex FFT (row A in the real part, row B in the imaginary
-// part; X_A(m) = (Z(m) + conj Z(N-m))/2, X_B(m) = (Z(m) - conj Z(N-m))/(2i)): an iterative radix-2
-// decimation-in-time FFT in shared memory (bit-reversed load, log2 N butterfly stages, twiddles from a
-// shared table built once per CTA with sincospif), |X|^2 accumulated in double per CTA and added to the
-// global accumulator once at the end.  4 B read per pixel; the butterflies make it shared-memory bound, not
-// HBM bound.
+// part; X_A(m) = (Z(m) + conj Z(N-m))/2, X_B(m) = (Z(m) - conj Z(N-m))/(2i)).  The FFT is a Stockham
+// autosort transform in 1-4 passes of radix 16 / 8 / 4: a thread loads R points (the first pass straight
+// from global memory, coalesced), applies the pass twiddles (one table look-up, the powers by at most four
+// complex products), does the R-point DFT in registers (radix-2 DIF with compile-time constants) and
+// scatters the result to the other shared-memory buffer, whose index is padded by one slot in 16 so that the
+// stride-R scatter of the first pass is bank-conflict free.  |X|^2 is accumulated in double per CTA and added
+// to the global accumulator once at the end.  4 B read per pixel; N = 1024 makes 3 passes = 2 shared-memory
+// round trips per point (the radix-2 version this replaces made 10, with a barrier each).
 #include "lya_internal.h"
 
 namespace {
@@ -15,23 +18,102 @@ struct PowArgs {
     const float *flux;
     size_t       n_rows;
     int          n, log2n;
+    int          n_pass, radix[4];
     float        inv_mean;
     double      *acc;          // device, n/2 + 1 doubles, zeroed by the host
 };
 
+__device__ __forceinline__ float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
+__device__ __forceinline__ int pad16(int i) { return i + (i >> 4); }
+
+// R-point DFT in registers, radix-2 decimation in frequency: the result for frequency t ends up in
+// v[bitrev_R(t)].  All indices and twiddles are compile-time constants once unrolled.
+template <int R>
+__device__ __forceinline__ void dft_regs(float2 (&v)[R])
+{
+    constexpr float C[8] = {1.0f, 0.92387953251128674f, 0.70710678118654752f, 0.38268343236508977f,
+                            0.0f, -0.38268343236508977f, -0.70710678118654752f, -0.92387953251128674f};
+    constexpr float S[8] = {0.0f, 0.38268343236508977f, 0.70710678118654752f, 0.92387953251128674f,
+                            1.0f, 0.92387953251128674f, 0.70710678118654752f, 0.38268343236508977f};
+#pragma unroll
+    for (int len = R; len >= 2; len >>= 1) {
+        const int half = len >> 1;
+#pragma unroll
+        for (int s = 0; s < R; s += len) {
+#pragma unroll
+            for (int p = 0; p < half; ++p) {
+                const float2 a = v[s + p], b = v[s + p + half];
+                v[s + p] = make_float2(a.x + b.x, a.y + b.y);
+                const float2 d = make_float2(a.x - b.x, a.y - b.y);
+                const int q = p * (16 / len);              // W_len^p = exp(-2 pi i q / 16), q < 8
+                if (q == 0)      v[s + p + half] = d;
+                else if (q == 4) v[s + p + half] = make_float2(d.y, -d.x);          // times -i
+                else             v[s + p + half] = cmul(d, make_float2(C[q], -S[q]));
+            }
+        }
+    }
+}
+
+template <int R> __device__ __forceinline__ constexpr int bitrev(int t)
+{
+    int r = 0;
+    for (int b = 1; b < R; b <<= 1) { r = (r << 1) | (t & 1); t >>= 1; }
+    return r;
+}
+
+// One Stockham pass of radix R.  ns = product of the radices of the passes already done.
+//   v[t] = in[j + t N/R] ;  v[t] *= exp(-2 pi i t k / (ns R)), k = j mod ns ;  V = DFT_R(v) ;
+//   out[(j - k) R + k + t ns] = V[t]
+// FIRST: `in` is global memory (two rows -> one complex sequence, dF = F inv_mean - 1).
+template <int R, bool FIRST>
+__device__ __forceinline__ void stockham_pass(const PowArgs &a, const float *ra, const float *rb, bool has_b,
+                                              const float2 *in, float2 *out, const float2 *tw, int ns)
+{
+    const int n = a.n, m = n / R;
+    for (int j = threadIdx.x; j < m; j += blockDim.x) {
+        float2 v[R];
+#pragma unroll
+        for (int t = 0; t < R; ++t) {
+            const int i = j + t * m;
+            if (FIRST) {
+                const float fa = fmaf(__ldcs(ra + i), a.inv_mean, -1.0f);
+                const float fb = has_b ? fmaf(__ldcs(rb + i), a.inv_mean, -1.0f) : 0.0f;
+                v[t] = make_float2(fa, fb);
+            } else {
+                v[t] = in[pad16(i)];
+            }
+        }
+        const int k = j & (ns - 1);
+        if (!FIRST) {                                     // ns == 1 in the first pass: all twiddles are 1
+            // w^t, w = exp(-2 pi i k / (ns R)) = tw[k (n / (ns R))]; powers by products of depth <= 4
+            float2 w[R];
+            w[1] = tw[k * (m / ns)];
+#pragma unroll
+            for (int t = 2; t < R; ++t) w[t] = (t & 1) ? cmul(w[t - 1], w[1]) : cmul(w[t >> 1], w[t >> 1]);
+#pragma unroll
+            for (int t = 1; t < R; ++t) v[t] = cmul(v[t], w[t]);
+        }
+        dft_regs<R>(v);
+        const int j0 = (j - k) * R + k;
+#pragma unroll
+        for (int t = 0; t < R; ++t) out[pad16(j0 + t * ns)] = v[bitrev<R>(t)];
+    }
+}
+
 __global__ void __launch_bounds__(256) flux_power_kernel(const PowArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int n = a.n, nh = n >> 1;
+    const int n = a.n, nh = n >> 1, npad = n + (n >> 4) + 1;
     double *pw  = reinterpret_cast<double *>(smem_raw);                    // [nh + 1] (+1 pad)
-    float2 *z   = reinterpret_cast<float2 *>(pw + nh + 2);                 // [n]
-    float2 *tw  = z + n;                                                   // [nh]
+    float2 *bufA = reinterpret_cast<float2 *>(pw + nh + 2);                // [npad]
+    float2 *bufB = bufA + npad;                                            // [npad]
+    float2 *tw  = bufB + npad;                                             // [nh]: exp(-2 pi i q / n)
     const int tid = threadIdx.x, T = blockDim.x;
 
-    for (int k = tid; k < nh; k += T) {
+    for (int q = tid; q < nh; q += T) {
         float s, c;
-        sincospif(2.0f * (float)k / (float)n, &s, &c);
-        tw[k] = make_float2(c, -s);
+        sincospif(2.0f * (float)q / (float)n, &s, &c);
+        tw[q] = make_float2(c, -s);
     }
     for (int m = tid; m <= nh; m += T) pw[m] = 0.0;
 
@@ -41,27 +123,27 @@ __global__ void __launch_bounds__(256) flux_power_kernel(const PowArgs a)
         const bool has_b = 2 * pair + 1 < a.n_rows;
         const float *rb = ra + n;
         __syncthreads();                                   // previous pair's read-out done (and tables built)
-        for (int i = tid; i < n; i += T) {
-            const int r = (int)(__brev((unsigned int)i) >> (32 - a.log2n));
-            const float fa = fmaf(__ldcs(ra + i), a.inv_mean, -1.0f);
-            const float fb = has_b ? fmaf(__ldcs(rb + i), a.inv_mean, -1.0f) : 0.0f;
-            z[r] = make_float2(fa, fb);
-        }
-        __syncthreads();
-        for (int s = 0; s < a.log2n; ++s) {
-            const int half = 1 << s, tstep = nh >> s;
-            for (int bfly = tid; bfly < nh; bfly += T) {
-                const int pos = bfly & (half - 1);
-                const int i0 = ((bfly >> s) << (s + 1)) + pos, i1 = i0 + half;
-                const float2 w = tw[pos * tstep], u = z[i0], v = z[i1];
-                const float tr = w.x * v.x - w.y * v.y, ti = w.x * v.y + w.y * v.x;
-                z[i0] = make_float2(u.x + tr, u.y + ti);
-                z[i1] = make_float2(u.x - tr, u.y - ti);
+        float2 *src = bufB, *dst = bufA;
+        int ns = 1;
+#pragma unroll 1
+        for (int ps = 0; ps < a.n_pass; ++ps) {
+            const int R = a.radix[ps];
+            if (ps == 0) {
+                if (R == 16)     stockham_pass<16, true>(a, ra, rb, has_b, nullptr, dst, tw, 1);
+                else if (R == 8) stockham_pass<8, true>(a, ra, rb, has_b, nullptr, dst, tw, 1);
+                else             stockham_pass<4, true>(a, ra, rb, has_b, nullptr, dst, tw, 1);
+            } else {
+                if (R == 16)     stockham_pass<16, false>(a, ra, rb, has_b, src, dst, tw, ns);
+                else if (R == 8) stockham_pass<8, false>(a, ra, rb, has_b, src, dst, tw, ns);
+                else             stockham_pass<4, false>(a, ra, rb, has_b, src, dst, tw, ns);
             }
+            ns *= R;
+            float2 *tmp = src; src = dst; dst = tmp;       // src now holds the newest data
             __syncthreads();
         }
+        const float2 *z = src;
         for (int m = tid; m <= nh; m += T) {
-            const float2 p = z[m], q = z[(n - m) & (n - 1)];
+            const float2 p = z[pad16(m)], q = z[pad16((n - m) & (n - 1))];
             // X_A = (p + conj q)/2, X_B = (p - conj q)/(2i)
             const float ar = 0.5f * (p.x + q.x), ai = 0.5f * (p.y - q.y);
             const float br = 0.5f * (p.y + q.y), bi = 0.5f * (q.x - p.x);
@@ -90,9 +172,17 @@ extern "C" lya_status lya_flux_power_rows(lya_ctx *ctx, size_t n_rows, int32_t n
     LYA_CUDA(ctx, cudaSetDevice(ctx->device));
     const int nk = n_pix / 2 + 1;
     LYA_CUDA(ctx, cudaMemsetAsync(ctx->d_stats, 0, (size_t)nk * sizeof(double), ctx->stream));
-    PowArgs a{flux, n_rows, n_pix, log2n, (float)(1.0 / mean_flux), ctx->d_stats};
-    const size_t smem = (size_t)(nk + 1) * sizeof(double) + (size_t)n_pix * sizeof(float2) + (size_t)(n_pix / 2) * sizeof(float2);
-    int threads = n_pix / 2;
+    PowArgs a;
+    memset(&a, 0, sizeof(a));
+    a.flux = flux; a.n_rows = n_rows; a.n = n_pix; a.log2n = log2n;
+    a.inv_mean = (float)(1.0 / mean_flux); a.acc = ctx->d_stats;
+    // radices of the passes (log2: 4, 3, 2), largest first
+    static const int plan[14][4] = {{0}, {0}, {0}, {3}, {4}, {3, 2}, {3, 3}, {4, 3}, {4, 4}, {3, 3, 3}, {4, 3, 3},
+                                    {4, 4, 3}, {4, 4, 4}, {4, 4, 3, 2}};
+    for (int i = 0; i < 4 && plan[log2n][i]; ++i) a.radix[a.n_pass++] = 1 << plan[log2n][i];
+    const int npad = n_pix + (n_pix >> 4) + 1;
+    const size_t smem = (size_t)(nk + 1) * sizeof(double) + 2 * (size_t)npad * sizeof(float2) + (size_t)(n_pix / 2) * sizeof(float2);
+    int threads = n_pix / 8;
     threads = threads < 32 ? 32 : (threads > 256 ? 256 : threads);
     LYA_CUDA(ctx, cudaFuncSetAttribute(flux_power_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
