@@ -70,33 +70,48 @@ __device__ __forceinline__ void stockham_pass(const PowArgs &a, const float *ra,
                                               const float2 *in, float2 *out, const float2 *tw, int ns)
 {
     const int n = a.n, m = n / R;
+    // padded addresses are affine in t: pad16(j + t m) = pad16(j) + t (m + m/16) for m >= 16, and
+    // pad16(j0 + t ns) = pad16(j0) + t os_a + (t >> 1) os_b with (os_a, os_b) = (ns + ns/16, 0) for ns >= 16,
+    // (8, 1) for ns == 8 (j0 mod 16 < 8 there), (1, 0) for ns == 1 (j0 = j R)
+    const int is = m + (m >> 4);
+    const int os_a = ns >= 16 ? ns + (ns >> 4) : ns, os_b = ns == 8 ? 1 : 0;
+    const int tstep = m / ns;
     for (int j = threadIdx.x; j < m; j += blockDim.x) {
         float2 v[R];
+        if (FIRST) {
 #pragma unroll
-        for (int t = 0; t < R; ++t) {
-            const int i = j + t * m;
-            if (FIRST) {
-                const float fa = fmaf(__ldcs(ra + i), a.inv_mean, -1.0f);
-                const float fb = has_b ? fmaf(__ldcs(rb + i), a.inv_mean, -1.0f) : 0.0f;
+            for (int t = 0; t < R; ++t) {
+                const float fa = fmaf(__ldcs(ra + j + t * m), a.inv_mean, -1.0f);
+                const float fb = has_b ? fmaf(__ldcs(rb + j + t * m), a.inv_mean, -1.0f) : 0.0f;
                 v[t] = make_float2(fa, fb);
-            } else {
-                v[t] = in[pad16(i)];
             }
+        } else if (m >= 16) {
+            const float2 *ib = in + pad16(j);
+#pragma unroll
+            for (int t = 0; t < R; ++t) v[t] = ib[t * is];
+        } else {
+#pragma unroll
+            for (int t = 0; t < R; ++t) v[t] = in[pad16(j + t * m)];
         }
         const int k = j & (ns - 1);
         if (!FIRST) {                                     // ns == 1 in the first pass: all twiddles are 1
             // w^t, w = exp(-2 pi i k / (ns R)) = tw[k (n / (ns R))]; powers by products of depth <= 4
             float2 w[R];
-            w[1] = tw[k * (m / ns)];
+            w[1] = tw[k * tstep];
 #pragma unroll
             for (int t = 2; t < R; ++t) w[t] = (t & 1) ? cmul(w[t - 1], w[1]) : cmul(w[t >> 1], w[t >> 1]);
 #pragma unroll
             for (int t = 1; t < R; ++t) v[t] = cmul(v[t], w[t]);
         }
         dft_regs<R>(v);
-        const int j0 = (j - k) * R + k;
+        float2 *ob = out + pad16((j - k) * R + k);
+        if (ns == 2 || ns == 4) {                         // never produced by the plans (radices 16 / 8 first)
 #pragma unroll
-        for (int t = 0; t < R; ++t) out[pad16(j0 + t * ns)] = v[bitrev<R>(t)];
+            for (int t = 0; t < R; ++t) out[pad16((j - k) * R + k + t * ns)] = v[bitrev<R>(t)];
+        } else {
+#pragma unroll
+            for (int t = 0; t < R; ++t) ob[t * os_a + (t >> 1) * os_b] = v[bitrev<R>(t)];
+        }
     }
 }
 
@@ -127,7 +142,7 @@ __global__ void __launch_bounds__(256) flux_power_kernel(const PowArgs a)
         int ns = 1;
 #pragma unroll 1
         for (int ps = 0; ps < a.n_pass; ++ps) {
-            const int R = a.radix[ps];
+            const int R = ps == 0 ? a.radix[0] : (ps == 1 ? a.radix[1] : (ps == 2 ? a.radix[2] : a.radix[3]));
             if (ps == 0) {
                 if (R == 16)     stockham_pass<16, true>(a, ra, rb, has_b, nullptr, dst, tw, 1);
                 else if (R == 8) stockham_pass<8, true>(a, ra, rb, has_b, nullptr, dst, tw, 1);
