@@ -124,28 +124,30 @@ __device__ __forceinline__ float stage_from_global(const TauArgs &a, float jf, s
     return stage_cell(a, jf, nh, bb, __ldcs(a.v + g), out);
 }
 
-// Fast path: unwrapped walk over the `len` sources jj = start .. start + len - 1 (at most one wrap, len <= n),
-// no per-pair image logic.  Full sum: start = tile centre - n/2, len = n.  Windowed: start = i0 - W,
-// len = 32 R + 2 W with W the sightline's reach -- every source left out would have added exactly 0, and the
-// ones kept are added in the same order, so the result is bit-identical.  Lane owns pixels i0 + lane*R + r.
-template <int R>
-__device__ __forceinline__ void tile_fast(const float4 *__restrict__ cs, int n, int i0, int lane, int start, int len,
-                                          float (&acc)[R])
+// Staged cells are stored at cpos(j): plain for the full sum (every lane reads the same cell: broadcast), one
+// pad slot in 8 for LYA_TAU_WINDOWED, where lanes read DIFFERENT cells R apart (16 R bytes: without the pad the
+// eight lanes of an LDS.128 phase would hit two banks).
+template <bool PAD> __device__ __forceinline__ int cpos(int j) { return PAD ? j + (j >> 3) : j; }
+
+// Fast path, full sum: unwrapped walk over all n sources jj = start .. start + n - 1 around the tile centre (at
+// most one wrap), no per-pair image logic.  Lane owns pixels i0 + lane*R + r.
+template <int R, bool PAD>
+__device__ __forceinline__ void tile_fast(const float4 *__restrict__ cs, int n, int i0, int lane, float (&acc)[R])
 {
     constexpr int RH = R / 2;                          // reference pixel of the lane
+    const int start = i0 + 16 * R - (n >> 1);          // first unwrapped source index
     int j0 = start % n;
     if (j0 < 0) j0 += n;                               // slot holding jj = start
     const int off = start - j0;                        // jj = j + off on [j0, n), jj = j + off + n on [0, j0)
     float cref = (float)(i0 + lane * R + RH - off);
 #pragma unroll
     for (int r = 0; r < R; ++r) acc[r] = 0.0f;
-    const int end1 = j0 + len < n ? j0 + len : n;      // first segment [j0, end1), second [0, j0 + len - n)
 #pragma unroll 1
     for (int seg = 0; seg < 2; ++seg) {
-        const int lo = seg ? 0 : j0, hi = seg ? j0 + len - n : end1;
+        const int lo = seg ? 0 : j0, hi = seg ? j0 : n;
 #pragma unroll 8
         for (int j = lo; j < hi; ++j) {
-            const float4 q = cs[j];
+            const float4 q = cs[cpos<PAD>(j)];
             const float E  = cref - q.x;
             const float xr = fmaf(E, q.y, q.z);
 #pragma unroll
@@ -159,23 +161,42 @@ __device__ __forceinline__ void tile_fast(const float4 *__restrict__ cs, int n, 
     }
 }
 
-// which sources a tile walks: returns false if the sightline needs the general loop
+// LYA_TAU_WINDOWED: every LANE walks only its own window jj = il - W .. il + R - 1 + W around its R pixels
+// (il = i0 + lane R), W = the sightline's reach: 2 W + R sources instead of n.  A source outside the window is
+// further than its reach from all R pixels, so it would have added ex2(..) == 0 exactly; the sources kept are
+// added in the same ascending order with the same arithmetic (same reference pixel), so the result is
+// bit-identical to tile_fast.  Lanes read different cells (conflict-free through cpos<true>); the wrap is one
+// compare per source cell.
 template <int R>
-__device__ __forceinline__ bool tile_span(const TauArgs &a, float reach, int i0, int &start, int &len)
+__device__ __forceinline__ void tile_window(const float4 *__restrict__ cs, int n, float n_f, int i0, int lane, int W,
+                                            float (&acc)[R])
 {
-    const int n = a.n;
-    if (!(reach <= (float)((n >> 1) - 16 * R))) return false;          // also catches +inf
-    start = i0 + 16 * R - (n >> 1);
-    len = n;
-    if (a.windowed) {
-        const int W = (int)reach + 1;
-        if (32 * R + 2 * W < n) { start = i0 - W; len = 32 * R + 2 * W; }
+    constexpr int RH = R / 2;
+    const int il = i0 + lane * R;
+    const int jj = il - W;
+    int j = jj % n;
+    if (j < 0) j += n;
+    float cref = (float)(il + RH - (jj - j));
+#pragma unroll
+    for (int r = 0; r < R; ++r) acc[r] = 0.0f;
+    const int cnt = 2 * W + R;
+#pragma unroll 4
+    for (int t = 0; t < cnt; ++t) {
+        const float4 q = cs[cpos<true>(j)];
+        const float E  = cref - q.x;
+        const float xr = fmaf(E, q.y, q.z);
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const float x = (r == RH) ? xr : fmaf((float)(r - RH), q.y, xr);
+            const float e = ex2_ftz(-(x * x));
+            acc[r] = fmaf(q.w, e, acc[r]);
+        }
+        if (++j == n) { j = 0; cref -= n_f; }
     }
-    return true;
 }
 
 // General path: nearest image chosen per pair (tiny N, or |v_pec| comparable to the box).
-template <int R>
+template <int R, bool PAD>
 __device__ __forceinline__ void tile_general(const float4 *__restrict__ cs, int n, float n_f, float inv_n, int i0,
                                              int lane, float (&acc)[R])
 {
@@ -187,7 +208,7 @@ __device__ __forceinline__ void tile_general(const float4 *__restrict__ cs, int 
     }
 #pragma unroll 2
     for (int j = 0; j < n; ++j) {
-        const float4 q = cs[j];
+        const float4 q = cs[cpos<PAD>(j)];
         const float  f = -q.z / q.y;                    // fractional displacement (only picks the image)
 #pragma unroll
         for (int r = 0; r < R; ++r) {
@@ -199,6 +220,25 @@ __device__ __forceinline__ void tile_general(const float4 *__restrict__ cs, int 
             acc[r]   = fmaf(q.w, e, acc[r]);
         }
     }
+}
+
+// one tile of one sightline: picks the loop from the sightline's reach; returns the sources walked per pixel
+template <int R, bool WIN>
+__device__ __forceinline__ int tile_any(const TauArgs &a, const float4 *cs, float reach, int i0, int lane,
+                                        float (&acc)[R])
+{
+    const int n = a.n;
+    if (!(reach <= (float)((n >> 1) - 16 * R))) {       // also catches +inf
+        tile_general<R, WIN>(cs, n, a.n_f, a.inv_n, i0, lane, acc);
+        return n;
+    }
+    if (WIN) {
+        const int W = (int)reach + 1;
+        tile_window<R>(cs, n, a.n_f, i0, lane, W, acc);
+        return 2 * W + R;
+    }
+    tile_fast<R, WIN>(cs, n, i0, lane, acc);
+    return n;
 }
 
 __device__ __forceinline__ void group_sync(int G, int bar_id)
@@ -213,15 +253,16 @@ __device__ __forceinline__ void group_sync(int G, int bar_id)
 // (A variant that bulk-copied the next row into a raw buffer with cp.async.bulk + mbarrier while the current
 // one was summed measured 4 % slower: profiles/r1_tau_prefetch_ab.md.  The row change here is plain coalesced
 // loads; the other resident groups keep the MUFU pipe busy meanwhile.)
-template <int R, bool FUSED>
+template <int R, bool FUSED, bool WIN>
 __global__ void __launch_bounds__(1024, 1) tau_x_kernel(const TauArgs a, const int G, const int gpc)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int grp = warp / G, wg = warp - grp * G;       // group in CTA, warp in group
     const int n = a.n;
-    float4 *cells = reinterpret_cast<float4 *>(smem) + (size_t)grp * n;
-    volatile int *ctl = reinterpret_cast<volatile int *>(smem + (size_t)gpc * n * sizeof(float4)) + 4 * grp;
+    const int crow = WIN ? n + (n >> 3) + 1 : n;         // float4 slots per staged row
+    float4 *cells = reinterpret_cast<float4 *>(smem) + (size_t)grp * crow;
+    volatile int *ctl = reinterpret_cast<volatile int *>(smem + (size_t)gpc * crow * sizeof(float4)) + 4 * grp;
     const int bar_id = grp;      // named barrier of the group (G >= 2: at most 16 groups; no __syncthreads here)
     const int gl = wg * 32 + lane, gthreads = G * 32;    // thread index / count inside the group
 
@@ -240,7 +281,7 @@ __global__ void __launch_bounds__(1024, 1) tau_x_kernel(const TauArgs a, const i
         for (int j = gl; j < n; j += gthreads) {
             float4 q;
             reach = fmaxf(reach, stage_from_global<FUSED>(a, jf, g0 + j, q));
-            cells[j] = q;
+            cells[cpos<WIN>(j)] = q;
             jf += (float)gthreads;
         }
 #pragma unroll
@@ -255,14 +296,11 @@ __global__ void __launch_bounds__(1024, 1) tau_x_kernel(const TauArgs a, const i
         }
 
         // ---- sum: the group's warps take the pixel tiles of the row
-        int start = 0, len = n;
-        const bool fast = tile_span<R>(a, reach, 0, start, len);
-        if (gl == 0 && a.pairs) atomicAdd(a.pairs, (unsigned long long)n * (unsigned long long)len);
+        int walked = 0;
         for (int tile = wg; tile < a.tiles; tile += G) {
             const int i0 = tile * 32 * R;
             float acc[R];
-            if (fast) tile_fast<R>(cells, n, i0, lane, start + i0, len, acc);
-            else      tile_general<R>(cells, n, a.n_f, a.inv_n, i0, lane, acc);
+            walked = tile_any<R, WIN>(a, cells, reach, i0, lane, acc);
             const int i = i0 + lane * R;
             float *dst = a.tau + g0 + i;
             if (R == 4 && a.vec) {
@@ -276,6 +314,7 @@ __global__ void __launch_bounds__(1024, 1) tau_x_kernel(const TauArgs a, const i
             }
         }
         group_sync(G, bar_id);                           // cells consumed by every warp of the group
+        if (gl == 0 && a.pairs) atomicAdd(a.pairs, (unsigned long long)n * (unsigned long long)walked);
         if (gl == 0) ctl[0] = ctl[2];
         group_sync(G, bar_id);
     }
@@ -299,7 +338,7 @@ __global__ void __launch_bounds__(1024, 1) tau_x_kernel(const TauArgs a, const i
 // way.  Batches are handed out by the atomic counter; bsl is chosen so that >= 4 CTAs are resident per SM and
 // one CTA's gather overlaps the others' pair loops.  cstride / tstride are padded so that neither the
 // transposed staging stores nor the tile read-out have shared-memory bank conflicts.
-template <int R, bool FUSED>
+template <int R, bool FUSED, bool WIN>
 __global__ void __launch_bounds__(TAU_THREADS) tau_strided_kernel(const TauArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem[];
@@ -330,7 +369,7 @@ __global__ void __launch_bounds__(TAU_THREADS) tau_strided_kernel(const TauArgs 
             if (bx < nb) {
                 float4 q;
                 reach = fmaxf(reach, stage_from_global<FUSED>(a, (float)j, (size_t)(base + (long long)j * a.stride + bx), q));
-                cells[bx * cstride + j] = q;
+                cells[bx * cstride + cpos<WIN>(j)] = q;
             }
         }
 #pragma unroll
@@ -341,17 +380,14 @@ __global__ void __launch_bounds__(TAU_THREADS) tau_strided_kernel(const TauArgs 
         reach = __int_as_float(s_reach);
         if (tid == 0) s_batch = atomicAdd(&a.sched[0], 1u);
 
-        int start = 0, len = n;
-        const bool fast = tile_span<R>(a, reach, 0, start, len);
-        if (tid == 0 && a.pairs) atomicAdd(a.pairs, (unsigned long long)nb * n * (unsigned long long)len);
+        int walked = 0;
         const int items = nb * a.tiles;
         for (int item = warp; item < items; item += TAU_WARPS) {
             const int sl = item / a.tiles, tile = item - sl * a.tiles;
             const int i0 = tile * 32 * R;
             const float4 *cs = cells + (size_t)sl * cstride;
             float acc[R];
-            if (fast) tile_fast<R>(cs, n, i0, lane, start + i0, len, acc);
-            else      tile_general<R>(cs, n, a.n_f, a.inv_n, i0, lane, acc);
+            walked = tile_any<R, WIN>(a, cs, reach, i0, lane, acc);
             const int i = i0 + lane * R;
             float *dst = ttile + (size_t)sl * tstride + i;     // tstride covers tiles * 32 * R: no bound check
             if (R == 4)      *reinterpret_cast<float4 *>(dst) = make_float4(acc[0], acc[1], acc[2], acc[3]);
@@ -359,6 +395,7 @@ __global__ void __launch_bounds__(TAU_THREADS) tau_strided_kernel(const TauArgs 
             else             dst[0] = acc[0];
         }
         __syncthreads();                                 // cells consumed, tau tile complete, s_batch written
+        if (tid == 0 && a.pairs) atomicAdd(a.pairs, (unsigned long long)nb * n * (unsigned long long)walked);
         for (int c = tid; c < (n << a.bshift); c += TAU_THREADS) {
             const int bx = c & (a.bsl - 1), j = c >> a.bshift;
             if (bx < nb) __stcs(a.tau + base + (long long)j * a.stride + bx, ttile[bx * tstride + j]);
@@ -376,12 +413,12 @@ __global__ void __launch_bounds__(TAU_THREADS) tau_strided_kernel(const TauArgs 
     }
 }
 
-template <int R, bool FUSED>
+template <int R, bool FUSED, bool WIN>
 lya_status launch_x(lya_ctx *ctx, const TauArgs &a)
 {
-    auto kern = tau_x_kernel<R, FUSED>;
+    auto kern = tau_x_kernel<R, FUSED, WIN>;
     const size_t cap = (size_t)ctx->max_smem_optin;
-    const size_t per_group = (size_t)a.n * sizeof(float4) + 16;
+    const size_t per_group = (size_t)(WIN ? a.n + (a.n >> 3) + 1 : a.n) * sizeof(float4) + 16;
     int groups = (int)(cap / per_group);                 // groups that fit in one SM's shared memory
     if (groups < 1) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: sightline too long for shared memory");
     // G warps per group: as few as keep >= 24 warps resident, never more than the row has tiles
@@ -402,10 +439,10 @@ lya_status launch_x(lya_ctx *ctx, const TauArgs &a)
     return LYA_OK;
 }
 
-template <int R, bool FUSED>
+template <int R, bool FUSED, bool WIN>
 lya_status launch_strided(lya_ctx *ctx, const TauArgs &a, size_t smem_bytes)
 {
-    auto kern = tau_strided_kernel<R, FUSED>;
+    auto kern = tau_strided_kernel<R, FUSED, WIN>;
     LYA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
     int per_sm = 0;
     LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, TAU_THREADS, smem_bytes));
@@ -426,6 +463,7 @@ lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
                           unsigned long long *d_pairs)
 {
     const bool fused = (flags & LYA_TAU_FROM_DENSITY) != 0;
+    const bool win = (flags & LYA_TAU_WINDOWED) != 0;
     TauArgs a;
     memset(&a, 0, sizeof(a));
     a.n_hi = n_hi; a.b = b; a.v = v; a.tau = tau;
@@ -450,11 +488,15 @@ lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
         if (a.n_sl >= (1LL << 31)) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: more than 2^31 sightlines");
         a.vec = (n % 4 == 0) && (((uintptr_t)tau & 15) == 0);
         a.sched = ctx->d_sched;
+#define LYA_TAU_X(RR)                                                                                       \
+    return win ? (fused ? launch_x<RR, true, true>(ctx, a) : launch_x<RR, false, true>(ctx, a))             \
+               : (fused ? launch_x<RR, true, false>(ctx, a) : launch_x<RR, false, false>(ctx, a))
         switch (R) {
-            case 1:  return fused ? launch_x<1, true>(ctx, a) : launch_x<1, false>(ctx, a);
-            case 2:  return fused ? launch_x<2, true>(ctx, a) : launch_x<2, false>(ctx, a);
-            default: return fused ? launch_x<4, true>(ctx, a) : launch_x<4, false>(ctx, a);
+            case 1:  LYA_TAU_X(1);
+            case 2:  LYA_TAU_X(2);
+            default: LYA_TAU_X(4);
         }
+#undef LYA_TAU_X
     }
 
     // strided: axis 1 (pixels along y, outer index iz) or axis 2 (pixels along z, outer index iy)
@@ -468,7 +510,7 @@ lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
     auto pad_to = [](int v, int mod, int want) { return v + ((want - v % mod) % mod + mod) % mod; };
     auto strides = [&](int sh, int &cs, int &ts) {
         const int bs = 1 << sh;
-        cs = pad_to(n, 8, (8 / bs) % 8);
+        cs = pad_to(win ? n + (n >> 3) + 1 : n, 8, (8 / bs) % 8);
         ts = pad_to(a.tiles * 32 * R, 32, (32 / bs) % 32);
     };
     auto need2 = [&](int sh) {
@@ -488,9 +530,15 @@ lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
     a.n_batches = n_outer * a.nxb;
     if (a.n_batches >= (1LL << 31)) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: more than 2^31 batches");
     a.sched = ctx->d_sched;
+#define LYA_TAU_S(RR)                                                                                       \
+    return win ? (fused ? launch_strided<RR, true, true>(ctx, a, need2(bshift))                             \
+                        : launch_strided<RR, false, true>(ctx, a, need2(bshift)))                           \
+               : (fused ? launch_strided<RR, true, false>(ctx, a, need2(bshift))                            \
+                        : launch_strided<RR, false, false>(ctx, a, need2(bshift)))
     switch (R) {
-        case 1:  return fused ? launch_strided<1, true>(ctx, a, need2(bshift)) : launch_strided<1, false>(ctx, a, need2(bshift));
-        case 2:  return fused ? launch_strided<2, true>(ctx, a, need2(bshift)) : launch_strided<2, false>(ctx, a, need2(bshift));
-        default: return fused ? launch_strided<4, true>(ctx, a, need2(bshift)) : launch_strided<4, false>(ctx, a, need2(bshift));
+        case 1:  LYA_TAU_S(1);
+        case 2:  LYA_TAU_S(2);
+        default: LYA_TAU_S(4);
     }
+#undef LYA_TAU_S
 }
