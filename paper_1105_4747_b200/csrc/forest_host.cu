@@ -1,7 +1,7 @@
 // forest_host.cu -- lya_forest_host: S1..S5 end to end from HOST buffers, z-slab streamed
 // (the build's analogue of the paper's "only read into memory a small section of the volume at any one
 // time", App. B).  Slab s+1 is copied host->device on ctx->copy_stream while slab s runs
-// S1 + S3 on ctx->stream; tau stays resident for S4; S5 streams F back chunk by chunk.
+// S1 + S3 (one kernel: LYA_TAU_FROM_DENSITY) on ctx->stream; tau stays resident for S4; S5 streams F back chunk by chunk.
 #include "lya_internal.h"
 
 namespace {
@@ -46,12 +46,11 @@ extern "C" lya_status lya_forest_host(lya_ctx *ctx, const lya_params *p, int axi
     const size_t slab_cells = plane * snz;
     const int n_slabs = (p->nz + snz - 1) / snz;
 
-    lya_status st = ensure_ws(ctx, (total + 6 * slab_cells) * sizeof(float) + 256);
+    lya_status st = ensure_ws(ctx, (total + 4 * slab_cells) * sizeof(float) + 256);
     if (st != LYA_OK) return st;
     float *tau = (float *)ctx->ws;
     float *d_delta[2] = {tau + total, tau + total + slab_cells};
     float *d_v[2]     = {tau + total + 2 * slab_cells, tau + total + 3 * slab_cells};
-    float *d_nhi = tau + total + 4 * slab_cells, *d_b = tau + total + 5 * slab_cells;
 
     auto copy_in = [&](int s) -> cudaError_t {
         const int buf = s & 1;
@@ -73,9 +72,9 @@ extern "C" lya_status lya_forest_host(lya_ctx *ctx, const lya_params *p, int axi
         const size_t cells = (s == n_slabs - 1) ? total - off : slab_cells;
         const int nzl = (int)(cells / plane);
         LYA_CUDA(ctx, cudaStreamWaitEvent(ctx->stream, ctx->ev_copy[buf], 0));
-        st = lya_gas_from_density(ctx, p, d_delta[buf], cells, d_nhi, d_b);
-        if (st != LYA_OK) return st;
-        st = lya_tau_sightlines(ctx, p, axis, nzl, d_nhi, d_b, d_v[buf], tau + off);
+        // S1 fused into the staging of S3 (bit-identical to the two-call path; n_HI and b never touch memory)
+        st = lya_tau_sightlines_opt(ctx, p, axis, nzl, LYA_TAU_FROM_DENSITY, d_delta[buf], nullptr, d_v[buf],
+                                    tau + off, nullptr);
         if (st != LYA_OK) return st;
         LYA_CUDA(ctx, cudaEventRecord(ctx->ev_comp[buf], ctx->stream));
     }
