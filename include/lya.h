@@ -201,6 +201,32 @@ lya_status lya_flux_pdf(lya_ctx *ctx, const float *flux, size_t n, int32_t n_bin
 lya_status lya_flux_power_rows(lya_ctx *ctx, size_t n_rows, int32_t n_pix, double dv_kms, const float *flux,
                                double mean_flux, double *power);
 
+/* ---------------------------------------------------------------------------------------------------------
+ * Before the hot path: the baryon density and the peculiar velocity from a
+ * dark-matter density field, sections 2.1-2.2 of the paper.
+ *   Eq.1  delta_b(k) = delta_DM(k) / (1 + k^2 / k_F^2)
+ *   Eq.3  v(k) = E_+ i k / k^2 delta_DM(k),  E_+ = H(z) f(z) / (1+z)  (delta_DM already at z: U1)
+ * k is the comoving wavevector in Mpc^-1, k_i = 2 pi m_i h / L_i (readings U1-U5 in DESIGN.md section 12).  The
+ * 3D transforms are cuFFT's (a library primitive, loaded with dlopen on first use: LYA_ECUDA if it is not
+ * installed); the k-space operators are the library's own kernels.
+ * --------------------------------------------------------------------------------------------------------- */
+typedef struct {
+    int32_t nx, ny, nz;
+    double  box_mpch;        /* comoving box length along x [h^-1 Mpc]; cells are cubic (L_y = L ny/nx, ...)  */
+    double  h, z, omega_m;   /* flat LCDM                                                                     */
+    double  k_filter_mpc;    /* k_F [comoving Mpc^-1], paper: 6.5; <= 0: delta_b = delta_DM                   */
+} lya_field_params;
+
+/* f = dln D_+ / dln a of flat LCDM (Heath 1977 integral by Simpson quadrature).  Host only. */
+lya_status lya_growth_rate(double z, double omega_m, double *f_out);
+
+/* delta_dm: DEVICE [nz][ny][nx] fp32.  delta_b, v_x, v_y, v_z: DEVICE outputs of the same shape, any may be NULL
+ * (v in km/s, proper, along +axis: what lya_tau_sightlines takes); no output may alias delta_dm or another output.  Asynchronous on ctx's stream apart from the first call's
+ * plan creation.  Workspace (two complex half-spectra, 8 (nx/2+1) ny nz bytes each, plus cuFFT's) is cached in
+ * ctx. */
+lya_status lya_fields_from_dm(lya_ctx *ctx, const lya_field_params *p, const float *delta_dm,
+                              float *delta_b, float *v_x, float *v_y, float *v_z);
+
 /* Roofline denominator of the tau kernel (BASELINE.json: "MUFU.EX2 ... issue rate from SM count x clock"):
  * runs a pure ex2.approx micro-kernel on every SM of ctx's device and returns MUFU.EX2 results per second
  * (HOST double; best of 3 after a warm-up).  Synchronises the stream.  16 / clk / SM on B200. */

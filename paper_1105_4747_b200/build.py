@@ -15,10 +15,10 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "liblya.so")
 STAMP = LIB + ".sha256"
-SOURCES = ["lya_api.cu", "gas.cu", "tau.cu", "normalize.cu", "forest_host.cu", "probe.cu", "observe.cu", "power.cu"]
+SOURCES = ["lya_api.cu", "gas.cu", "tau.cu", "normalize.cu", "forest_host.cu", "probe.cu", "observe.cu", "power.cu", "fields.cu"]
 HEADERS = ["lya_internal.h", "root_iter.h", "gas_cell.h", os.path.join("..", "..", "include", "lya.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-shared"]
+              "-Xcompiler", "-fPIC", "-shared", "-ldl"]
 
 
 def nvcc() -> str:

@@ -1,0 +1,187 @@
+// fields.cu -- before the hot path: baryon density and peculiar velocity from a
+// dark-matter density field.
+//   Eq.1  delta_b(k) = delta_DM(k) / (1 + k^2 / k_F^2)
+//   Eq.3  v_a(k)     = E_+ i k_a / k^2 delta_DM(k),  E_+ = H(z) f(z) / (1+z)   [km/s per comoving Mpc]
+// One real-to-complex 3D FFT of delta_DM, then per requested output one k-space kernel (8 B read + 8 B written
+// per half-spectrum mode, HBM-bound; the 1/N^3 of the unnormalised transforms is folded in) and one
+// complex-to-real FFT.  The FFTs are cuFFT's (library primitive), resolved with dlopen at first use so that
+// liblya.so itself does not depend on libcufft; everything else is this file.  Readings U1-U5: DESIGN.md 12.
+#include <cufft.h>
+#include <dlfcn.h>
+#include <math.h>
+
+#include "lya_internal.h"
+
+namespace {
+
+struct CufftApi {
+    void *handle;
+    cufftResult (*Plan3d)(cufftHandle *, int, int, int, cufftType);
+    cufftResult (*SetStream)(cufftHandle, cudaStream_t);
+    cufftResult (*ExecR2C)(cufftHandle, cufftReal *, cufftComplex *);
+    cufftResult (*ExecC2R)(cufftHandle, cufftComplex *, cufftReal *);
+    cufftResult (*Destroy)(cufftHandle);
+};
+
+CufftApi *cufft_api()
+{
+    static CufftApi api = {};
+    static int state = 0;                                  // 0 untried, 1 ok, -1 missing
+    if (state == 0) {
+        const char *names[] = {"libcufft.so.11", "libcufft.so", "/usr/local/cuda/lib64/libcufft.so.11",
+                               "/usr/local/cuda/lib64/libcufft.so"};
+        for (const char *nm : names)
+            if ((api.handle = dlopen(nm, RTLD_NOW | RTLD_LOCAL))) break;
+        if (api.handle) {
+            api.Plan3d    = (decltype(api.Plan3d))dlsym(api.handle, "cufftPlan3d");
+            api.SetStream = (decltype(api.SetStream))dlsym(api.handle, "cufftSetStream");
+            api.ExecR2C   = (decltype(api.ExecR2C))dlsym(api.handle, "cufftExecR2C");
+            api.ExecC2R   = (decltype(api.ExecC2R))dlsym(api.handle, "cufftExecC2R");
+            api.Destroy   = (decltype(api.Destroy))dlsym(api.handle, "cufftDestroy");
+        }
+        state = (api.handle && api.Plan3d && api.SetStream && api.ExecR2C && api.ExecC2R && api.Destroy) ? 1 : -1;
+    }
+    return state == 1 ? &api : nullptr;
+}
+
+struct KArgs {
+    const float2 *in;
+    float2       *out;
+    int           nxh, nx, ny, nz;
+    float         dkx, dky, dkz;       // 2 pi h / L_i [Mpc^-1]
+    float         inv_kf2;             // 1 / k_F^2 (0: no filtering)
+    float         scale;               // mode 0: 1/N^3; mode a: E_+ / N^3
+    int           mode;                // 0: Eq.1 filter; 1, 2, 3: Eq.3 velocity along x, y, z
+};
+
+// grid (ny, nz), one block per (iz, iy) row of nx/2 + 1 modes
+__global__ void __launch_bounds__(128) kspace_kernel(const KArgs a)
+{
+    const int iy = blockIdx.x, iz = blockIdx.y;
+    const int my = iy < (a.ny + 1) / 2 ? iy : iy - a.ny;           // signed frequency, -n/2 at the Nyquist slot
+    const int mz = iz < (a.nz + 1) / 2 ? iz : iz - a.nz;
+    const float ky = a.dky * (float)my, kz = a.dkz * (float)mz;
+    const float kyz2 = ky * ky + kz * kz;
+    const bool nyq_y = (a.ny % 2 == 0) && iy == a.ny / 2, nyq_z = (a.nz % 2 == 0) && iz == a.nz / 2;
+    const size_t row = ((size_t)iz * a.ny + iy) * a.nxh;
+    for (int ix = threadIdx.x; ix < a.nxh; ix += blockDim.x) {
+        const float kx = a.dkx * (float)ix;
+        const float k2 = fmaf(kx, kx, kyz2);
+        const float2 d = __ldcs(a.in + row + ix);
+        float2 o;
+        if (a.mode == 0) {
+            const float f = a.scale / fmaf(k2, a.inv_kf2, 1.0f);
+            o = make_float2(d.x * f, d.y * f);
+        } else {
+            const float ka = a.mode == 1 ? kx : (a.mode == 2 ? ky : kz);
+            const bool nyq = a.mode == 1 ? ((a.nx % 2 == 0) && ix == a.nx / 2) : (a.mode == 2 ? nyq_y : nyq_z);
+            const float c = (k2 > 0.0f && !nyq) ? a.scale * ka / k2 : 0.0f;      // U4
+            o = make_float2(-d.y * c, d.x * c);                                  // times i c
+        }
+        __stcs(a.out + row + ix, o);
+    }
+}
+
+lya_status ensure_ws(lya_ctx *ctx, size_t bytes)
+{
+    if (ctx->ws_bytes >= bytes) return LYA_OK;
+    if (ctx->ws) { cudaFree(ctx->ws); ctx->ws = nullptr; ctx->ws_bytes = 0; }
+    if (cudaMalloc(&ctx->ws, bytes) != cudaSuccess) {
+        cudaGetLastError();
+        return lya_fail(ctx, LYA_ENOMEM, "lya_fields_from_dm: device workspace allocation failed");
+    }
+    ctx->ws_bytes = bytes;
+    return LYA_OK;
+}
+
+}  // namespace
+
+extern "C" lya_status lya_growth_rate(double z, double omega_m, double *f_out)
+{
+    if (!f_out || !(z > -1.0) || !(omega_m > 0.0) || !(omega_m <= 1.0)) return LYA_EINVAL;
+    // D(a) ~ E(a) I(a), I = int_0^a dx / (x E(x))^3; with x = t^2 the integrand 2 t^4 / (Om + OL t^6)^1.5 is smooth
+    const double a = 1.0 / (1.0 + z), ol = 1.0 - omega_m, T = sqrt(a);
+    const int n = 4096;
+    auto g = [&](double t) { const double t2 = t * t, t6 = t2 * t2 * t2; return 2.0 * t2 * t2 / pow(omega_m + ol * t6, 1.5); };
+    double s = g(0.0) + g(T);
+    for (int i = 1; i < n; ++i) s += (i & 1 ? 4.0 : 2.0) * g(T * i / n);
+    const double I = s * T / (3.0 * n);
+    const double E2 = omega_m / (a * a * a) + ol, E = sqrt(E2);
+    *f_out = -1.5 * omega_m / (a * a * a) / E2 + a / pow(a * E, 3.0) / I;
+    return LYA_OK;
+}
+
+extern "C" lya_status lya_fields_from_dm(lya_ctx *ctx, const lya_field_params *p, const float *delta_dm,
+                                         float *delta_b, float *v_x, float *v_y, float *v_z)
+{
+    if (!ctx) return LYA_EINVAL;
+    ctx->err[0] = 0;
+    if (!p || !delta_dm) return lya_fail(ctx, LYA_EINVAL, "lya_fields_from_dm: null pointer");
+    if (p->nx < 2 || p->ny < 1 || p->nz < 1 || !(p->box_mpch > 0.0) || !(p->h > 0.0) || !(p->z > -1.0) ||
+        !(p->omega_m > 0.0) || !(p->omega_m <= 1.0))
+        return lya_fail(ctx, LYA_EINVAL, "lya_fields_from_dm: bad parameters");
+    float *outs[4] = {delta_b, v_x, v_y, v_z};
+    for (int i = 0; i < 4; ++i) {
+        if (outs[i] && (outs[i] == delta_dm || ((uintptr_t)outs[i] & 3))) return lya_fail(ctx, LYA_EINVAL, "lya_fields_from_dm: output aliases the input or is misaligned");
+        for (int j = 0; j < i; ++j)
+            if (outs[i] && outs[i] == outs[j]) return lya_fail(ctx, LYA_EINVAL, "lya_fields_from_dm: outputs alias each other");
+    }
+    CufftApi *fft = cufft_api();
+    if (!fft) return lya_fail(ctx, LYA_ECUDA, "lya_fields_from_dm: libcufft not found (dlopen)");
+    LYA_CUDA(ctx, cudaSetDevice(ctx->device));
+
+    const int nxh = p->nx / 2 + 1;
+    const size_t half = (size_t)p->nz * p->ny * nxh;
+    lya_status st = ensure_ws(ctx, 2 * half * sizeof(float2) + 256);
+    if (st != LYA_OK) return st;
+    float2 *A = (float2 *)ctx->ws, *B = A + half;
+
+    if (ctx->fft_dims[0] != p->nz || ctx->fft_dims[1] != p->ny || ctx->fft_dims[2] != p->nx) {
+        if (ctx->fft_dims[0]) { fft->Destroy(ctx->fft_r2c); fft->Destroy(ctx->fft_c2r); ctx->fft_dims[0] = 0; }
+        if (fft->Plan3d(&ctx->fft_r2c, p->nz, p->ny, p->nx, CUFFT_R2C) != CUFFT_SUCCESS)
+            return lya_fail(ctx, LYA_ECUDA, "lya_fields_from_dm: cufftPlan3d(R2C) failed");
+        if (fft->Plan3d(&ctx->fft_c2r, p->nz, p->ny, p->nx, CUFFT_C2R) != CUFFT_SUCCESS) {
+            fft->Destroy(ctx->fft_r2c);
+            return lya_fail(ctx, LYA_ECUDA, "lya_fields_from_dm: cufftPlan3d(C2R) failed");
+        }
+        ctx->fft_dims[0] = p->nz; ctx->fft_dims[1] = p->ny; ctx->fft_dims[2] = p->nx;
+    }
+    fft->SetStream(ctx->fft_r2c, ctx->stream);
+    fft->SetStream(ctx->fft_c2r, ctx->stream);
+    if (fft->ExecR2C(ctx->fft_r2c, const_cast<float *>(delta_dm), A) != CUFFT_SUCCESS)
+        return lya_fail(ctx, LYA_ECUDA, "lya_fields_from_dm: cufftExecR2C failed");
+
+    double f = 0.0;
+    lya_growth_rate(p->z, p->omega_m, &f);
+    const double zp1 = 1.0 + p->z;
+    const double Hz = 100.0 * p->h * sqrt(p->omega_m * zp1 * zp1 * zp1 + 1.0 - p->omega_m);
+    const double eplus = Hz * f / zp1;                                        // km/s per comoving Mpc (U1)
+    const double n3 = (double)p->nx * p->ny * p->nz;
+    const double dk = 2.0 * M_PI * p->h / p->box_mpch * (double)p->nx;        // 2 pi h / (cell size x n_i), per axis below
+    KArgs a;
+    memset(&a, 0, sizeof(a));
+    a.in = A; a.out = B; a.nxh = nxh; a.nx = p->nx; a.ny = p->ny; a.nz = p->nz;
+    a.dkx = (float)(dk / p->nx); a.dky = (float)(dk / p->ny); a.dkz = (float)(dk / p->nz);
+    a.inv_kf2 = p->k_filter_mpc > 0.0 ? (float)(1.0 / (p->k_filter_mpc * p->k_filter_mpc)) : 0.0f;
+    const dim3 grid(p->ny, p->nz);
+    if (p->ny > 65535 * 32767 || p->nz > 65535) return lya_fail(ctx, LYA_EINVAL, "lya_fields_from_dm: grid too large");
+    for (int mode = 0; mode < 4; ++mode) {
+        if (!outs[mode]) continue;
+        a.mode = mode;
+        a.scale = (float)((mode == 0 ? 1.0 : eplus) / n3);
+        kspace_kernel<<<grid, 128, 0, ctx->stream>>>(a);
+        ctx->launches++;
+        LYA_CUDA(ctx, cudaGetLastError());
+        if (fft->ExecC2R(ctx->fft_c2r, B, outs[mode]) != CUFFT_SUCCESS)
+            return lya_fail(ctx, LYA_ECUDA, "lya_fields_from_dm: cufftExecC2R failed");
+    }
+    return LYA_OK;
+}
+
+// called by lya_destroy
+void lya_fields_release(lya_ctx *ctx)
+{
+    CufftApi *fft = ctx->fft_dims[0] ? cufft_api() : nullptr;
+    if (fft) { fft->Destroy(ctx->fft_r2c); fft->Destroy(ctx->fft_c2r); }
+    ctx->fft_dims[0] = 0;
+}

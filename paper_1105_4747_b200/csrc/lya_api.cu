@@ -101,6 +101,7 @@ void lya_destroy(lya_ctx *ctx)
 {
     if (!ctx) return;
     cudaSetDevice(ctx->device);
+    lya_fields_release(ctx);
     if (ctx->ws) cudaFree(ctx->ws);
     if (ctx->d_partials) cudaFree(ctx->d_partials);
     if (ctx->d_root) cudaFree(ctx->d_root);

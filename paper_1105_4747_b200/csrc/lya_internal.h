@@ -25,7 +25,9 @@ struct lya_ctx {
     double       *d_stats;        // 8192 doubles: flux-PDF counts (as uint64) / power-spectrum accumulators
     float        *d_taps, *h_taps; // lya_observe_rows: Gaussian taps (device / host staging), grown on demand
     size_t        taps_cap;
-    // lya_forest_host workspace (device), grown on demand
+    int           fft_dims[3];    // lya_fields_from_dm: cached cuFFT plans (handles are ints) for [nz][ny][nx]
+    int           fft_r2c, fft_c2r;
+    // lya_forest_host / lya_fields_from_dm workspace (device), grown on demand
     void         *ws;
     size_t        ws_bytes;
     char          err[512];
@@ -66,6 +68,8 @@ static inline lya_status lya_cuda_fail(lya_ctx *ctx, cudaError_t e, const char *
 #define LYA_RHOCRIT100 1.87834e-29            // g/cm^3 for h = 1
 #define LYA_NHI_COEFF  7.24e-6                // Eq.4
 #define LYA_ALPHA_T    (-0.7)                 // recombination-rate temperature slope
+
+void lya_fields_release(lya_ctx *ctx);   // fields.cu: destroys the cached cuFFT plans
 
 // kernels' host launchers (each enqueues on ctx->stream and bumps ctx->launches)
 lya_status lya_launch_gas(lya_ctx *ctx, const float *delta, size_t n, float *n_hi, float *b,

@@ -41,6 +41,11 @@ class CInstrument(C.Structure):
     _fields_ = [("fwhm_kms", C.c_double), ("bin_kms", C.c_double), ("snr", C.c_double)]
 
 
+class CFieldParams(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32), ("box_mpch", C.c_double),
+                ("h", C.c_double), ("z", C.c_double), ("omega_m", C.c_double), ("k_filter_mpc", C.c_double)]
+
+
 class CRootState(C.Structure):
     _fields_ = [("f_target", C.c_double), ("rel_tol", C.c_double), ("n_pix", C.c_double),
                 ("lo", C.c_double), ("hi", C.c_double), ("a", C.c_double), ("f_at_a", C.c_double),
@@ -80,7 +85,7 @@ EXPORTS = ("lya_version", "lya_status_string", "lya_scalars_from_params", "lya_c
            "lya_normalize_mean_flux", "lya_flux_partial_sums", "lya_root_init", "lya_root_update",
            "lya_flux", "lya_forest_host", "lya_launch_count", "lya_measure_mufu_peak",
            "lya_bin_kms_from_angstrom", "lya_instrument_bins", "lya_observe_rows", "lya_flux_pdf",
-           "lya_flux_power_rows", "lya_tau_sightlines_opt")
+           "lya_flux_power_rows", "lya_tau_sightlines_opt", "lya_growth_rate", "lya_fields_from_dm")
 
 _lib = None
 
@@ -117,6 +122,8 @@ def lib() -> C.CDLL:
     L.lya_forest_host.argtypes = [vp, pp, C.c_int, C.c_int32, fp, fp, C.c_double, C.c_double, C.c_int,
                                   fp, fp, dp, dp, ip]
     L.lya_measure_mufu_peak.argtypes = [vp, dp]
+    L.lya_growth_rate.argtypes = [C.c_double, C.c_double, dp]
+    L.lya_fields_from_dm.argtypes = [vp, C.POINTER(CFieldParams), fp, fp, fp, fp, fp]
     L.lya_bin_kms_from_angstrom.argtypes = [C.c_double, C.c_double]
     L.lya_bin_kms_from_angstrom.restype = C.c_double
     L.lya_instrument_bins.argtypes = [C.c_int32, C.c_double, C.POINTER(CInstrument)]
@@ -130,6 +137,13 @@ def lib() -> C.CDLL:
 
 def bin_kms_from_angstrom(z: float, dlambda: float) -> float:
     return float(lib().lya_bin_kms_from_angstrom(z, dlambda))
+
+
+def growth_rate(z: float, omega_m: float) -> float:
+    f = C.c_double()
+    if lib().lya_growth_rate(z, omega_m, C.byref(f)) != OK:
+        raise LyaError(EINVAL, "lya_growth_rate: bad arguments")
+    return f.value
 
 
 def scalars(p: Params, axis: int = 0) -> dict:
@@ -287,6 +301,18 @@ class Context:
         self._check(lib().lya_flux_power_rows(self._h, flux.numel() // n_pix, n_pix, dv_kms, _dev(flux, "flux"),
                                               mean_flux, P))
         return np.array(P, dtype=np.float64)
+
+    # before the hot path: Eq.1 and Eq.3
+    def fields_from_dm(self, delta_dm, box_mpch: float, h: float, z: float, omega_m: float, k_filter_mpc: float,
+                       want=("delta_b", "v_x", "v_y", "v_z")):
+        """delta_dm: [nz][ny][nx] CUDA fp32, box_mpch along x.  Returns a dict of the requested fields."""
+        nz, ny, nx = delta_dm.shape
+        fpar = CFieldParams(nx, ny, nz, box_mpch, h, z, omega_m, k_filter_mpc)
+        out = {k: torch.empty_like(delta_dm) for k in want}
+        ptr = lambda k: _dev(out[k], k) if k in out else None
+        self._check(lib().lya_fields_from_dm(self._h, C.byref(fpar), _dev(delta_dm, "delta_dm"), ptr("delta_b"),
+                                             ptr("v_x"), ptr("v_y"), ptr("v_z")))
+        return out
 
     # S1..S5 from host buffers
     def forest_host(self, p: Params, axis: int, delta_h, v_pec_h, f_target: float, rel_tol: float = 1e-7,
