@@ -281,6 +281,14 @@ def bench_ours(args) -> dict:
                                 "frac_hbm": 4 * n_cells / t_pow / 1e6 / pk["hbm_gbs"],
                                 "note": "radix-2 FFT in shared memory: shared-memory bound, not HBM bound"}}
         del noise, obs_out
+        # delta_b and v_x from a DM field (here: the workload's delta) -- one R2C, two k-space
+        # kernels, two C2R; the FFTs are cuFFT's
+        if w.cfg <= 3 or args.fields:
+            t_fld = timed_ms(lambda: ctx.fields_from_dm(delta, w.box_mpch, w.h, w.z, w.omega_m, 6.5,
+                                                        want=("delta_b", "v_x")), reps=3)
+            next_rows["fields_from_dm"] = {"outputs": "delta_b, v_x", "ms": t_fld,
+                                           "kspace_kernel_bytes": int(2 * 16 * (n // 2 + 1) * n * n),
+                                           "note": "3 cuFFT transforms + 2 k-space kernels (8 B in + 8 B out per mode)"}
 
     # ---- end to end through lya_forest_host: pinned host inputs, F read back, every step
     e2e = None
@@ -429,6 +437,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--fields", action="store_true", help="time lya_fields_from_dm on config 4 too (17 GB of workspace)")
     ap.add_argument("--no-next", action="store_true", help="skip the per-kernel timing of the rows after F")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     args = ap.parse_args()
