@@ -109,6 +109,8 @@ void lya_destroy(lya_ctx *ctx)
     if (ctx->d_stats) cudaFree(ctx->d_stats);
     if (ctx->d_taps) cudaFree(ctx->d_taps);
     free(ctx->h_taps);
+    if (ctx->d_bins) cudaFree(ctx->d_bins);
+    free(ctx->h_bins);
     if (ctx->h_pinned) cudaFreeHost(ctx->h_pinned);
     for (int i = 0; i < 2; ++i) {
         if (ctx->ev_copy[i]) cudaEventDestroy(ctx->ev_copy[i]);

@@ -25,6 +25,8 @@ struct lya_ctx {
     double       *d_stats;        // 8192 doubles: flux-PDF counts (as uint64) / power-spectrum accumulators
     float        *d_taps, *h_taps; // lya_observe_rows: Gaussian taps (device / host staging), grown on demand
     size_t        taps_cap;
+    void         *d_bins, *h_bins; // lya_observe_rows: per-bin geometry table (int4 per output bin)
+    size_t        bins_cap;
     int           fft_dims[3];    // lya_fields_from_dm: cached cuFFT plans (handles are ints) for [nz][ny][nx]
     int           fft_r2c, fft_c2r;
     // lya_forest_host / lya_fields_from_dm workspace (device), grown on demand

@@ -29,6 +29,7 @@ struct ObsArgs {
     unsigned long long bin_fx;            // B = bin / dv [pixels] in 32.32 fixed point
     float        inv_bin_f;               // 1 / B
     float        inv_snr;                 // 0: no noise
+    const int4  *bins;                    // lean kernel: per output bin {i0, i1, bits(w_first), bits(w_last)}
 };
 
 // A CTA works on batches of D rows.  NV = float4 loads per thread and row (n4 <= 4 * NV * blockDim.x).  The
@@ -199,6 +200,92 @@ __global__ void __launch_bounds__(256) observe_rows_kernel(const ObsArgs a)
     }
 }
 
+// ---- the lean kernel: the common case (16-byte aligned rows, n % 4 == 0, at most LT + 1 <= 125 taps incl. the
+// alignment padding, one float4 per thread and row).  Same data flow as above, but the instruction count per
+// pixel is roughly halved: the taps arrive as a __grid_constant__ kernel parameter, so with the tap loop fully
+// unrolled every FFMA takes its weight straight from the constant bank and every LDS.128 of inputs has an
+// immediate offset (17 instructions per 16 FFMA instead of 26); and the bin geometry of the rebinning, which
+// is the same for every row, comes from a table built once on the host (bins[m] = first pixel, last pixel,
+// weight of the first and of the last pixel) and kept in shared memory.
+struct ObsTaps { float wp[136]; };                       // wp[t + 3] = g(KO - t); zero outside the real taps
+
+template <int LT>                                        // LT >= L, multiple of 4: taps t = 0 .. LT
+__global__ void __launch_bounds__(256) observe_rows_lean_kernel(const ObsArgs a, const __grid_constant__ ObsTaps tp)
+{
+    extern __shared__ __align__(16) float sm[];
+    const int n = a.n, T = blockDim.x, tid = threadIdx.x;
+    const int in_len = n + LT + 8;
+    float *s_in = sm;                                    // s_in[h] = F[(h - KO) mod n], zero beyond n + L
+    float *s_c  = sm + in_len;                           // convolved row, n floats
+    int4  *s_b  = reinterpret_cast<int4 *>(s_c + n);     // bin table, nb entries (rebin only)
+    for (int h = tid; h < in_len; h += T) s_in[h] = 0.0f;
+    if (a.rebin)
+        for (int m = tid; m < a.nb; m += T) s_b[m] = a.bins[m];
+
+    const int p = 4 * tid;                               // this thread's pixels p .. p+3 (p < n by construction)
+    float4 reg = make_float4(0.f, 0.f, 0.f, 0.f);
+    float hreg = 0.0f, nzr[OBS_NBR];
+    auto fetch = [&](size_t row) {
+        const float *src = a.flux + row * (size_t)n;
+        if (p < n) reg = __ldcs(reinterpret_cast<const float4 *>(src + p));
+        if (tid < a.L) hreg = __ldg(src + (tid < a.KO ? n - a.KO + tid : tid - a.KO));
+    };
+    size_t row = blockIdx.x;
+    if (row < a.n_rows) fetch(row);
+    for (; row < a.n_rows; row += gridDim.x) {
+        __syncthreads();                                 // previous row's s_in / s_c consumed
+        if (p < n) *reinterpret_cast<float4 *>(s_in + a.KO + p) = reg;
+        if (tid < a.L) s_in[tid < a.KO ? tid : n + tid] = hreg;
+        if (row + gridDim.x < a.n_rows) fetch(row + gridDim.x);
+        if (a.noise) {
+#pragma unroll
+            for (int k = 0; k < OBS_NBR; ++k) {
+                const int m = tid + k * T;
+                nzr[k] = m < a.nb ? __ldcs(a.noise + row * (size_t)a.nb + m) : 0.0f;
+            }
+        }
+        __syncthreads();
+        if (p < n) {
+            const float *si = s_in + p;
+            float acc0 = 0.f, acc1 = 0.f, acc2 = 0.f, acc3 = 0.f;
+#pragma unroll
+            for (int u = 0; u < LT + 4; u += 4) {        // input u and output r use wp[u - r + 3]
+                const float4 x = *reinterpret_cast<const float4 *>(si + u);
+                acc0 = fmaf(tp.wp[u + 3], x.x, acc0); acc0 = fmaf(tp.wp[u + 4], x.y, acc0); acc0 = fmaf(tp.wp[u + 5], x.z, acc0); acc0 = fmaf(tp.wp[u + 6], x.w, acc0);
+                acc1 = fmaf(tp.wp[u + 2], x.x, acc1); acc1 = fmaf(tp.wp[u + 3], x.y, acc1); acc1 = fmaf(tp.wp[u + 4], x.z, acc1); acc1 = fmaf(tp.wp[u + 5], x.w, acc1);
+                acc2 = fmaf(tp.wp[u + 1], x.x, acc2); acc2 = fmaf(tp.wp[u + 2], x.y, acc2); acc2 = fmaf(tp.wp[u + 3], x.z, acc2); acc2 = fmaf(tp.wp[u + 4], x.w, acc2);
+                acc3 = fmaf(tp.wp[u + 0], x.x, acc3); acc3 = fmaf(tp.wp[u + 1], x.y, acc3); acc3 = fmaf(tp.wp[u + 2], x.z, acc3); acc3 = fmaf(tp.wp[u + 3], x.w, acc3);
+            }
+            *reinterpret_cast<float4 *>(s_c + p) = make_float4(acc0, acc1, acc2, acc3);
+        }
+        __syncthreads();
+
+        float *dst = a.out + row * (size_t)a.nb;
+#pragma unroll
+        for (int k = 0; k < OBS_NBR; ++k) {              // nb <= OBS_NBR * T is a launch condition
+            const int m = tid + k * T;
+            if (m < a.nb) {
+                float v;
+                if (a.rebin) {
+                    const int4 e = s_b[m];
+                    if (e.y <= e.x) {
+                        v = __int_as_float(e.z) * s_c[e.x];                       // bin inside one pixel
+                    } else {                                                      // weights carry the 1/B
+                        float mid = 0.0f;
+#pragma unroll 1
+                        for (int i = e.x + 1; i < e.y; ++i) mid += s_c[i];
+                        v = fmaf(__int_as_float(e.w), s_c[e.y], fmaf(mid, a.inv_bin_f, __int_as_float(e.z) * s_c[e.x]));
+                    }
+                } else {
+                    v = s_c[m];
+                }
+                if (a.noise) v = fmaf(nzr[k], a.inv_snr, v);
+                __stcs(dst + m, v);
+            }
+        }
+    }
+}
+
 // ---- flux PDF: private per-thread histograms in shared memory (hist[bin][thread]: conflict-free, no atomics)
 constexpr int PDF_THREADS = 128;
 
@@ -318,6 +405,60 @@ extern "C" lya_status lya_observe_rows(lya_ctx *ctx, size_t n_rows, int32_t n_pi
         }
         LYA_CUDA(ctx, cudaMemcpyAsync(ctx->d_taps, ctx->h_taps, (size_t)n_t * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
         a.taps = ctx->d_taps;
+    }
+    // ---- lean kernel for the common case
+    if (fast && a.L >= 0 && a.L <= 124 && a.n4 / 4 <= threads && nb <= OBS_NBR * threads) {
+        ObsTaps tp;
+        memset(&tp, 0, sizeof(tp));
+        for (int t = 0; t < a.L + 11; ++t) tp.wp[t] = ctx->h_taps[t];
+        if (a.rebin) {
+            if (ctx->bins_cap < (size_t)nb) {
+                if (ctx->d_bins) cudaFree(ctx->d_bins);
+                ctx->d_bins = nullptr; ctx->bins_cap = 0;
+                free(ctx->h_bins);
+                ctx->h_bins = malloc((size_t)(nb + 64) * sizeof(int4));
+                if (!ctx->h_bins) return lya_fail(ctx, LYA_ENOMEM, "lya_observe_rows: host allocation failed");
+                LYA_CUDA(ctx, cudaMalloc(&ctx->d_bins, (size_t)(nb + 64) * sizeof(int4)));
+                ctx->bins_cap = (size_t)nb + 64;
+            }
+            LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));             // previous call may still read h_bins
+            int4 *hb = (int4 *)ctx->h_bins;
+            for (int m = 0; m < nb; ++m) {                                  // bin [lo, hi) in pixel units (reading O2)
+                const double lo = (double)m * bin_px, hi = lo + bin_px;
+                int i0 = (int)floor(lo), i1 = (int)ceil(hi) - 1;
+                if (i1 > n_pix - 1) i1 = n_pix - 1;
+                float wf, wl;
+                if (i1 <= i0) { i1 = i0; wf = (float)((hi - lo) / bin_px); wl = 0.0f; }
+                else { wf = (float)(((double)(i0 + 1) - lo) / bin_px); wl = (float)((hi - (double)i1) / bin_px); }
+                int4 e;
+                e.x = i0; e.y = i1;
+                memcpy(&e.z, &wf, 4); memcpy(&e.w, &wl, 4);
+                hb[m] = e;
+            }
+            LYA_CUDA(ctx, cudaMemcpyAsync(ctx->d_bins, hb, (size_t)nb * sizeof(int4), cudaMemcpyHostToDevice, ctx->stream));
+            a.bins = (const int4 *)ctx->d_bins;
+        }
+        // LT: the smallest instantiated multiple of 4 that is >= L (every multiple of 4 up to 64, then 96, 124)
+        const int LT = a.L <= 64 ? ((a.L + 3) & ~3) : (a.L <= 96 ? 96 : 124);
+        void (*lean)(const ObsArgs, const ObsTaps) = nullptr;
+        switch (LT) {
+#define LYA_LEAN(N) case N: lean = observe_rows_lean_kernel<N>; break;
+            LYA_LEAN(0) LYA_LEAN(4) LYA_LEAN(8) LYA_LEAN(12) LYA_LEAN(16) LYA_LEAN(20) LYA_LEAN(24) LYA_LEAN(28)
+            LYA_LEAN(32) LYA_LEAN(36) LYA_LEAN(40) LYA_LEAN(44) LYA_LEAN(48) LYA_LEAN(52) LYA_LEAN(56) LYA_LEAN(60)
+            LYA_LEAN(64) LYA_LEAN(96) LYA_LEAN(124)
+#undef LYA_LEAN
+        }
+        const size_t smem_l = ((size_t)n_pix + LT + 8 + n_pix) * sizeof(float) + (a.rebin ? (size_t)nb * sizeof(int4) : 0);
+        LYA_CUDA(ctx, cudaFuncSetAttribute(lean, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_l));
+        int per_sm_l = 0;
+        LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_l, lean, threads, smem_l));
+        if (per_sm_l >= 1) {
+            const size_t cap_l = (size_t)ctx->sm_count * per_sm_l;
+            lean<<<(int)(n_rows < cap_l ? n_rows : cap_l), threads, smem_l, ctx->stream>>>(a, tp);
+            ctx->launches++;
+            LYA_CUDA(ctx, cudaGetLastError());
+            return LYA_OK;
+        }
     }
     const int nv = (a.n4 / 4 + threads - 1) / threads;                 // float4 per thread and row
     void (*kern)(const ObsArgs) = nullptr;
