@@ -1,9 +1,10 @@
 // normalize.cu -- S4 and S5: mean-flux normalisation constant A and F = exp(-A tau).
 //
 // S4: one cooperative, persistent kernel runs the whole iteration on the device.  Each pass streams tau once
-// (4 B / pixel, 128-bit loads), evaluates e = ex2(-A log2(e) tau) on the MUFU pipe and reduces both
-// sum(e) and sum(tau e) -- fp32 only inside one float4, double from the thread level up, warp shuffles, then
-// one partial pair per block.  After a grid-wide barrier EVERY block reduces the same partials in the same
+// (4 B / pixel, 128-bit loads), evaluates e = ex2(-A log2(e) tau) on the MUFU pipe and reduces the five tilted
+// moments sum(tau^k e), k = 0..4 -- fp32 only inside one float4, double from the thread level up, warp
+// shuffles, then five partials per block; the moments give a fifth-order step (root_iter.h), so the whole
+// iteration takes 3-4 passes.  After a grid-wide barrier EVERY block reduces the same partials in the same
 // order and applies the same scalar update (root_iter.h), so no second barrier or broadcast is needed and the
 // result is bit-reproducible.  The host sees only the final (A, <F>, passes, status).
 //
@@ -82,6 +83,56 @@ __device__ __forceinline__ void accumulate(const float *__restrict__ tau, size_t
     }
 }
 
+// the same stream, five tilted moments sum tau^k e, k = 0..4, for one trial (lya_root_step_moments)
+__device__ __forceinline__ void accumulate_moments(const float *__restrict__ tau, size_t n, const Trial &tr, double (&s)[5])
+{
+#pragma unroll
+    for (int k = 0; k < 5; ++k) s[k] = 0.0;
+    const size_t gtid = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t gsz  = (size_t)gridDim.x * blockDim.x;
+    size_t head = ((16 - ((uintptr_t)tau & 15)) & 15) >> 2;
+    if (head > n) head = n;
+    const size_t n4 = (n - head) >> 2;
+    const float4 *t4 = reinterpret_cast<const float4 *>(tau + head);
+    // fp32 inside a group of up to four float4 (16 pixels), double above: one cvt + DADD per moment and group
+    float q[5] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
+    auto add4 = [&](const float4 &t) {
+        float pa = flux_of(t.x, tr), pb = flux_of(t.y, tr), pc = flux_of(t.z, tr), pd = flux_of(t.w, tr);
+        q[0] += (pa + pb) + (pc + pd);
+#pragma unroll
+        for (int k = 1; k < 5; ++k) {
+            pa *= t.x; pb *= t.y; pc *= t.z; pd *= t.w;
+            q[k] += (pa + pb) + (pc + pd);
+        }
+    };
+    size_t i = gtid;
+    for (; i + 3 * gsz < n4; i += 4 * gsz) {
+        const float4 t0 = __ldg(t4 + i), t1 = __ldg(t4 + i + gsz), t2 = __ldg(t4 + i + 2 * gsz), t3 = __ldg(t4 + i + 3 * gsz);
+#pragma unroll
+        for (int k = 0; k < 5; ++k) q[k] = 0.0f;
+        add4(t0); add4(t1); add4(t2); add4(t3);
+#pragma unroll
+        for (int k = 0; k < 5; ++k) s[k] += (double)q[k];
+    }
+    for (; i < n4; i += gsz) {
+        const float4 t0 = __ldg(t4 + i);
+#pragma unroll
+        for (int k = 0; k < 5; ++k) q[k] = 0.0f;
+        add4(t0);
+#pragma unroll
+        for (int k = 0; k < 5; ++k) s[k] += (double)q[k];
+    }
+    const size_t tail0 = head + (n4 << 2);
+    const size_t n_edge = head + (n - tail0);
+    for (size_t e = gtid; e < n_edge; e += gsz) {
+        const size_t i = e < head ? e : tail0 + (e - head);
+        const float t = tau[i];
+        float p = flux_of(t, tr);
+#pragma unroll
+        for (int k = 0; k < 5; ++k) { s[k] += (double)p; p *= t; }
+    }
+}
+
 __device__ __forceinline__ double warp_sum(double v)
 {
 #pragma unroll
@@ -115,36 +166,36 @@ struct NormArgs {
     size_t       n;
     double       f_target, rel_tol;
     int          max_iter;
-    double      *partials;     // [2][gridDim.x][2]
+    double      *partials;     // [2][gridDim.x][5]
     double      *result;       // [0] A, [1] <F> at A, [2] passes, [3] status
 };
 
-__global__ void __launch_bounds__(RED_THREADS) normalize_kernel(const NormArgs a)
+__global__ void __launch_bounds__(RED_THREADS, 4) normalize_kernel(const NormArgs a)
 {
     cg::grid_group grid = cg::this_grid();
-    __shared__ double sh[2 * 32];
+    __shared__ double sh[5 * 32];
     __shared__ lya_root_state st;
     if (threadIdx.x == 0) lya_root_reset(&st, a.f_target, a.rel_tol, (double)a.n);
     __syncthreads();
 
     for (int pass = 0;; ++pass) {
-        Trial tr[1] = {make_trial(st.a)};
-        double s[2], s0[1], s1[1];
-        accumulate<1>(a.tau, a.n, tr, s0, s1);
-        s[0] = s0[0]; s[1] = s1[0];
-        block_sum<2>(s, sh);
-        double *part = a.partials + (size_t)(pass & 1) * gridDim.x * 2;
-        if (threadIdx.x == 0) { part[2 * blockIdx.x] = s[0]; part[2 * blockIdx.x + 1] = s[1]; }
+        const Trial tr = make_trial(st.a);
+        double s[5];
+        accumulate_moments(a.tau, a.n, tr, s);
+        block_sum<5>(s, sh);
+        double *part = a.partials + (size_t)(pass & 1) * gridDim.x * 5;
+        if (threadIdx.x == 0)
+#pragma unroll
+            for (int k = 0; k < 5; ++k) part[5 * blockIdx.x + k] = s[k];
         grid.sync();
         // every block: identical fixed-order reduction of all partials
-        double t[2] = {0.0, 0.0};
-        for (unsigned b = threadIdx.x; b < gridDim.x; b += blockDim.x) {
-            t[0] += __ldcg(part + 2 * b);
-            t[1] += __ldcg(part + 2 * b + 1);
-        }
-        block_sum<2>(t, sh);
+        double t[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+        for (unsigned b = threadIdx.x; b < gridDim.x; b += blockDim.x)
+#pragma unroll
+            for (int k = 0; k < 5; ++k) t[k] += __ldcg(part + 5 * b + k);
+        block_sum<5>(t, sh);
         if (threadIdx.x == 0) {
-            lya_root_step(&st, t[0], t[1]);
+            lya_root_step_moments(&st, t);
             if (!st.done && st.iters >= a.max_iter) { st.status = LYA_ENOCONV; st.done = 1; }
         }
         __syncthreads();
