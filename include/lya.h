@@ -146,6 +146,13 @@ typedef struct {
 lya_status lya_root_init(lya_root_state *s, double f_target, double rel_tol, double n_pix_global);
 lya_status lya_root_update(lya_root_state *s, double sum_exp, double sum_tau_exp);
 
+/* The same building blocks with the five tilted moments sums5[k] = sum_p tau_p^k exp(-a_trial tau_p), k = 0..4,
+ * which lya_normalize_mean_flux's device loop uses: lya_root_update_moments solves a quartic cumulant model of
+ * ln <exp(-A tau)> (fifth-order convergence, 3-4 passes instead of 7-8, no confirming pass: when it sets done,
+ * f_at_a is the model's value at the final a).  Feed the GLOBAL sums.  tau DEVICE; sums5 HOST. */
+lya_status lya_flux_moment_sums(lya_ctx *ctx, const float *tau, size_t n_pix, double a_trial, double *sums5);
+lya_status lya_root_update_moments(lya_root_state *s, const double *sums5);
+
 /* S5.  tau, flux: DEVICE, n_pix floats; flux == tau (in place) allowed.  Asynchronous. */
 lya_status lya_flux(lya_ctx *ctx, const float *tau, size_t n_pix, double a, float *flux);
 

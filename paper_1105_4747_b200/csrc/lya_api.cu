@@ -234,6 +234,24 @@ lya_status lya_root_init(lya_root_state *s, double f_target, double rel_tol, dou
     return LYA_OK;
 }
 
+lya_status lya_flux_moment_sums(lya_ctx *ctx, const float *tau, size_t n_pix, double a_trial, double *sums5)
+{
+    if (!ctx) return LYA_EINVAL;
+    ctx->err[0] = 0;
+    if (!tau || ((uintptr_t)tau & 3) || !sums5) return lya_fail(ctx, LYA_EINVAL, "lya_flux_moment_sums: null or misaligned pointer");
+    if (!(a_trial >= 0.0) || !(a_trial < 1.0e30)) return lya_fail(ctx, LYA_EINVAL, "lya_flux_moment_sums: trial A must be finite and >= 0");
+    if (n_pix == 0) { for (int i = 0; i < 5; ++i) sums5[i] = 0.0; return LYA_OK; }
+    LYA_CUDA(ctx, cudaSetDevice(ctx->device));
+    return lya_run_moment_sums(ctx, tau, n_pix, a_trial, sums5);
+}
+
+lya_status lya_root_update_moments(lya_root_state *s, const double *sums5)
+{
+    if (!s || !sums5 || s->done) return LYA_EINVAL;
+    lya_root_step_moments(s, sums5);
+    return (lya_status)s->status;
+}
+
 lya_status lya_root_update(lya_root_state *s, double sum_exp, double sum_tau_exp)
 {
     if (!s || s->done) return LYA_EINVAL;

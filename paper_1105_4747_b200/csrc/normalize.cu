@@ -229,6 +229,18 @@ __global__ void __launch_bounds__(RED_THREADS) partial_sums_kernel(const float *
         for (int k = 0; k < 2 * K; ++k) partials[(size_t)blockIdx.x * 2 * K + k] = s[k];
 }
 
+__global__ void __launch_bounds__(RED_THREADS) moment_sums_kernel(const float *__restrict__ tau, size_t n, const Trial tr,
+                                                                 double *partials)
+{
+    __shared__ double sh[5 * 32];
+    double s[5];
+    accumulate_moments(tau, n, tr, s);
+    block_sum<5>(s, sh);
+    if (threadIdx.x == 0)
+#pragma unroll
+        for (int k = 0; k < 5; ++k) partials[(size_t)blockIdx.x * 5 + k] = s[k];
+}
+
 // one block: fixed-order sum of the per-block partials -> out[0 .. nv)
 __global__ void __launch_bounds__(RED_THREADS) finish_sums_kernel(const double *partials, int n_blocks, int nv,
                                                                   double *out)
@@ -342,5 +354,18 @@ lya_status lya_launch_flux(lya_ctx *ctx, const float *tau, size_t n, double a, f
     flux_kernel<<<grid, 256, 0, ctx->stream>>>(tau, n, make_trial(a), flux);
     ctx->launches++;
     LYA_CUDA(ctx, cudaGetLastError());
+    return LYA_OK;
+}
+
+lya_status lya_run_moment_sums(lya_ctx *ctx, const float *tau, size_t n, double a_trial, double *sums5)
+{
+    const int grid = red_grid(ctx, n, 8);
+    moment_sums_kernel<<<grid, RED_THREADS, 0, ctx->stream>>>(tau, n, make_trial(a_trial), ctx->d_partials);
+    finish_sums_kernel<<<1, RED_THREADS, 0, ctx->stream>>>(ctx->d_partials, grid, 5, ctx->d_root);
+    ctx->launches += 2;
+    LYA_CUDA(ctx, cudaGetLastError());
+    LYA_CUDA(ctx, cudaMemcpyAsync(ctx->h_pinned, ctx->d_root, 5 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    for (int i = 0; i < 5; ++i) sums5[i] = ctx->h_pinned[i];
     return LYA_OK;
 }

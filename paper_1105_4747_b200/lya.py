@@ -85,7 +85,8 @@ EXPORTS = ("lya_version", "lya_status_string", "lya_scalars_from_params", "lya_c
            "lya_normalize_mean_flux", "lya_flux_partial_sums", "lya_root_init", "lya_root_update",
            "lya_flux", "lya_forest_host", "lya_launch_count", "lya_measure_mufu_peak",
            "lya_bin_kms_from_angstrom", "lya_instrument_bins", "lya_observe_rows", "lya_flux_pdf",
-           "lya_flux_power_rows", "lya_tau_sightlines_opt", "lya_growth_rate", "lya_fields_from_dm")
+           "lya_flux_power_rows", "lya_tau_sightlines_opt", "lya_growth_rate", "lya_fields_from_dm", "lya_flux_moment_sums",
+           "lya_root_update_moments")
 
 _lib = None
 
@@ -118,6 +119,8 @@ def lib() -> C.CDLL:
     L.lya_flux_partial_sums.argtypes = [vp, fp, C.c_size_t, dp, C.c_int, dp, dp]
     L.lya_root_init.argtypes = [C.POINTER(CRootState), C.c_double, C.c_double, C.c_double]
     L.lya_root_update.argtypes = [C.POINTER(CRootState), C.c_double, C.c_double]
+    L.lya_flux_moment_sums.argtypes = [vp, fp, C.c_size_t, C.c_double, dp]
+    L.lya_root_update_moments.argtypes = [C.POINTER(CRootState), dp]
     L.lya_flux.argtypes = [vp, fp, C.c_size_t, C.c_double, fp]
     L.lya_forest_host.argtypes = [vp, pp, C.c_int, C.c_int32, fp, fp, C.c_double, C.c_double, C.c_int,
                                   fp, fp, dp, dp, ip]
@@ -263,6 +266,11 @@ class Context:
         self._check(lib().lya_flux_partial_sums(self._h, _dev(tau, "tau"), tau.numel(), at, k, s, d))
         return list(s), list(d)
 
+    def flux_moment_sums(self, tau, a_trial: float):
+        s5 = (C.c_double * 5)()
+        self._check(lib().lya_flux_moment_sums(self._h, _dev(tau, "tau"), tau.numel(), a_trial, s5))
+        return list(s5)
+
     # S5
     def flux(self, tau, a: float, out=None):
         out = torch.empty_like(tau) if out is None else out
@@ -330,8 +338,8 @@ def normalize_mean_flux_sharded(ctx: Context, tau_local, f_target: float, n_pix_
                                 rel_tol: float = 1e-7, max_iter: int = 60, group=None, partial_sums=None):
     """S4 when the pixels are sharded over ranks (z-slabs per GPU).
 
-    Each pass: local (sum e, sum tau e) from lya_flux_partial_sums, one all-reduce of two doubles, then the
-    library's scalar update lya_root_update -- identical on every rank, so all ranks hold the same A.
+    Each pass: the five local tilted moments from lya_flux_moment_sums, one all-reduce of five doubles, then the
+    library's scalar update lya_root_update_moments -- identical on every rank, so all ranks hold the same A.
     `partial_sums` lets a CPU test (gloo) stand in for the kernel; the product path leaves it None.
     """
     import torch.distributed as dist
@@ -339,16 +347,21 @@ def normalize_mean_flux_sharded(ctx: Context, tau_local, f_target: float, n_pix_
     st = CRootState()
     if L.lya_root_init(C.byref(st), f_target, rel_tol, float(n_pix_global)) != OK:
         raise LyaError(EINVAL, "lya_root_init: bad arguments")
-    sums_fn = partial_sums if partial_sums is not None else (lambda a: ctx.flux_partial_sums(tau_local, [a]))
+    # per pass: five local tilted moments (or, with the two-sum stand-in of a CPU test, sum e and sum tau e)
+    sums_fn = partial_sums if partial_sums is not None else (lambda a: ctx.flux_moment_sums(tau_local, a))
     while not st.done:
-        s, d = sums_fn(st.a)
-        buf = torch.tensor([s[0], d[0]], dtype=torch.float64)
+        got = sums_fn(st.a)
+        vals = list(got) if len(got) == 5 else [got[0][0], got[1][0]]
+        buf = torch.tensor(vals, dtype=torch.float64)
         if dist.is_available() and dist.is_initialized():
             if dist.get_backend(group) == "nccl":
                 buf = buf.cuda()
             dist.all_reduce(buf, op=dist.ReduceOp.SUM, group=group)
             buf = buf.cpu()
-        rc = L.lya_root_update(C.byref(st), float(buf[0]), float(buf[1]))
+        if len(vals) == 5:
+            rc = L.lya_root_update_moments(C.byref(st), (C.c_double * 5)(*[float(x) for x in buf]))
+        else:
+            rc = L.lya_root_update(C.byref(st), float(buf[0]), float(buf[1]))
         if rc == ENOROOT:
             raise LyaError(rc, "no A > 0 reaches f_target")
         if not st.done and st.iters >= max_iter:

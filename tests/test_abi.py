@@ -143,3 +143,37 @@ def test_params_struct_layout_matches_header():
     assert C.sizeof(lya.CParams) == 16 + 10 * 8
     assert C.sizeof(lya.CScalars) == 8 + 11 * 8
     assert C.sizeof(lya.CRootState) == 7 * 8 + 4 * 4
+
+
+def test_root_iteration_with_moments_closed_forms_and_oracle(oracle):
+    """lya_root_update_moments (quartic cumulant model of ln f): exact in two passes for constant tau (ln f is
+    linear), and the oracle's A on a heavy-tailed sample in at most 6 passes."""
+    import ctypes as C
+    L = lya.lib()
+
+    def solve(tau, f_target, tol=1e-12):
+        st = lya.CRootState()
+        assert L.lya_root_init(C.byref(st), f_target, tol, float(tau.size)) == lya.OK
+        while not st.done:
+            e = np.exp(-st.a * tau)
+            s5 = (C.c_double * 5)(*[float((tau ** k * e).sum()) for k in range(5)])
+            assert L.lya_root_update_moments(C.byref(st), s5) == lya.OK
+            assert st.iters < 30
+        return st.a, st.f_at_a, st.iters
+
+    A, f, it = solve(np.full(1000, 0.7), 0.8)
+    assert A == pytest.approx(-np.log(0.8) / 0.7, rel=1e-13) and f == pytest.approx(0.8, rel=1e-13) and it <= 2
+    tau1 = 0.4
+    tau = np.concatenate([np.full(500, tau1), np.full(500, 2 * tau1)])          # x^2 + x = 2 F, x = exp(-A tau1)
+    A, f, it = solve(tau, 0.6)
+    x = (-1 + np.sqrt(1 + 8 * 0.6)) / 2
+    assert A == pytest.approx(-np.log(x) / tau1, rel=1e-11) and it <= 6
+    rng = np.random.default_rng(3)
+    tau = rng.lognormal(-1.0, 1.5, 300_000)
+    for ft in (0.9, 0.78, 0.3):
+        A, f, it = solve(tau, ft, tol=1e-10)
+        A_ref, _, _ = oracle.normalize_mean_flux(tau, ft)
+        assert A == pytest.approx(A_ref, rel=1e-9) and abs(f - ft) < 1e-9 and it <= 6
+    st = lya.CRootState()                                                           # all tau == 0: no root
+    L.lya_root_init(C.byref(st), 0.8, 1e-9, 10.0)
+    assert L.lya_root_update_moments(C.byref(st), (C.c_double * 5)(10.0, 0.0, 0.0, 0.0, 0.0)) == lya.ENOROOT
