@@ -34,8 +34,8 @@ METRIC = "tau_pixel_pair_evals_per_s"
 UNIT = "pair-evals/s"
 SM_COUNT_B200, MUFU_PER_CLK_SM = 148, 16          # MUFU.EX2 results / clk / SM
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE tau-kernel launch (x pass), from the committed
-# `ncu --set full` captures in profiles/r1_ncu_full_v3.md; algorithmic traffic is 16 B per cell
-TAU_TRAFFIC_BYTES = {2: 201.416192e6 + 35.475200e6, 3: 1.612064e9 + 0.505183e9}
+# `ncu --set full` captures in profiles/r1_ncu_full_final.md; algorithmic traffic is 16 B per cell
+TAU_TRAFFIC_BYTES = {2: 201.476864e6 + 35.543552e6, 3: 1.611410e9 + 0.504592e9}
 
 
 def peaks() -> dict:
@@ -343,7 +343,7 @@ def bench_ours(args) -> dict:
         "kernel_ms": k_ms, "wall_s_timed_region_incl_flush": wall,
         "roofline": {"bound": "alu", "kernel": "tau_kernel", "achieved": tau_rate / 1e9, "peak": f_peak / 1e9,
                      "unit": "Gpair-evals/s", "frac": tau_rate / f_peak, "traffic": TAU_TRAFFIC_BYTES.get(w.cfg),
-                     "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1_ncu_full_v3.md); algorithmic %d" % (16 * n_cells),
+                     "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1_ncu_full_final.md); algorithmic %d" % (16 * n_cells),
                      "peak_measured": mufu_measured / 1e9, "frac_of_measured_peak": tau_rate / mufu_measured,
                      "peak_def": "16 MUFU.EX2/clk/SM x %d SMs x %.0f MHz (max SM clock, %s)" %
                                  (ctx.sm_count, pk["sm_max_mhz"], pk["src"]),
