@@ -201,7 +201,7 @@ __global__ void __launch_bounds__(256) observe_rows_kernel(const ObsArgs a)
 }
 
 // ---- the lean kernel: the common case (16-byte aligned rows, n % 4 == 0, at most LT + 1 <= 125 taps incl. the
-// alignment padding, one float4 per thread and row).  Same data flow as above, but the instruction count per
+// alignment padding, at most four float4 per thread and row: rows up to 4096 pixels).  Same data flow as above, but the instruction count per
 // pixel is roughly halved: the taps arrive as a __grid_constant__ kernel parameter, so with the tap loop fully
 // unrolled every FFMA takes its weight straight from the constant bank and every LDS.128 of inputs has an
 // immediate offset (17 instructions per 16 FFMA instead of 26); and the bin geometry of the rebinning, which
@@ -209,7 +209,7 @@ __global__ void __launch_bounds__(256) observe_rows_kernel(const ObsArgs a)
 // weight of the first and of the last pixel) and kept in shared memory.
 struct ObsTaps { float wp[136]; };                       // wp[t + 3] = g(KO - t); zero outside the real taps
 
-template <int LT>                                        // LT >= L, multiple of 4: taps t = 0 .. LT
+template <int LT, int NV>                                // LT >= L, multiple of 4: taps t = 0 .. LT; NV float4 per thread
 __global__ void __launch_bounds__(256) observe_rows_lean_kernel(const ObsArgs a, const __grid_constant__ ObsTaps tp)
 {
     extern __shared__ __align__(16) float sm[];
@@ -222,19 +222,26 @@ __global__ void __launch_bounds__(256) observe_rows_lean_kernel(const ObsArgs a,
     if (a.rebin)
         for (int m = tid; m < a.nb; m += T) s_b[m] = a.bins[m];
 
-    const int p = 4 * tid;                               // this thread's pixels p .. p+3 (p < n by construction)
-    float4 reg = make_float4(0.f, 0.f, 0.f, 0.f);
+    float4 reg[NV];                                      // this thread's pixels 4 (tid + q T) .. + 3
     float hreg = 0.0f, nzr[OBS_NBR];
     auto fetch = [&](size_t row) {
         const float *src = a.flux + row * (size_t)n;
-        if (p < n) reg = __ldcs(reinterpret_cast<const float4 *>(src + p));
+#pragma unroll
+        for (int q = 0; q < NV; ++q) {
+            const int p = 4 * (tid + q * T);
+            reg[q] = p < n ? __ldcs(reinterpret_cast<const float4 *>(src + p)) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
         if (tid < a.L) hreg = __ldg(src + (tid < a.KO ? n - a.KO + tid : tid - a.KO));
     };
     size_t row = blockIdx.x;
     if (row < a.n_rows) fetch(row);
     for (; row < a.n_rows; row += gridDim.x) {
         __syncthreads();                                 // previous row's s_in / s_c consumed
-        if (p < n) *reinterpret_cast<float4 *>(s_in + a.KO + p) = reg;
+#pragma unroll
+        for (int q = 0; q < NV; ++q) {
+            const int p = 4 * (tid + q * T);
+            if (p < n) *reinterpret_cast<float4 *>(s_in + a.KO + p) = reg[q];
+        }
         if (tid < a.L) s_in[tid < a.KO ? tid : n + tid] = hreg;
         if (row + gridDim.x < a.n_rows) fetch(row + gridDim.x);
         if (a.noise) {
@@ -245,43 +252,54 @@ __global__ void __launch_bounds__(256) observe_rows_lean_kernel(const ObsArgs a,
             }
         }
         __syncthreads();
-        if (p < n) {
-            const float *si = s_in + p;
-            float acc0 = 0.f, acc1 = 0.f, acc2 = 0.f, acc3 = 0.f;
 #pragma unroll
-            for (int u = 0; u < LT + 4; u += 4) {        // input u and output r use wp[u - r + 3]
-                const float4 x = *reinterpret_cast<const float4 *>(si + u);
-                acc0 = fmaf(tp.wp[u + 3], x.x, acc0); acc0 = fmaf(tp.wp[u + 4], x.y, acc0); acc0 = fmaf(tp.wp[u + 5], x.z, acc0); acc0 = fmaf(tp.wp[u + 6], x.w, acc0);
-                acc1 = fmaf(tp.wp[u + 2], x.x, acc1); acc1 = fmaf(tp.wp[u + 3], x.y, acc1); acc1 = fmaf(tp.wp[u + 4], x.z, acc1); acc1 = fmaf(tp.wp[u + 5], x.w, acc1);
-                acc2 = fmaf(tp.wp[u + 1], x.x, acc2); acc2 = fmaf(tp.wp[u + 2], x.y, acc2); acc2 = fmaf(tp.wp[u + 3], x.z, acc2); acc2 = fmaf(tp.wp[u + 4], x.w, acc2);
-                acc3 = fmaf(tp.wp[u + 0], x.x, acc3); acc3 = fmaf(tp.wp[u + 1], x.y, acc3); acc3 = fmaf(tp.wp[u + 2], x.z, acc3); acc3 = fmaf(tp.wp[u + 3], x.w, acc3);
+        for (int q = 0; q < NV; ++q) {
+            const int p = 4 * (tid + q * T);
+            if (p < n) {
+                const float *si = s_in + p;
+                float acc0 = 0.f, acc1 = 0.f, acc2 = 0.f, acc3 = 0.f;
+#pragma unroll
+                for (int u = 0; u < LT + 4; u += 4) {    // input u and output r use wp[u - r + 3]
+                    const float4 x = *reinterpret_cast<const float4 *>(si + u);
+                    acc0 = fmaf(tp.wp[u + 3], x.x, acc0); acc0 = fmaf(tp.wp[u + 4], x.y, acc0); acc0 = fmaf(tp.wp[u + 5], x.z, acc0); acc0 = fmaf(tp.wp[u + 6], x.w, acc0);
+                    acc1 = fmaf(tp.wp[u + 2], x.x, acc1); acc1 = fmaf(tp.wp[u + 3], x.y, acc1); acc1 = fmaf(tp.wp[u + 4], x.z, acc1); acc1 = fmaf(tp.wp[u + 5], x.w, acc1);
+                    acc2 = fmaf(tp.wp[u + 1], x.x, acc2); acc2 = fmaf(tp.wp[u + 2], x.y, acc2); acc2 = fmaf(tp.wp[u + 3], x.z, acc2); acc2 = fmaf(tp.wp[u + 4], x.w, acc2);
+                    acc3 = fmaf(tp.wp[u + 0], x.x, acc3); acc3 = fmaf(tp.wp[u + 1], x.y, acc3); acc3 = fmaf(tp.wp[u + 2], x.z, acc3); acc3 = fmaf(tp.wp[u + 3], x.w, acc3);
+                }
+                *reinterpret_cast<float4 *>(s_c + p) = make_float4(acc0, acc1, acc2, acc3);
             }
-            *reinterpret_cast<float4 *>(s_c + p) = make_float4(acc0, acc1, acc2, acc3);
         }
         __syncthreads();
 
         float *dst = a.out + row * (size_t)a.nb;
-#pragma unroll
-        for (int k = 0; k < OBS_NBR; ++k) {              // nb <= OBS_NBR * T is a launch condition
-            const int m = tid + k * T;
-            if (m < a.nb) {
-                float v;
-                if (a.rebin) {
-                    const int4 e = s_b[m];
-                    if (e.y <= e.x) {
-                        v = __int_as_float(e.z) * s_c[e.x];                       // bin inside one pixel
-                    } else {                                                      // weights carry the 1/B
-                        float mid = 0.0f;
+        const float *nz = a.noise ? a.noise + row * (size_t)a.nb : nullptr;
+        int k = 0;
+        for (int m = tid; m < a.nb; m += T, ++k) {
+            float v;
+            if (a.rebin) {
+                const int4 e = s_b[m];
+                if (e.y <= e.x) {
+                    v = __int_as_float(e.z) * s_c[e.x];                           // bin inside one pixel
+                } else {                                                          // weights carry the 1/B
+                    float mid = 0.0f;
 #pragma unroll 1
-                        for (int i = e.x + 1; i < e.y; ++i) mid += s_c[i];
-                        v = fmaf(__int_as_float(e.w), s_c[e.y], fmaf(mid, a.inv_bin_f, __int_as_float(e.z) * s_c[e.x]));
-                    }
-                } else {
-                    v = s_c[m];
+                    for (int i = e.x + 1; i < e.y; ++i) mid += s_c[i];
+                    v = fmaf(__int_as_float(e.w), s_c[e.y], fmaf(mid, a.inv_bin_f, __int_as_float(e.z) * s_c[e.x]));
                 }
-                if (a.noise) v = fmaf(nzr[k], a.inv_snr, v);
-                __stcs(dst + m, v);
+            } else {
+                v = s_c[m];
             }
+            if (nz) {
+                float z = 0.0f;
+                if (k < OBS_NBR) {
+#pragma unroll
+                    for (int kk = 0; kk < OBS_NBR; ++kk) if (kk == k) z = nzr[kk];
+                } else {
+                    z = __ldcs(nz + m);
+                }
+                v = fmaf(z, a.inv_snr, v);
+            }
+            __stcs(dst + m, v);
         }
     }
 }
@@ -407,7 +425,8 @@ extern "C" lya_status lya_observe_rows(lya_ctx *ctx, size_t n_rows, int32_t n_pi
         a.taps = ctx->d_taps;
     }
     // ---- lean kernel for the common case
-    if (fast && a.L >= 0 && a.L <= 124 && a.n4 / 4 <= threads && nb <= OBS_NBR * threads) {
+    const int nv_lean = (a.n4 / 4 + threads - 1) / threads;
+    if (fast && a.L >= 0 && a.L <= 124 && nv_lean <= 4) {
         ObsTaps tp;
         memset(&tp, 0, sizeof(tp));
         for (int t = 0; t < a.L + 11; ++t) tp.wp[t] = ctx->h_taps[t];
@@ -442,7 +461,7 @@ extern "C" lya_status lya_observe_rows(lya_ctx *ctx, size_t n_rows, int32_t n_pi
         const int LT = a.L <= 64 ? ((a.L + 3) & ~3) : (a.L <= 96 ? 96 : 124);
         void (*lean)(const ObsArgs, const ObsTaps) = nullptr;
         switch (LT) {
-#define LYA_LEAN(N) case N: lean = observe_rows_lean_kernel<N>; break;
+#define LYA_LEAN(N) case N: lean = nv_lean == 1 ? observe_rows_lean_kernel<N, 1> : (nv_lean == 2 ? observe_rows_lean_kernel<N, 2> : observe_rows_lean_kernel<N, 4>); break;
             LYA_LEAN(0) LYA_LEAN(4) LYA_LEAN(8) LYA_LEAN(12) LYA_LEAN(16) LYA_LEAN(20) LYA_LEAN(24) LYA_LEAN(28)
             LYA_LEAN(32) LYA_LEAN(36) LYA_LEAN(40) LYA_LEAN(44) LYA_LEAN(48) LYA_LEAN(52) LYA_LEAN(56) LYA_LEAN(60)
             LYA_LEAN(64) LYA_LEAN(96) LYA_LEAN(124)
