@@ -108,3 +108,28 @@ def test_cfg5_slab_of_complete_rows(ctx, oracle):
                sightline_rows(tau, 0, ia, ib), sightline_rows(F, 0, ia, ib), A, "cfg5 slab")
     A_ref, _, _ = oracle.normalize_mean_flux(tau.cpu().numpy().astype(np.float64).ravel(), w.f_target)
     assert abs(A / A_ref - 1.0) < A_REL
+
+
+@pytest.mark.parametrize("n,rows,windowed", [(4096, 96, False), (4096, 96, True), (8192, 24, False), (12000, 10, False)])
+def test_long_sightlines(ctx, oracle, n, rows, windowed):
+    """The paper's own sightline length (4096 pixels of ~244 kpc) and beyond: groups of 8-16 warps
+    share a row whose staged cells fill most of an SM's shared memory."""
+    w = WORKLOADS[5]
+    rng = np.random.default_rng(n)
+    delta = torch.from_numpy(np.expm1(rng.normal(0, 1.3, (1, rows, n)) - 0.845).astype(np.float32)).cuda()
+    v = torch.from_numpy(rng.normal(0, 150.0, (1, rows, n)).astype(np.float32)).cuda()
+    p = lya.Params(nx=n, ny=rows, nz=1, box_mpch=w.box_mpch * n / w.n, z=w.z, T0=w.T0, gamma=w.gamma)
+    n_hi, b = ctx.gas_from_density(p, delta)
+    if windowed:
+        tau = ctx.tau_sightlines_opt(p, 0, v, n_hi=n_hi, b_kms=b, windowed=True)
+        assert torch.equal(tau, ctx.tau_sightlines(p, 0, n_hi, b, v))
+    else:
+        tau = ctx.tau_sightlines(p, 0, n_hi, b, v)
+    torch.cuda.synchronize()
+    po = oracle.Params(n_pix=n, box_mpch=p.box_mpch, z=w.z, T0=w.T0, gamma=w.gamma)
+    sel = [0, rows // 2, rows - 1]
+    _, n_ref, b_ref = oracle.gas_from_density(po, delta[0, sel].cpu().numpy())
+    ref = oracle.tau_rows(po, n_ref, b_ref, v[0, sel].cpu().numpy(), mode=1)
+    g = tau[0, sel].cpu().numpy().astype(np.float64)
+    big = ref > 1e-3
+    assert np.abs(g[big] / ref[big] - 1).max() <= TAU_REL and np.abs(g[~big] - ref[~big]).max() <= TAU_ABS
