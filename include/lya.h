@@ -115,10 +115,12 @@ lya_status lya_tau_sightlines_opt(lya_ctx *ctx, const lya_params *p, int axis, i
                                   float *tau, uint64_t *pairs_evaluated);
 
 /* S4.  tau: DEVICE, n_pix floats in any layout (the mean runs over all of them).  Finds the unique A > 0
- * with mean(exp(-A tau)) = f_target by a bracketed Newton/bisection iteration that runs entirely on the
- * device (one cooperative kernel); synchronises the stream because A returns to the HOST.
- * rel_tol: stop when the step or the bracket is below rel_tol * A (suggest 1e-7); max_iter passes over tau
- * (suggest 60).  a_out, f_achieved, iters: HOST, any may be NULL. */
+ * with mean(exp(-A tau)) = f_target by an iteration that runs entirely on the device (one cooperative
+ * kernel): every pass over tau yields five tilted moments and a fifth-order step on ln <exp(-A tau)>,
+ * safeguarded by Newton's step and a bisection bracket (3-5 passes).  Synchronises the
+ * stream because A returns to the HOST.  rel_tol: stop when the step, or the truncation error of the step's
+ * model, is below rel_tol * A (suggest 1e-7); max_iter passes over tau (suggest 60).  a_out, f_achieved (the
+ * mean flux at A), iters (passes used): HOST, any may be NULL. */
 lya_status lya_normalize_mean_flux(lya_ctx *ctx, const float *tau, size_t n_pix, double f_target,
                                    double rel_tol, int max_iter,
                                    double *a_out, double *f_achieved, int *iters);

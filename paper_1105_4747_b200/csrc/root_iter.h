@@ -4,9 +4,10 @@
 // f(A) = mean_p exp(-A tau_p) is strictly decreasing for tau >= 0 and g(A) = ln f(A) (a cumulant generating
 // function) is decreasing and CONVEX, so Newton's iteration on g(A) = ln f_target started at A = 0 climbs
 // monotonically to the unique root -- and, g being exactly linear when all tau are equal, in far fewer steps
-// than Newton on f itself (4-5 passes instead of 7-8 on the lognormal test fields).  A bracket [lo, hi] is
-// kept from the sign of f - f_target and any step that leaves it is replaced by the midpoint (bisection),
-// which makes the loop safe against rounding in f.  One pass over tau gives both sums f and -f' for the trial.
+// than Newton on f itself (7-8 passes on the lognormal test fields; lya_root_step_moments below needs 3-4).
+// A bracket [lo, hi] is kept from the sign of f - f_target and any step that leaves it is replaced by the
+// midpoint (bisection), which makes the loop safe against rounding in f.  One pass over tau gives both sums f
+// and -f' for the trial.
 #pragma once
 #include <math.h>
 
