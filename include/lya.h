@@ -12,8 +12,9 @@
  *
  * Every entry point is extern "C", takes plain pointers and sizes, returns a status code and never
  * throws, exits or prints.  Pointers are marked DEVICE (CUDA global memory of ctx's device, owned by
- * the caller, fp32, 4-byte aligned at least; 16-byte alignment enables the vector / bulk-copy paths)
- * or HOST.  The library never retains or frees a caller pointer; its only allocations are private
+ * the caller, fp32, 4-byte aligned at least; 16-byte alignment enables the vector paths; the pointers of
+ * an EMPTY array -- n_cells, n_pix or n_rows == 0 -- may be NULL: such calls return LYA_OK without a launch,
+ * except lya_normalize_mean_flux, for which the mean of nothing is LYA_EINVAL) or HOST.  The library never retains or frees a caller pointer; its only allocations are private
  * scratch inside lya_ctx.  There is no CPU fallback: without a CUDA device lya_create fails with
  * LYA_ECUDA and nothing else can be called.
  *

@@ -130,12 +130,12 @@ lya_status lya_gas_from_density(lya_ctx *ctx, const lya_params *p, const float *
     if (!ctx) return LYA_EINVAL;
     ctx->err[0] = 0;
     if (!params_ok(p)) return lya_fail(ctx, LYA_EINVAL, "lya_gas_from_density: bad parameters");
+    if (n_cells == 0) return LYA_OK;                 // nothing to do; pointers of empty arrays may be NULL
     if (!delta || !n_hi || !b_kms) return lya_fail(ctx, LYA_EINVAL, "lya_gas_from_density: null pointer");
     if ((((uintptr_t)delta | (uintptr_t)n_hi | (uintptr_t)b_kms) & 3) != 0)
         return lya_fail(ctx, LYA_EINVAL, "lya_gas_from_density: pointers must be 4-byte aligned");
     if (n_hi == delta || b_kms == delta || n_hi == b_kms)
         return lya_fail(ctx, LYA_EINVAL, "lya_gas_from_density: outputs may not alias");
-    if (n_cells == 0) return LYA_OK;
     lya_scalars s;
     lya_scalars_from_params(p, 0, &s);          // nbarHI and b0 do not depend on the axis
     LYA_CUDA(ctx, cudaSetDevice(ctx->device));
@@ -198,8 +198,8 @@ lya_status lya_normalize_mean_flux(lya_ctx *ctx, const float *tau, size_t n_pix,
 {
     if (!ctx) return LYA_EINVAL;
     ctx->err[0] = 0;
-    if (!tau || ((uintptr_t)tau & 3)) return lya_fail(ctx, LYA_EINVAL, "lya_normalize_mean_flux: bad tau pointer");
     if (n_pix == 0) return lya_fail(ctx, LYA_EINVAL, "lya_normalize_mean_flux: n_pix == 0");
+    if (!tau || ((uintptr_t)tau & 3)) return lya_fail(ctx, LYA_EINVAL, "lya_normalize_mean_flux: bad tau pointer");
     if (!(f_target > 0.0 && f_target < 1.0))
         return lya_fail(ctx, LYA_EINVAL, "lya_normalize_mean_flux: f_target must lie in (0,1)");
     if (!(rel_tol > 0.0) || max_iter < 2)
@@ -213,7 +213,7 @@ lya_status lya_flux_partial_sums(lya_ctx *ctx, const float *tau, size_t n_pix, c
 {
     if (!ctx) return LYA_EINVAL;
     ctx->err[0] = 0;
-    if (!tau || ((uintptr_t)tau & 3) || !a_trial || !sums)
+    if ((n_pix > 0 && (!tau || ((uintptr_t)tau & 3))) || !a_trial || !sums)
         return lya_fail(ctx, LYA_EINVAL, "lya_flux_partial_sums: null or misaligned pointer");
     if (k < 1 || k > LYA_MAX_TRIALS) return lya_fail(ctx, LYA_EINVAL, "lya_flux_partial_sums: k must be 1..8");
     for (int i = 0; i < k; ++i)
@@ -238,7 +238,7 @@ lya_status lya_flux_moment_sums(lya_ctx *ctx, const float *tau, size_t n_pix, do
 {
     if (!ctx) return LYA_EINVAL;
     ctx->err[0] = 0;
-    if (!tau || ((uintptr_t)tau & 3) || !sums5) return lya_fail(ctx, LYA_EINVAL, "lya_flux_moment_sums: null or misaligned pointer");
+    if ((n_pix > 0 && (!tau || ((uintptr_t)tau & 3))) || !sums5) return lya_fail(ctx, LYA_EINVAL, "lya_flux_moment_sums: null or misaligned pointer");
     if (!(a_trial >= 0.0) || !(a_trial < 1.0e30)) return lya_fail(ctx, LYA_EINVAL, "lya_flux_moment_sums: trial A must be finite and >= 0");
     if (n_pix == 0) { for (int i = 0; i < 5; ++i) sums5[i] = 0.0; return LYA_OK; }
     LYA_CUDA(ctx, cudaSetDevice(ctx->device));
@@ -263,7 +263,7 @@ lya_status lya_flux(lya_ctx *ctx, const float *tau, size_t n_pix, double a, floa
 {
     if (!ctx) return LYA_EINVAL;
     ctx->err[0] = 0;
-    if (!tau || !flux || (((uintptr_t)tau | (uintptr_t)flux) & 3))
+    if (n_pix > 0 && (!tau || !flux || (((uintptr_t)tau | (uintptr_t)flux) & 3)))
         return lya_fail(ctx, LYA_EINVAL, "lya_flux: null or misaligned pointer");
     if (!(a >= 0.0) || !(a < 1.0e30)) return lya_fail(ctx, LYA_EINVAL, "lya_flux: A must be finite and >= 0");
     if (n_pix == 0) return LYA_OK;

@@ -366,11 +366,11 @@ extern "C" lya_status lya_observe_rows(lya_ctx *ctx, size_t n_rows, int32_t n_pi
 {
     if (!ctx) return LYA_EINVAL;
     ctx->err[0] = 0;
-    if (!inst || !flux || !out) return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: null pointer");
+    if (!inst || (n_rows > 0 && (!flux || !out))) return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: null pointer");
     if (n_pix < 1 || !(dv_kms > 0.0)) return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: n_pix >= 1 and dv > 0 required");
     if ((((uintptr_t)flux | (uintptr_t)out | (uintptr_t)unit_noise) & 3) != 0)
         return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: pointers must be 4-byte aligned");
-    if (out == flux) return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: out may not alias flux");
+    if (n_rows > 0 && out == flux) return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: out may not alias flux");
     if (inst->snr > 0.0 && !unit_noise) return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: snr > 0 needs unit_noise");
     const int32_t nb = lya_instrument_bins(n_pix, dv_kms, inst);
     if (nb < 1) return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: bin wider than the row");
@@ -509,7 +509,7 @@ extern "C" lya_status lya_flux_pdf(lya_ctx *ctx, const float *flux, size_t n, in
 {
     if (!ctx) return LYA_EINVAL;
     ctx->err[0] = 0;
-    if (!flux || ((uintptr_t)flux & 3)) return lya_fail(ctx, LYA_EINVAL, "lya_flux_pdf: bad flux pointer");
+    if (n > 0 && (!flux || ((uintptr_t)flux & 3))) return lya_fail(ctx, LYA_EINVAL, "lya_flux_pdf: bad flux pointer");
     if (n_bins < 1 || n_bins > 256 || !(width > 0.0)) return lya_fail(ctx, LYA_EINVAL, "lya_flux_pdf: 1 <= n_bins <= 256 and width > 0 required");
     LYA_CUDA(ctx, cudaSetDevice(ctx->device));
     unsigned long long *d_counts = reinterpret_cast<unsigned long long *>(ctx->d_stats);

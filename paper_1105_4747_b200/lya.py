@@ -158,10 +158,10 @@ def scalars(p: Params, axis: int = 0) -> dict:
     return {k: getattr(s, k) for k, _ in CScalars._fields_}
 
 
-def _dev(t: torch.Tensor, name: str) -> int:
+def _dev(t: torch.Tensor, name: str):
     if not (t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
         raise TypeError(f"{name}: contiguous float32 CUDA tensor required")
-    return t.data_ptr()
+    return t.data_ptr() or None                          # an empty tensor has no storage: NULL
 
 
 def _host(t: torch.Tensor | None, name: str):

@@ -320,3 +320,36 @@ def test_tau_windowed_falls_back_when_the_reach_does_not_fit(ctx):
         lya.lib().lya_tau_sightlines_opt  # noqa: B018  (symbol exists)
         ctx._check(lya.lib().lya_tau_sightlines_opt(ctx._h, lya.C.byref(p.c()), 0, 4, 8, n_hi.data_ptr(),
                                                     b.data_ptr(), v.data_ptr(), full.data_ptr(), None))
+
+
+# ------------------------------------------------------------------ empty inputs and size limits
+def test_empty_inputs_and_size_limits(ctx):
+    p = lya.Params(nx=64, ny=4, nz=1, box_mpch=20.0, z=2.5, T0=1e4, gamma=1.5)
+    empty = torch.empty((0,), device="cuda")
+    n_hi, b = ctx.gas_from_density(p, empty)                        # zero cells: nothing launched, no error
+    assert n_hi.numel() == 0 and b.numel() == 0
+    assert ctx.flux(empty, 0.5).numel() == 0
+    s, d = ctx.flux_partial_sums(empty, [0.3, 0.6])
+    assert s == [0.0, 0.0] and d == [0.0, 0.0]
+    assert ctx.flux_moment_sums(empty, 0.3) == [0.0] * 5
+    counts, pdf = ctx.flux_pdf(empty)
+    assert counts.sum() == 0 and not pdf.any()
+    with pytest.raises(lya.LyaError) as e:
+        ctx.normalize_mean_flux(empty, 0.8)                         # the mean of nothing is undefined
+    assert e.value.status == lya.EINVAL
+    assert ctx.observe_rows(torch.empty((0, 64), device="cuda"), 5.0, 10.0).shape == (0, 64)
+    # a sightline whose staged cells (16 B each) exceed one SM's shared memory is refused, not mis-computed
+    n = 20000
+    big = lya.Params(nx=n, ny=1, nz=1, box_mpch=2000.0, z=2.5, T0=1e4, gamma=1.5)
+    x = torch.ones((1, 1, n), device="cuda")
+    for axis_p, arr in ((big, x),):
+        with pytest.raises(lya.LyaError) as e:
+            ctx.tau_sightlines(axis_p, 0, arr, arr, arr)
+        assert e.value.status == lya.EINVAL and "shared memory" in str(e.value)
+    # the longest row that does fit (14 000 pixels: 224 KB of cells) still runs and gives the uniform-field value
+    n = 14000
+    ok = lya.Params(nx=n, ny=2, nz=1, box_mpch=1500.0, z=2.5, T0=1e4, gamma=1.5)
+    n_hi, b = ctx.gas_from_density(ok, torch.zeros((1, 2, n), device="cuda"))
+    tau = ctx.tau_sightlines(ok, 0, n_hi, b, torch.zeros((1, 2, n), device="cuda"))
+    torch.cuda.synchronize()
+    assert torch.allclose(tau, tau[0, 0, 0].expand_as(tau), rtol=1e-6) and tau[0, 0, 0].item() > 0
