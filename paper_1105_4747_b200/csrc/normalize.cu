@@ -19,6 +19,9 @@ namespace cg = cooperative_groups;
 namespace {
 
 constexpr int RED_THREADS = 256;
+constexpr int NORM_THREADS = 1024;   // normalize_kernel: ONE CTA per SM -- every CTA re-reads all per-CTA partials after
+                                     // the grid barrier, and with 592 CTAs of 256 that gather (all CTAs hitting the same
+                                     // L2 lines) cost 6-9 us per pass and the barrier 7-13 us; with 148 CTAs both are ~1 us
 constexpr double LOG2E_D  = 1.4426950408889634074;
 
 __device__ __forceinline__ float ex2_ftz(float x)
@@ -166,11 +169,11 @@ struct NormArgs {
     size_t       n;
     double       f_target, rel_tol;
     int          max_iter;
-    double      *partials;     // [2][gridDim.x][5]
+    double      *partials;     // [2][gridDim.x][5], gridDim.x <= SM count
     double      *result;       // [0] A, [1] <F> at A, [2] passes, [3] status
 };
 
-__global__ void __launch_bounds__(RED_THREADS, 4) normalize_kernel(const NormArgs a)
+__global__ void __launch_bounds__(NORM_THREADS, 1) normalize_kernel(const NormArgs a)
 {
     cg::grid_group grid = cg::this_grid();
     __shared__ double sh[5 * 32];
@@ -295,12 +298,14 @@ lya_status lya_run_normalize(lya_ctx *ctx, const float *tau, size_t n, double f_
 {
     if (!ctx->coop_ok) return lya_fail(ctx, LYA_ECUDA, "device does not support cooperative launch");
     int per_sm = 0;
-    LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, normalize_kernel, RED_THREADS, 0));
+    LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, normalize_kernel, NORM_THREADS, 0));
     if (per_sm < 1) return lya_fail(ctx, LYA_ECUDA, "normalize_kernel: zero occupancy");
     NormArgs a{tau, n, f_target, rel_tol, max_iter, ctx->d_partials, ctx->d_root};
-    int grid = red_grid(ctx, n, per_sm);
+    size_t want = (n / 4 + NORM_THREADS - 1) / NORM_THREADS;           // at least one float4 per thread
+    if (want < 1) want = 1;
+    const int grid = (int)(want < (size_t)ctx->sm_count ? want : (size_t)ctx->sm_count);
     void *args[] = {(void *)&a};
-    LYA_CUDA(ctx, cudaLaunchCooperativeKernel((void *)normalize_kernel, dim3(grid), dim3(RED_THREADS), args, 0,
+    LYA_CUDA(ctx, cudaLaunchCooperativeKernel((void *)normalize_kernel, dim3(grid), dim3(NORM_THREADS), args, 0,
                                               ctx->stream));
     ctx->launches++;
     LYA_CUDA(ctx, cudaMemcpyAsync(ctx->h_pinned, ctx->d_root, 4 * sizeof(double), cudaMemcpyDeviceToHost,
