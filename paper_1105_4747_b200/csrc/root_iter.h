@@ -106,7 +106,6 @@ LYA_HD void lya_root_step_moments(lya_root_state *s, const double *S)
     if (s->a > 0.0) { if (f > s->f_target) s->lo = s->a; else s->hi = s->a; }
     const double h_newton = t / k1;
     const double h4 = lya_poly_root(t, k1, k2, k3, k4, h_newton);
-    const double h3 = lya_poly_root(t, k1, k2, k3, 0.0, h_newton);
     double a_new = s->a + h4;
     const double ratio = h4 / h_newton;
     // by convexity of ln f the Newton step undershoots from the left (t > 0) and overshoots from the right
@@ -120,9 +119,14 @@ LYA_HD void lya_root_step_moments(lya_root_state *s, const double *S)
         lya_root_step(s, S[0], S[1]);
         return;
     }
-    double trunc = h4 - h3;
-    if (trunc < 0.0) trunc = -trunc;
     s->a = a_new;
+    // truncation estimate = |quartic root - cubic root|; a step above 5 % of A cannot pass it, so the cubic
+    // solve (a dozen double divisions on one thread) is skipped there
+    double trunc = 1.0e300;
+    if ((h4 < 0.0 ? -h4 : h4) <= 0.05 * a_new) {
+        trunc = h4 - lya_poly_root(t, k1, k2, k3, 0.0, h4);
+        if (trunc < 0.0) trunc = -trunc;
+    }
     if (trunc <= 0.1 * s->rel_tol * a_new) {           // model converged: stop here, report the model's f(a_new)
         const double h = h4;
         s->f_at_a = f * exp(h * (-k1 + h * (0.5 * k2 + h * (-k3 / 6.0 + h * (k4 / 24.0)))));
