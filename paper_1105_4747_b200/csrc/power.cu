@@ -65,11 +65,14 @@ template <int R> __device__ __forceinline__ constexpr int bitrev(int t)
 //   v[t] = in[j + t N/R] ;  v[t] *= exp(-2 pi i t k / (ns R)), k = j mod ns ;  V = DFT_R(v) ;
 //   out[(j - k) R + k + t ns] = V[t]
 // FIRST: `in` is global memory (two rows -> one complex sequence, dF = F inv_mean - 1).
-template <int R, bool FIRST>
+// N_CT / NS_CT > 0: row length and ns known at compile time (the common sizes), which turns every shared-memory
+// offset below into an immediate; 0: taken from the arguments.
+template <int R, bool FIRST, int N_CT = 0, int NS_CT = 0>
 __device__ __forceinline__ void stockham_pass(const PowArgs &a, const float *ra, const float *rb, bool has_b,
-                                              const float2 *in, float2 *out, const float2 *tw, int ns)
+                                              const float2 *in, float2 *out, const float2 *tw, int ns_rt)
 {
-    const int n = a.n, m = n / R;
+    const int n = N_CT > 0 ? N_CT : a.n, m = n / R;
+    const int ns = NS_CT > 0 ? NS_CT : ns_rt;
     // padded addresses are affine in t: pad16(j + t m) = pad16(j) + t (m + m/16) for m >= 16, and
     // pad16(j0 + t ns) = pad16(j0) + t os_a + (t >> 1) os_b with (os_a, os_b) = (ns + ns/16, 0) for ns >= 16,
     // (8, 1) for ns == 8 (j0 mod 16 < 8 there), (1, 0) for ns == 1 (j0 = j R)
@@ -115,10 +118,18 @@ __device__ __forceinline__ void stockham_pass(const PowArgs &a, const float *ra,
     }
 }
 
+// radix of pass i for the sizes with a compile-time plan (0: no such pass)
+__host__ __device__ constexpr int plan_radix(int n, int i)
+{
+    return n == 256 ? (i < 2 ? 16 : 0) : n == 512 ? (i < 3 ? 8 : 0) : n == 1024 ? (i == 0 ? 16 : (i < 3 ? 8 : 0))
+         : n == 2048 ? (i < 2 ? 16 : (i == 2 ? 8 : 0)) : n == 4096 ? (i < 3 ? 16 : 0) : 0;
+}
+
+template <int N_CT>
 __global__ void __launch_bounds__(256) flux_power_kernel(const PowArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int n = a.n, nh = n >> 1, npad = n + (n >> 4) + 1;
+    const int n = N_CT > 0 ? N_CT : a.n, nh = n >> 1, npad = n + (n >> 4) + 1;
     double *pw  = reinterpret_cast<double *>(smem_raw);                    // [nh + 1] (+1 pad)
     float2 *bufA = reinterpret_cast<float2 *>(pw + nh + 2);                // [npad]
     float2 *bufB = bufA + npad;                                            // [npad]
@@ -139,22 +150,39 @@ __global__ void __launch_bounds__(256) flux_power_kernel(const PowArgs a)
         const float *rb = ra + n;
         __syncthreads();                                   // previous pair's read-out done (and tables built)
         float2 *src = bufB, *dst = bufA;
-        int ns = 1;
-#pragma unroll 1
-        for (int ps = 0; ps < a.n_pass; ++ps) {
-            const int R = ps == 0 ? a.radix[0] : (ps == 1 ? a.radix[1] : (ps == 2 ? a.radix[2] : a.radix[3]));
-            if (ps == 0) {
-                if (R == 16)     stockham_pass<16, true>(a, ra, rb, has_b, nullptr, dst, tw, 1);
-                else if (R == 8) stockham_pass<8, true>(a, ra, rb, has_b, nullptr, dst, tw, 1);
-                else             stockham_pass<4, true>(a, ra, rb, has_b, nullptr, dst, tw, 1);
-            } else {
-                if (R == 16)     stockham_pass<16, false>(a, ra, rb, has_b, src, dst, tw, ns);
-                else if (R == 8) stockham_pass<8, false>(a, ra, rb, has_b, src, dst, tw, ns);
-                else             stockham_pass<4, false>(a, ra, rb, has_b, src, dst, tw, ns);
-            }
-            ns *= R;
-            float2 *tmp = src; src = dst; dst = tmp;       // src now holds the newest data
+        if constexpr (N_CT > 0) {                          // compile-time plan: immediates everywhere
+            constexpr int R0 = plan_radix(N_CT, 0), R1 = plan_radix(N_CT, 1), R2 = plan_radix(N_CT, 2);
+            stockham_pass<R0, true, N_CT, 1>(a, ra, rb, has_b, nullptr, bufA, tw, 1);
             __syncthreads();
+            src = bufA;
+            if constexpr (R1 > 0) {
+                stockham_pass<R1, false, N_CT, R0>(a, ra, rb, has_b, bufA, bufB, tw, R0);
+                __syncthreads();
+                src = bufB;
+            }
+            if constexpr (R2 > 0) {
+                stockham_pass<R2, false, N_CT, R0 * R1>(a, ra, rb, has_b, bufB, bufA, tw, R0 * R1);
+                __syncthreads();
+                src = bufA;
+            }
+        } else {
+            int ns = 1;
+#pragma unroll 1
+            for (int ps = 0; ps < a.n_pass; ++ps) {
+                const int R = ps == 0 ? a.radix[0] : (ps == 1 ? a.radix[1] : (ps == 2 ? a.radix[2] : a.radix[3]));
+                if (ps == 0) {
+                    if (R == 16)     stockham_pass<16, true>(a, ra, rb, has_b, nullptr, dst, tw, 1);
+                    else if (R == 8) stockham_pass<8, true>(a, ra, rb, has_b, nullptr, dst, tw, 1);
+                    else             stockham_pass<4, true>(a, ra, rb, has_b, nullptr, dst, tw, 1);
+                } else {
+                    if (R == 16)     stockham_pass<16, false>(a, ra, rb, has_b, src, dst, tw, ns);
+                    else if (R == 8) stockham_pass<8, false>(a, ra, rb, has_b, src, dst, tw, ns);
+                    else             stockham_pass<4, false>(a, ra, rb, has_b, src, dst, tw, ns);
+                }
+                ns *= R;
+                float2 *tmp = src; src = dst; dst = tmp;   // src now holds the newest data
+                __syncthreads();
+            }
         }
         const float2 *z = src;
         for (int m = tid; m <= nh; m += T) {
@@ -199,12 +227,15 @@ extern "C" lya_status lya_flux_power_rows(lya_ctx *ctx, size_t n_rows, int32_t n
     const size_t smem = (size_t)(nk + 1) * sizeof(double) + 2 * (size_t)npad * sizeof(float2) + (size_t)(n_pix / 2) * sizeof(float2);
     int threads = n_pix / 8;
     threads = threads < 32 ? 32 : (threads > 256 ? 256 : threads);
-    LYA_CUDA(ctx, cudaFuncSetAttribute(flux_power_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    void (*kern)(const PowArgs) = n_pix == 256 ? flux_power_kernel<256> : n_pix == 512 ? flux_power_kernel<512>
+                                : n_pix == 1024 ? flux_power_kernel<1024> : n_pix == 2048 ? flux_power_kernel<2048>
+                                : n_pix == 4096 ? flux_power_kernel<4096> : flux_power_kernel<0>;
+    LYA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
-    LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, flux_power_kernel, threads, smem));
+    LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
     if (per_sm < 1) return lya_fail(ctx, LYA_ECUDA, "flux_power_kernel: zero occupancy");
     const size_t n_pairs = (n_rows + 1) / 2, cap = (size_t)ctx->sm_count * per_sm;
-    flux_power_kernel<<<(int)(n_pairs < cap ? n_pairs : cap), threads, smem, ctx->stream>>>(a);
+    kern<<<(int)(n_pairs < cap ? n_pairs : cap), threads, smem, ctx->stream>>>(a);
     ctx->launches++;
     LYA_CUDA(ctx, cudaGetLastError());
     LYA_CUDA(ctx, cudaMemcpyAsync(power, ctx->d_stats, (size_t)nk * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
