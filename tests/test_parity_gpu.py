@@ -353,3 +353,21 @@ def test_empty_inputs_and_size_limits(ctx):
     tau = ctx.tau_sightlines(ok, 0, n_hi, b, torch.zeros((1, 2, n), device="cuda"))
     torch.cuda.synchronize()
     assert torch.allclose(tau, tau[0, 0, 0].expand_as(tau), rtol=1e-6) and tau[0, 0, 0].item() > 0
+
+
+def test_nan_in_one_sightline_stays_in_that_sightline(ctx):
+    """The per-cell content is not scanned (lya.h): a NaN density or velocity poisons its own sightline only."""
+    w = scaled(WORKLOADS[2], 256)
+    f = inputs.make_fields(w, device="cuda", z0=0, z1=2)
+    delta, v = f["delta"].clone(), f["v_pec"][0].clone()
+    p = lya.Params(nx=256, ny=256, nz=2, box_mpch=w.box_mpch, z=w.z, T0=w.T0, gamma=w.gamma)
+    n_hi, b = ctx.gas_from_density(p, delta)
+    good = ctx.tau_sightlines(p, 0, n_hi, b, v)
+    delta[0, 7, 100] = float("nan")
+    v[1, 200, 3] = float("nan")
+    n_hi, b = ctx.gas_from_density(p, delta)
+    for kw in (dict(), dict(windowed=True)):
+        tau = ctx.tau_sightlines_opt(p, 0, v, n_hi=n_hi, b_kms=b, **kw)
+        bad = torch.isnan(tau).any(dim=2)
+        assert bad[0, 7] and bad[1, 200] and int(bad.sum()) == 2
+        assert torch.equal(tau[~bad], good[~bad])
