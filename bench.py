@@ -7,7 +7,7 @@ A step is one pass of the whole hot path over one synthetic grid.  Default workl
 configs[1] (256^3, 65,536 sightlines x 256 px, fp32).  `value` = tau pixel-pair evaluations per second
 over the whole step, inputs resident in HBM; `e2e` = the same through lya_forest_host with pinned HOST buffers
 (H2D of delta and v_pec, D2H of F inside the timed region).  N > 1 (torchrun): every rank owns a z-slab of
-256 planes of an N*256-plane grid (weak scaling); the only exchange is S4's all-reduce of two doubles per pass.
+256 planes of an N*256-plane grid (weak scaling); the only exchange is S4's all-reduce of five doubles per pass.
 `--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
 """
 from __future__ import annotations
@@ -339,7 +339,7 @@ def bench_ours(args) -> dict:
                    "pixels_per_sightline": n, "axes": list(w.axes), "f_target": w.f_target, "slab_nz": slab_nz,
                    "l2": "256 MiB memset between steps (outside the event spans); working set %d MiB" %
                          (6 * 4 * n_cells >> 20),
-                   "parallelism": "z-slabs per rank; S4 all-reduce of 2 doubles per pass" if world > 1 else "1 GPU"},
+                   "parallelism": "z-slabs per rank; S4 all-reduce of 5 doubles per pass" if world > 1 else "1 GPU"},
         "sightline_pixels_per_s": pix_per_step / (ms_per_step * 1e-3),
         "tau_kernel_pixels_per_s": float(slab_cells) / (k_ms["tau"] * 1e-3),
         "A": results["A"], "mean_flux": results["f"], "normalize_passes": passes,
