@@ -29,7 +29,8 @@ struct ObsArgs {
     unsigned long long bin_fx;            // B = bin / dv [pixels] in 32.32 fixed point
     float        inv_bin_f;               // 1 / B
     float        inv_snr;                 // 0: no noise
-    const int4  *bins;                    // lean kernel: per output bin {i0, i1, bits(w_first), bits(w_last)}
+    const int4  *bins;                    // lean kernel: per output bin {i0, i1, bits(w_first), bits(w_last)}, or
+    int          bins3;                   // (bins3, bins <= 2 pixels wide) {i0, bits(w0), bits(w1), bits(w2)}
 };
 
 // A CTA works on batches of D rows.  NV = float4 loads per thread and row (n4 <= 4 * NV * blockDim.x).  The
@@ -216,9 +217,10 @@ __global__ void __launch_bounds__(256) observe_rows_lean_kernel(const ObsArgs a,
     const int n = a.n, T = blockDim.x, tid = threadIdx.x;
     const int in_len = n + LT + 8;
     float *s_in = sm;                                    // s_in[h] = F[(h - KO) mod n], zero beyond n + L
-    float *s_c  = sm + in_len;                           // convolved row, n floats
-    int4  *s_b  = reinterpret_cast<int4 *>(s_c + n);     // bin table, nb entries (rebin only)
+    float *s_c  = sm + in_len;                           // convolved row, n floats (+ 4 zeros for the 3-tap rebin)
+    int4  *s_b  = reinterpret_cast<int4 *>(s_c + n + 4); // bin table, nb entries (rebin only)
     for (int h = tid; h < in_len; h += T) s_in[h] = 0.0f;
+    if (tid < 4) s_c[n + tid] = 0.0f;
     if (a.rebin)
         for (int m = tid; m < a.nb; m += T) s_b[m] = a.bins[m];
 
@@ -276,7 +278,11 @@ __global__ void __launch_bounds__(256) observe_rows_lean_kernel(const ObsArgs a,
         int k = 0;
         for (int m = tid; m < a.nb; m += T, ++k) {
             float v;
-            if (a.rebin) {
+            if (a.bins3) {                                                        // bins <= 2 pixels wide: at most three
+                const int4 e = s_b[m];                                            // pixels overlap -> {i0, w0, w1, w2}
+                v = fmaf(__int_as_float(e.w), s_c[e.x + 2],
+                         fmaf(__int_as_float(e.z), s_c[e.x + 1], __int_as_float(e.y) * s_c[e.x]));
+            } else if (a.rebin) {
                 const int4 e = s_b[m];
                 if (e.y <= e.x) {
                     v = __int_as_float(e.z) * s_c[e.x];                           // bin inside one pixel
@@ -442,16 +448,28 @@ extern "C" lya_status lya_observe_rows(lya_ctx *ctx, size_t n_rows, int32_t n_pi
             }
             LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));             // previous call may still read h_bins
             int4 *hb = (int4 *)ctx->h_bins;
+            a.bins3 = bin_px <= 2.0;
             for (int m = 0; m < nb; ++m) {                                  // bin [lo, hi) in pixel units (reading O2)
                 const double lo = (double)m * bin_px, hi = lo + bin_px;
                 int i0 = (int)floor(lo), i1 = (int)ceil(hi) - 1;
                 if (i1 > n_pix - 1) i1 = n_pix - 1;
-                float wf, wl;
-                if (i1 <= i0) { i1 = i0; wf = (float)((hi - lo) / bin_px); wl = 0.0f; }
-                else { wf = (float)(((double)(i0 + 1) - lo) / bin_px); wl = (float)((hi - (double)i1) / bin_px); }
                 int4 e;
-                e.x = i0; e.y = i1;
-                memcpy(&e.z, &wf, 4); memcpy(&e.w, &wl, 4);
+                if (a.bins3) {                                              // overlap of the bin with pixels i0, i0+1, i0+2
+                    float wq[3];
+                    for (int q = 0; q < 3; ++q) {
+                        const double l = lo > (double)(i0 + q) ? lo : (double)(i0 + q);
+                        const double h = hi < (double)(i0 + q + 1) ? hi : (double)(i0 + q + 1);
+                        wq[q] = (h > l && i0 + q < n_pix) ? (float)((h - l) / bin_px) : 0.0f;
+                    }
+                    e.x = i0;
+                    memcpy(&e.y, &wq[0], 4); memcpy(&e.z, &wq[1], 4); memcpy(&e.w, &wq[2], 4);
+                } else {
+                    float wf, wl;
+                    if (i1 <= i0) { i1 = i0; wf = (float)((hi - lo) / bin_px); wl = 0.0f; }
+                    else { wf = (float)(((double)(i0 + 1) - lo) / bin_px); wl = (float)((hi - (double)i1) / bin_px); }
+                    e.x = i0; e.y = i1;
+                    memcpy(&e.z, &wf, 4); memcpy(&e.w, &wl, 4);
+                }
                 hb[m] = e;
             }
             LYA_CUDA(ctx, cudaMemcpyAsync(ctx->d_bins, hb, (size_t)nb * sizeof(int4), cudaMemcpyHostToDevice, ctx->stream));
@@ -467,7 +485,7 @@ extern "C" lya_status lya_observe_rows(lya_ctx *ctx, size_t n_rows, int32_t n_pi
             LYA_LEAN(64) LYA_LEAN(96) LYA_LEAN(124)
 #undef LYA_LEAN
         }
-        const size_t smem_l = ((size_t)n_pix + LT + 8 + n_pix) * sizeof(float) + (a.rebin ? (size_t)nb * sizeof(int4) : 0);
+        const size_t smem_l = ((size_t)n_pix + LT + 8 + n_pix + 4) * sizeof(float) + (a.rebin ? (size_t)nb * sizeof(int4) : 0);
         LYA_CUDA(ctx, cudaFuncSetAttribute(lean, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_l));
         int per_sm_l = 0;
         LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_l, lean, threads, smem_l));
