@@ -227,6 +227,20 @@ lya_status lya_flux_partial_sums(lya_ctx *ctx, const float *tau, size_t n_pix, c
     return lya_run_partial_sums(ctx, tau, n_pix, a_trial, k, sums, dsums);
 }
 
+lya_status lya_flux_with_pdf(lya_ctx *ctx, const float *tau, size_t n_pix, double a, float *flux, int32_t n_bins,
+                             double f_lo, double width, uint64_t *counts, double *pdf)
+{
+    if (!ctx) return LYA_EINVAL;
+    ctx->err[0] = 0;
+    if (n_pix > 0 && (!tau || !flux || (((uintptr_t)tau | (uintptr_t)flux) & 3)))
+        return lya_fail(ctx, LYA_EINVAL, "lya_flux_with_pdf: null or misaligned pointer");
+    if (!(a >= 0.0) || !(a < 1.0e30)) return lya_fail(ctx, LYA_EINVAL, "lya_flux_with_pdf: A must be finite and >= 0");
+    if (n_bins < 1 || n_bins > 256 || !(width > 0.0))
+        return lya_fail(ctx, LYA_EINVAL, "lya_flux_with_pdf: 1 <= n_bins <= 256 and width > 0 required");
+    LYA_CUDA(ctx, cudaSetDevice(ctx->device));
+    return lya_run_flux_with_pdf(ctx, tau, n_pix, a, flux, n_bins, f_lo, width, counts, pdf);
+}
+
 lya_status lya_root_init(lya_root_state *s, double f_target, double rel_tol, double n_pix_global)
 {
     if (!s || !(f_target > 0.0 && f_target < 1.0) || !(rel_tol > 0.0) || !(n_pix_global >= 1.0)) return LYA_EINVAL;

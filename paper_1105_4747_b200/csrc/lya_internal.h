@@ -85,6 +85,8 @@ lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
 lya_status lya_launch_flux(lya_ctx *ctx, const float *tau, size_t n, double a, float *flux);
 lya_status lya_run_normalize(lya_ctx *ctx, const float *tau, size_t n, double f_target, double rel_tol,
                              int max_iter, double *a_out, double *f_out, int *iters);
+lya_status lya_run_flux_with_pdf(lya_ctx *ctx, const float *tau, size_t n, double a, float *flux, int n_bins,
+                                 double f_lo, double width, uint64_t *counts, double *pdf);
 lya_status lya_run_moment_sums(lya_ctx *ctx, const float *tau, size_t n, double a_trial, double *sums5);
 lya_status lya_run_partial_sums(lya_ctx *ctx, const float *tau, size_t n, const double *a_trial, int k,
                                 double *sums, double *dsums);

@@ -282,6 +282,61 @@ __global__ void __launch_bounds__(256) flux_kernel(const float *tau, size_t n, T
     }
 }
 
+// S5 and the flux PDF in one pass: F is written as by flux_kernel and binned as by
+// flux_pdf_kernel (observe.cu) -- private per-thread histograms hist[bin][thread] in shared memory, the bin
+// decision taken in fp32 with two separately rounded operations (reading O4) -- so the counts are bit-identical
+// to lya_flux followed by lya_flux_pdf, with 8 B instead of 12 B of traffic per pixel.
+constexpr int FPDF_THREADS = 128;
+
+__global__ void __launch_bounds__(FPDF_THREADS) flux_pdf_fused_kernel(const float *tau, size_t n, Trial tr, float *flux,
+                                                                      int n_bins, float f_lo, float inv_width,
+                                                                      unsigned long long *__restrict__ counts)
+{
+    extern __shared__ unsigned int hist[];               // [n_bins][FPDF_THREADS]
+    for (int t = threadIdx.x; t < n_bins * FPDF_THREADS; t += FPDF_THREADS) hist[t] = 0u;
+    __syncthreads();
+    unsigned int *mine = hist + threadIdx.x;
+    const float top = (float)n_bins;
+    auto bin = [&](float f) {
+        const float t = floorf(__fmul_rn(__fsub_rn(f, f_lo), inv_width));
+        const int b = (t >= top) ? n_bins - 1 : (t > 0.0f ? (int)t : 0);
+        mine[b * FPDF_THREADS] += 1u;
+    };
+    const size_t gtid = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t gsz  = (size_t)gridDim.x * blockDim.x;
+    size_t head = ((16 - ((uintptr_t)tau & 15)) & 15) >> 2;
+    if (head > n) head = n;
+    const bool vec = (((uintptr_t)(flux + head)) & 15) == 0;
+    const size_t n4 = vec ? (n - head) >> 2 : 0;
+    const float4 *t4 = reinterpret_cast<const float4 *>(tau + head);
+    float4 *f4 = reinterpret_cast<float4 *>(flux + head);
+#pragma unroll 2
+    for (size_t i = gtid; i < n4; i += gsz) {
+        const float4 t = __ldcs(t4 + i);
+        float4 f;
+        f.x = flux_of(t.x, tr); f.y = flux_of(t.y, tr); f.z = flux_of(t.z, tr); f.w = flux_of(t.w, tr);
+        __stcs(f4 + i, f);
+        bin(f.x); bin(f.y); bin(f.z); bin(f.w);
+    }
+    const size_t tail0 = head + (n4 << 2);
+    const size_t n_edge = head + (n - tail0);
+    for (size_t e = gtid; e < n_edge; e += gsz) {
+        const size_t i = e < head ? e : tail0 + (e - head);
+        const float f = flux_of(tau[i], tr);
+        flux[i] = f;
+        bin(f);
+    }
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int b = warp; b < n_bins; b += FPDF_THREADS / 32) {
+        unsigned int sum = 0;
+        for (int t = lane; t < FPDF_THREADS; t += 32) sum += hist[b * FPDF_THREADS + t];
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
+        if (lane == 0 && sum) atomicAdd(counts + b, (unsigned long long)sum);
+    }
+}
+
 int red_grid(lya_ctx *ctx, size_t n, int per_sm)
 {
     size_t want = (n / 4 + RED_THREADS - 1) / RED_THREADS;
@@ -372,5 +427,34 @@ lya_status lya_run_moment_sums(lya_ctx *ctx, const float *tau, size_t n, double 
     LYA_CUDA(ctx, cudaMemcpyAsync(ctx->h_pinned, ctx->d_root, 5 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     for (int i = 0; i < 5; ++i) sums5[i] = ctx->h_pinned[i];
+    return LYA_OK;
+}
+
+lya_status lya_run_flux_with_pdf(lya_ctx *ctx, const float *tau, size_t n, double a, float *flux, int n_bins,
+                                 double f_lo, double width, uint64_t *counts, double *pdf)
+{
+    unsigned long long *d_counts = reinterpret_cast<unsigned long long *>(ctx->d_stats);
+    LYA_CUDA(ctx, cudaMemsetAsync(d_counts, 0, (size_t)n_bins * sizeof(unsigned long long), ctx->stream));
+    if (n > 0) {
+        const size_t smem = (size_t)n_bins * FPDF_THREADS * sizeof(unsigned int);
+        LYA_CUDA(ctx, cudaFuncSetAttribute(flux_pdf_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        int per_sm = 0;
+        LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, flux_pdf_fused_kernel, FPDF_THREADS, smem));
+        if (per_sm < 1) return lya_fail(ctx, LYA_EINVAL, "lya_flux_with_pdf: too many bins for shared memory");
+        size_t want = (n / 4 + FPDF_THREADS - 1) / FPDF_THREADS;
+        if (want < 1) want = 1;
+        const size_t cap = (size_t)ctx->sm_count * per_sm;
+        flux_pdf_fused_kernel<<<(int)(want < cap ? want : cap), FPDF_THREADS, smem, ctx->stream>>>(
+            tau, n, make_trial(a), flux, n_bins, (float)f_lo, (float)(1.0 / width), d_counts);
+        ctx->launches++;
+        LYA_CUDA(ctx, cudaGetLastError());
+    }
+    uint64_t host[256];
+    LYA_CUDA(ctx, cudaMemcpyAsync(host, d_counts, (size_t)n_bins * sizeof(uint64_t), cudaMemcpyDeviceToHost, ctx->stream));
+    LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    for (int b = 0; b < n_bins; ++b) {
+        if (counts) counts[b] = host[b];
+        if (pdf) pdf[b] = n ? (double)host[b] / ((double)n * width) : 0.0;
+    }
     return LYA_OK;
 }

@@ -86,7 +86,7 @@ EXPORTS = ("lya_version", "lya_status_string", "lya_scalars_from_params", "lya_c
            "lya_flux", "lya_forest_host", "lya_launch_count", "lya_measure_mufu_peak",
            "lya_bin_kms_from_angstrom", "lya_instrument_bins", "lya_observe_rows", "lya_flux_pdf",
            "lya_flux_power_rows", "lya_tau_sightlines_opt", "lya_growth_rate", "lya_fields_from_dm", "lya_flux_moment_sums",
-           "lya_root_update_moments")
+           "lya_root_update_moments", "lya_flux_with_pdf")
 
 _lib = None
 
@@ -133,6 +133,8 @@ def lib() -> C.CDLL:
     L.lya_instrument_bins.restype = C.c_int32
     L.lya_observe_rows.argtypes = [vp, C.c_size_t, C.c_int32, C.c_double, C.POINTER(CInstrument), fp, fp, fp]
     L.lya_flux_pdf.argtypes = [vp, fp, C.c_size_t, C.c_int32, C.c_double, C.c_double, C.POINTER(C.c_uint64), dp]
+    L.lya_flux_with_pdf.argtypes = [vp, fp, C.c_size_t, C.c_double, fp, C.c_int32, C.c_double, C.c_double,
+                                    C.POINTER(C.c_uint64), dp]
     L.lya_flux_power_rows.argtypes = [vp, C.c_size_t, C.c_int32, C.c_double, fp, C.c_double, dp]
     _lib = L
     return L
@@ -301,6 +303,16 @@ class Context:
         pdf = (C.c_double * n_bins)()
         self._check(lib().lya_flux_pdf(self._h, _dev(flux, "flux"), flux.numel(), n_bins, f_lo, width, counts, pdf))
         return np.array(counts, dtype=np.uint64), np.array(pdf, dtype=np.float64)
+
+    def flux_with_pdf(self, tau, a: float, out=None, n_bins: int = 21, f_lo: float = -0.025, width: float = 0.05):
+        """S5 and the flux PDF in one pass: returns (F, counts, pdf)."""
+        import numpy as np
+        out = torch.empty_like(tau) if out is None else out
+        counts = (C.c_uint64 * n_bins)()
+        pdf = (C.c_double * n_bins)()
+        self._check(lib().lya_flux_with_pdf(self._h, _dev(tau, "tau"), tau.numel(), a, _dev(out, "flux"), n_bins,
+                                            f_lo, width, counts, pdf))
+        return out, np.array(counts, dtype=np.uint64), np.array(pdf, dtype=np.float64)
 
     def flux_power_rows(self, flux, dv_kms: float, mean_flux: float):
         import numpy as np

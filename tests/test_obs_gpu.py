@@ -117,3 +117,20 @@ def test_flux_power_lengths_and_errors(ctx, obs, n):
     assert np.all(np.abs(P - ref) <= 1e-4 * ref + 1e-9 * ref.max())
     with pytest.raises(lya.LyaError):
         ctx.flux_power_rows(F[:, : n - 1].contiguous(), 2.0, 0.5)   # not a power of two
+
+
+def test_flux_with_pdf_equals_the_two_calls(ctx, flux_rows):
+    """S5 and the PDF fused in one pass: F and the counts are bit-identical to lya_flux + lya_flux_pdf."""
+    w = WORKLOADS[2]
+    f = inputs.make_fields(w, device="cuda", z0=0, z1=4)
+    p = lya.Params.from_workload(w)
+    n_hi, b = ctx.gas_from_density(p, f["delta"])
+    tau = ctx.tau_sightlines(p, 0, n_hi, b, f["v_pec"][0], nz_local=4)
+    for t in (tau, tau.reshape(-1)[5:200_003]):                       # aligned, and unaligned + ragged
+        t = t.contiguous() if t.dim() == 3 else t
+        F = ctx.flux(t, 0.7)
+        c_ref, p_ref = ctx.flux_pdf(F)
+        F2, counts, pdf = ctx.flux_with_pdf(t, 0.7)
+        assert torch.equal(F2, F) and np.array_equal(counts, c_ref) and np.allclose(pdf, p_ref, rtol=1e-14)
+    F3, counts, _ = ctx.flux_with_pdf(tau, 0.7, out=tau.clone(), n_bins=40, f_lo=0.0, width=0.025)
+    assert counts.sum() == tau.numel()
