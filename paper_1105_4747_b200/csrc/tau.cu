@@ -127,10 +127,18 @@ __device__ __forceinline__ float stage_from_global(const TauArgs &a, float jf, s
     return stage_cell(a, jf, nh, bb, __ldcs(a.v + g), out);
 }
 
-// Staged cells are stored at cpos(j): plain for the full sum (every lane reads the same cell: broadcast), one
-// pad slot in 8 for LYA_TAU_WINDOWED, where lanes read DIFFERENT cells R apart (16 R bytes: without the pad the
-// eight lanes of an LDS.128 phase would hit two banks).
-template <bool PAD> __device__ __forceinline__ int cpos(int j) { return PAD ? j + (j >> 3) : j; }
+// Staged cells are stored at cpos(j): plain for the full sum (every lane reads the same cell: broadcast); for
+// LYA_TAU_WINDOWED, where lane k reads cell j0 + R k, one pad slot per R cells, j + j / R: the lanes of an
+// LDS.128 phase then sit (R + 1) float4 apart, and R + 1 being odd the eight of them fall into the eight
+// different 16-byte bank groups whatever j0 is (R = 1 needs no pad: neighbouring cells).
+template <bool PAD, int R> __device__ __forceinline__ int cpos(int j)
+{
+    return (PAD && R > 1) ? j + (R == 2 ? (j >> 1) : (j >> 2)) : j;
+}
+template <int R> __host__ __device__ constexpr int crow_len(int n, bool pad)        // slots of one staged row
+{
+    return (pad && R > 1) ? n + (R == 2 ? (n >> 1) : (n >> 2)) + 1 : n;
+}
 
 // Fast path, full sum: unwrapped walk over all n sources jj = start .. start + n - 1 around the tile centre (at
 // most one wrap), no per-pair image logic.  Lane owns pixels i0 + lane*R + r.
@@ -150,7 +158,7 @@ __device__ __forceinline__ void tile_fast(const float4 *__restrict__ cs, int n, 
         const int lo = seg ? 0 : j0, hi = seg ? j0 : n;
 #pragma unroll 8
         for (int j = lo; j < hi; ++j) {
-            const float4 q = cs[cpos<PAD>(j)];
+            const float4 q = cs[cpos<PAD, R>(j)];
             const float E  = cref - q.x;
             const float xr = fmaf(E, q.y, q.z);
 #pragma unroll
@@ -168,7 +176,7 @@ __device__ __forceinline__ void tile_fast(const float4 *__restrict__ cs, int n, 
 // (il = i0 + lane R), W = the sightline's reach: 2 W + R sources instead of n.  A source outside the window is
 // further than its reach from all R pixels, so it would have added ex2(..) == 0 exactly; the sources kept are
 // added in the same ascending order with the same arithmetic (same reference pixel), so the result is
-// bit-identical to tile_fast.  Lanes read different cells (conflict-free through cpos<true>); the wrap is one
+// bit-identical to tile_fast.  Lanes read different cells (conflict-free through cpos<true, R>); the wrap is one
 // compare per source cell.
 template <int R>
 __device__ __forceinline__ void tile_window(const float4 *__restrict__ cs, int n, float n_f, int i0, int lane, int W,
@@ -185,7 +193,7 @@ __device__ __forceinline__ void tile_window(const float4 *__restrict__ cs, int n
     const int cnt = 2 * W + R;
 #pragma unroll 4
     for (int t = 0; t < cnt; ++t) {
-        const float4 q = cs[cpos<true>(j)];
+        const float4 q = cs[cpos<true, R>(j)];
         const float E  = cref - q.x;
         const float xr = fmaf(E, q.y, q.z);
 #pragma unroll
@@ -211,7 +219,7 @@ __device__ __forceinline__ void tile_general(const float4 *__restrict__ cs, int 
     }
 #pragma unroll 2
     for (int j = 0; j < n; ++j) {
-        const float4 q = cs[cpos<PAD>(j)];
+        const float4 q = cs[cpos<PAD, R>(j)];
         const float  f = -q.z / q.y;                    // fractional displacement (only picks the image)
 #pragma unroll
         for (int r = 0; r < R; ++r) {
@@ -263,7 +271,7 @@ __global__ void __launch_bounds__(1024, 1) tau_x_kernel(const TauArgs a, const i
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int grp = warp / G, wg = warp - grp * G;       // group in CTA, warp in group
     const int n = a.n;
-    const int crow = WIN ? n + (n >> 3) + 1 : n;         // float4 slots per staged row
+    const int crow = crow_len<R>(n, WIN);                // float4 slots per staged row
     float4 *cells = reinterpret_cast<float4 *>(smem) + (size_t)grp * crow;
     volatile int *ctl = reinterpret_cast<volatile int *>(smem + (size_t)gpc * crow * sizeof(float4)) + 4 * grp;
     const int bar_id = grp;      // named barrier of the group (G >= 2: at most 16 groups; no __syncthreads here)
@@ -284,7 +292,7 @@ __global__ void __launch_bounds__(1024, 1) tau_x_kernel(const TauArgs a, const i
         for (int j = gl; j < n; j += gthreads) {
             float4 q;
             reach = fmaxf(reach, stage_from_global<FUSED>(a, jf, g0 + j, q));
-            cells[cpos<WIN>(j)] = q;
+            cells[cpos<WIN, R>(j)] = q;
             jf += (float)gthreads;
         }
 #pragma unroll
@@ -372,7 +380,7 @@ __global__ void __launch_bounds__(TAU_THREADS) tau_strided_kernel(const TauArgs 
             if (bx < nb) {
                 float4 q;
                 reach = fmaxf(reach, stage_from_global<FUSED>(a, (float)j, (size_t)(base + (long long)j * a.stride + bx), q));
-                cells[bx * cstride + cpos<WIN>(j)] = q;
+                cells[bx * cstride + cpos<WIN, R>(j)] = q;
             }
         }
 #pragma unroll
@@ -421,7 +429,7 @@ lya_status launch_x(lya_ctx *ctx, const TauArgs &a)
 {
     auto kern = tau_x_kernel<R, FUSED, WIN>;
     const size_t cap = (size_t)ctx->max_smem_optin;
-    const size_t per_group = (size_t)(WIN ? a.n + (a.n >> 3) + 1 : a.n) * sizeof(float4) + 16;
+    const size_t per_group = (size_t)crow_len<R>(a.n, WIN) * sizeof(float4) + 16;
     int groups = (int)(cap / per_group);                 // groups that fit in one SM's shared memory
     if (groups < 1) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: sightline too long for shared memory");
     // G warps per group: as few as keep >= 24 warps resident, never more than the row has tiles
@@ -512,7 +520,7 @@ lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
     auto pad_to = [](int v, int mod, int want) { return v + ((want - v % mod) % mod + mod) % mod; };
     auto strides = [&](int sh, int &cs, int &ts) {
         const int bs = 1 << sh;
-        cs = pad_to(win ? n + (n >> 3) + 1 : n, 8, (8 / bs) % 8);
+        cs = pad_to(R == 4 ? crow_len<4>(n, win) : (R == 2 ? crow_len<2>(n, win) : n), 8, (8 / bs) % 8);
         ts = pad_to(a.tiles * 32 * R, 32, (32 / bs) % 32);
     };
     auto need2 = [&](int sh) {
