@@ -36,9 +36,9 @@ extern "C" lya_status lya_forest_host(lya_ctx *ctx, const lya_params *p, int axi
     const size_t plane = (size_t)p->nx * p->ny, total = plane * p->nz;
     int snz = slab_nz;
     if (axis == 2) snz = p->nz;
-    if (snz <= 0) {                                   // ~8 slabs, each between 2^22 and 2^28 cells
-        size_t cells = total / 8;
-        if (cells < ((size_t)1 << 22)) cells = (size_t)1 << 22;
+    if (snz <= 0) {                                   // ~16 slabs, each between 2^20 and 2^28 cells: only the
+        size_t cells = total / 16;                    // first slab's copy and the last slab's sums are exposed
+        if (cells < ((size_t)1 << 20)) cells = (size_t)1 << 20;
         if (cells > ((size_t)1 << 28)) cells = (size_t)1 << 28;
         snz = (int)((cells + plane - 1) / plane);
     }
