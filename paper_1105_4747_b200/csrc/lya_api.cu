@@ -79,7 +79,6 @@ lya_status lya_create(lya_ctx **out, int device, void *cuda_stream)
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->coop_ok, cudaDevAttrCooperativeLaunch, device);
     const size_t part_bytes = (size_t)2 * LYA_MAX_RED_BLOCKS * 2 * LYA_MAX_TRIALS * sizeof(double);
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->d_partials, part_bytes);
-    if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->d_root, 64 * sizeof(double));
     if (e == cudaSuccess) e = cudaMallocHost((void **)&ctx->h_pinned, 64 * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->d_stats, LYA_STATS_DOUBLES * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->d_sched, 4 * sizeof(unsigned int));
@@ -104,7 +103,6 @@ void lya_destroy(lya_ctx *ctx)
     lya_fields_release(ctx);
     if (ctx->ws) cudaFree(ctx->ws);
     if (ctx->d_partials) cudaFree(ctx->d_partials);
-    if (ctx->d_root) cudaFree(ctx->d_root);
     if (ctx->d_sched) cudaFree(ctx->d_sched);
     if (ctx->d_stats) cudaFree(ctx->d_stats);
     if (ctx->d_taps) cudaFree(ctx->d_taps);

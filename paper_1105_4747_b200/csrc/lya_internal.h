@@ -19,8 +19,7 @@ struct lya_ctx {
     uint64_t      launches;
     // reduction scratch (device): per-block partial sums, root state
     double       *d_partials;     // [2 parities][LYA_MAX_RED_BLOCKS][2*LYA_MAX_TRIALS]
-    double       *d_root;         // device copy of the root-iteration result (see normalize.cu)
-    double       *h_pinned;       // small pinned host mirror
+    double       *h_pinned;       // 64 doubles of pinned host memory, written by the kernels directly (UVA)
     unsigned int *d_sched;        // tau_x_kernel row counter {next row, groups finished}; zero between launches
     double       *d_stats;        // 8192 doubles: flux-PDF counts (as uint64) / power-spectrum accumulators
     float        *d_taps, *h_taps; // lya_observe_rows: Gaussian taps (device / host staging), grown on demand

@@ -355,7 +355,8 @@ lya_status lya_run_normalize(lya_ctx *ctx, const float *tau, size_t n, double f_
     int per_sm = 0;
     LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, normalize_kernel, NORM_THREADS, 0));
     if (per_sm < 1) return lya_fail(ctx, LYA_ECUDA, "normalize_kernel: zero occupancy");
-    NormArgs a{tau, n, f_target, rel_tol, max_iter, ctx->d_partials, ctx->d_root};
+    // the four result doubles go straight to the pinned host mirror (mapped under UVA): no copy to enqueue
+    NormArgs a{tau, n, f_target, rel_tol, max_iter, ctx->d_partials, ctx->h_pinned};
     size_t want = (n / 4 + NORM_THREADS - 1) / NORM_THREADS;           // at least one float4 per thread
     if (want < 1) want = 1;
     const int grid = (int)(want < (size_t)ctx->sm_count ? want : (size_t)ctx->sm_count);
@@ -363,8 +364,6 @@ lya_status lya_run_normalize(lya_ctx *ctx, const float *tau, size_t n, double f_
     LYA_CUDA(ctx, cudaLaunchCooperativeKernel((void *)normalize_kernel, dim3(grid), dim3(NORM_THREADS), args, 0,
                                               ctx->stream));
     ctx->launches++;
-    LYA_CUDA(ctx, cudaMemcpyAsync(ctx->h_pinned, ctx->d_root, 4 * sizeof(double), cudaMemcpyDeviceToHost,
-                                  ctx->stream));
     LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     if (a_out) *a_out = ctx->h_pinned[0];
     if (f_out) *f_out = ctx->h_pinned[1];
@@ -389,11 +388,9 @@ lya_status lya_run_partial_sums(lya_ctx *ctx, const float *tau, size_t n, const 
 #undef LYA_PS_CASE
         default: return lya_fail(ctx, LYA_EINVAL, "lya_flux_partial_sums: k must be 1..8");
     }
-    finish_sums_kernel<<<1, RED_THREADS, 0, ctx->stream>>>(part, grid, 2 * k, ctx->d_root);
+    finish_sums_kernel<<<1, RED_THREADS, 0, ctx->stream>>>(part, grid, 2 * k, ctx->h_pinned);   // mapped pinned memory
     ctx->launches += 2;
     LYA_CUDA(ctx, cudaGetLastError());
-    LYA_CUDA(ctx, cudaMemcpyAsync(ctx->h_pinned, ctx->d_root, 2 * k * sizeof(double), cudaMemcpyDeviceToHost,
-                                  ctx->stream));
     LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     for (int i = 0; i < k; ++i) {
         sums[i] = ctx->h_pinned[i];
@@ -421,10 +418,9 @@ lya_status lya_run_moment_sums(lya_ctx *ctx, const float *tau, size_t n, double 
 {
     const int grid = red_grid(ctx, n, 8);
     moment_sums_kernel<<<grid, RED_THREADS, 0, ctx->stream>>>(tau, n, make_trial(a_trial), ctx->d_partials);
-    finish_sums_kernel<<<1, RED_THREADS, 0, ctx->stream>>>(ctx->d_partials, grid, 5, ctx->d_root);
+    finish_sums_kernel<<<1, RED_THREADS, 0, ctx->stream>>>(ctx->d_partials, grid, 5, ctx->h_pinned);   // mapped pinned memory
     ctx->launches += 2;
     LYA_CUDA(ctx, cudaGetLastError());
-    LYA_CUDA(ctx, cudaMemcpyAsync(ctx->h_pinned, ctx->d_root, 5 * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     for (int i = 0; i < 5; ++i) sums5[i] = ctx->h_pinned[i];
     return LYA_OK;
