@@ -10,6 +10,8 @@
 #include <dlfcn.h>
 #include <math.h>
 
+#include <mutex>
+
 #include "lya_internal.h"
 
 namespace {
@@ -26,8 +28,9 @@ struct CufftApi {
 CufftApi *cufft_api()
 {
     static CufftApi api = {};
-    static int state = 0;                                  // 0 untried, 1 ok, -1 missing
-    if (state == 0) {
+    static std::once_flag once;
+    static bool ok = false;
+    std::call_once(once, [] {                               // contexts of several host threads may race here
         const char *names[] = {"libcufft.so.11", "libcufft.so", "/usr/local/cuda/lib64/libcufft.so.11",
                                "/usr/local/cuda/lib64/libcufft.so"};
         for (const char *nm : names)
@@ -39,9 +42,9 @@ CufftApi *cufft_api()
             api.ExecC2R   = (decltype(api.ExecC2R))dlsym(api.handle, "cufftExecC2R");
             api.Destroy   = (decltype(api.Destroy))dlsym(api.handle, "cufftDestroy");
         }
-        state = (api.handle && api.Plan3d && api.SetStream && api.ExecR2C && api.ExecC2R && api.Destroy) ? 1 : -1;
-    }
-    return state == 1 ? &api : nullptr;
+        ok = api.handle && api.Plan3d && api.SetStream && api.ExecR2C && api.ExecC2R && api.Destroy;
+    });
+    return ok ? &api : nullptr;
 }
 
 struct KArgs {

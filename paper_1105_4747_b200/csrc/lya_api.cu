@@ -72,6 +72,7 @@ lya_status lya_create(lya_ctx **out, int device, void *cuda_stream)
     if (!ctx) return LYA_ENOMEM;
     memset(ctx, 0, sizeof(*ctx));
     ctx->device = device;
+    ctx->taps_key[0] = ctx->bins_key[0] = -1.0;
     ctx->stream = (cudaStream_t)cuda_stream;
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device);

@@ -24,8 +24,10 @@ struct lya_ctx {
     double       *d_stats;        // 8192 doubles: flux-PDF counts (as uint64) / power-spectrum accumulators
     float        *d_taps, *h_taps; // lya_observe_rows: Gaussian taps (device / host staging), grown on demand
     size_t        taps_cap;
+    double        taps_key[4];    // (sigma_px, Kl, Kr, KO) of the taps now on the device
     void         *d_bins, *h_bins; // lya_observe_rows: per-bin geometry table (int4 per output bin)
     size_t        bins_cap;
+    double        bins_key[3];    // (bin_px, n_pix, n_bins) of the table now on the device
     int           fft_dims[3];    // lya_fields_from_dm: cached cuFFT plans (handles are ints) for [nz][ny][nx]
     int           fft_r2c, fft_c2r;
     // lya_forest_host / lya_fields_from_dm workspace (device), grown on demand

@@ -417,17 +417,24 @@ extern "C" lya_status lya_observe_rows(lya_ctx *ctx, size_t n_rows, int32_t n_pi
             if (!ctx->h_taps) return lya_fail(ctx, LYA_ENOMEM, "lya_observe_rows: host allocation failed");
             LYA_CUDA(ctx, cudaMalloc((void **)&ctx->d_taps, (size_t)(n_t + 64) * sizeof(float)));
             ctx->taps_cap = (size_t)n_t + 64;
+            ctx->taps_key[0] = -1.0;
         }
-        // the stream may still be reading the previous call's taps: wait before overwriting the host copy
-        LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-        double sum = 0.0;
-        for (int k = -a.Kl; k <= a.Kr; ++k) sum += exp(-0.5 * (double)k * k / (sigma_px * sigma_px));
-        for (int t = 0; t < n_t; ++t) ctx->h_taps[t] = 0.0f;
-        for (int t = a.KO - a.Kr; t <= a.L; ++t) {                      // offset k = KO - t in [-Kl, Kr]
-            const double k = (double)(a.KO - t);
-            ctx->h_taps[t + 3] = (float)(exp(-0.5 * k * k / (sigma_px * sigma_px)) / sum);
+        // the taps depend on (sigma, Kl, Kr, KO) only: a repeated call (the usual case: one instrument, many
+        // slabs) finds them on the device already and needs neither a synchronisation nor a copy
+        if (!(ctx->taps_key[0] == sigma_px && ctx->taps_key[1] == (double)a.Kl && ctx->taps_key[2] == (double)a.Kr &&
+              ctx->taps_key[3] == (double)a.KO)) {
+            // the stream may still be reading the previous call's taps: wait before overwriting the host copy
+            LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+            double sum = 0.0;
+            for (int k = -a.Kl; k <= a.Kr; ++k) sum += exp(-0.5 * (double)k * k / (sigma_px * sigma_px));
+            for (int t = 0; t < n_t; ++t) ctx->h_taps[t] = 0.0f;
+            for (int t = a.KO - a.Kr; t <= a.L; ++t) {                  // offset k = KO - t in [-Kl, Kr]
+                const double k = (double)(a.KO - t);
+                ctx->h_taps[t + 3] = (float)(exp(-0.5 * k * k / (sigma_px * sigma_px)) / sum);
+            }
+            LYA_CUDA(ctx, cudaMemcpyAsync(ctx->d_taps, ctx->h_taps, (size_t)n_t * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
+            ctx->taps_key[0] = sigma_px; ctx->taps_key[1] = a.Kl; ctx->taps_key[2] = a.Kr; ctx->taps_key[3] = a.KO;
         }
-        LYA_CUDA(ctx, cudaMemcpyAsync(ctx->d_taps, ctx->h_taps, (size_t)n_t * sizeof(float), cudaMemcpyHostToDevice, ctx->stream));
         a.taps = ctx->d_taps;
     }
     // ---- lean kernel for the common case
@@ -445,34 +452,39 @@ extern "C" lya_status lya_observe_rows(lya_ctx *ctx, size_t n_rows, int32_t n_pi
                 if (!ctx->h_bins) return lya_fail(ctx, LYA_ENOMEM, "lya_observe_rows: host allocation failed");
                 LYA_CUDA(ctx, cudaMalloc(&ctx->d_bins, (size_t)(nb + 64) * sizeof(int4)));
                 ctx->bins_cap = (size_t)nb + 64;
+                ctx->bins_key[0] = -1.0;
             }
-            LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));             // previous call may still read h_bins
-            int4 *hb = (int4 *)ctx->h_bins;
             a.bins3 = bin_px <= 2.0;
-            for (int m = 0; m < nb; ++m) {                                  // bin [lo, hi) in pixel units (reading O2)
-                const double lo = (double)m * bin_px, hi = lo + bin_px;
-                int i0 = (int)floor(lo), i1 = (int)ceil(hi) - 1;
-                if (i1 > n_pix - 1) i1 = n_pix - 1;
-                int4 e;
-                if (a.bins3) {                                              // overlap of the bin with pixels i0, i0+1, i0+2
-                    float wq[3];
-                    for (int q = 0; q < 3; ++q) {
-                        const double l = lo > (double)(i0 + q) ? lo : (double)(i0 + q);
-                        const double h = hi < (double)(i0 + q + 1) ? hi : (double)(i0 + q + 1);
-                        wq[q] = (h > l && i0 + q < n_pix) ? (float)((h - l) / bin_px) : 0.0f;
+            if (!(ctx->bins_key[0] == bin_px && ctx->bins_key[1] == (double)n_pix && ctx->bins_key[2] == (double)nb)) {
+                LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));         // previous call may still read h_bins
+                int4 *hb = (int4 *)ctx->h_bins;
+                a.bins3 = bin_px <= 2.0;
+                for (int m = 0; m < nb; ++m) {                                  // bin [lo, hi) in pixel units (reading O2)
+                    const double lo = (double)m * bin_px, hi = lo + bin_px;
+                    int i0 = (int)floor(lo), i1 = (int)ceil(hi) - 1;
+                    if (i1 > n_pix - 1) i1 = n_pix - 1;
+                    int4 e;
+                    if (a.bins3) {                                              // overlap of the bin with pixels i0, i0+1, i0+2
+                        float wq[3];
+                        for (int q = 0; q < 3; ++q) {
+                            const double l = lo > (double)(i0 + q) ? lo : (double)(i0 + q);
+                            const double h = hi < (double)(i0 + q + 1) ? hi : (double)(i0 + q + 1);
+                            wq[q] = (h > l && i0 + q < n_pix) ? (float)((h - l) / bin_px) : 0.0f;
+                        }
+                        e.x = i0;
+                        memcpy(&e.y, &wq[0], 4); memcpy(&e.z, &wq[1], 4); memcpy(&e.w, &wq[2], 4);
+                    } else {
+                        float wf, wl;
+                        if (i1 <= i0) { i1 = i0; wf = (float)((hi - lo) / bin_px); wl = 0.0f; }
+                        else { wf = (float)(((double)(i0 + 1) - lo) / bin_px); wl = (float)((hi - (double)i1) / bin_px); }
+                        e.x = i0; e.y = i1;
+                        memcpy(&e.z, &wf, 4); memcpy(&e.w, &wl, 4);
                     }
-                    e.x = i0;
-                    memcpy(&e.y, &wq[0], 4); memcpy(&e.z, &wq[1], 4); memcpy(&e.w, &wq[2], 4);
-                } else {
-                    float wf, wl;
-                    if (i1 <= i0) { i1 = i0; wf = (float)((hi - lo) / bin_px); wl = 0.0f; }
-                    else { wf = (float)(((double)(i0 + 1) - lo) / bin_px); wl = (float)((hi - (double)i1) / bin_px); }
-                    e.x = i0; e.y = i1;
-                    memcpy(&e.z, &wf, 4); memcpy(&e.w, &wl, 4);
+                    hb[m] = e;
                 }
-                hb[m] = e;
+                LYA_CUDA(ctx, cudaMemcpyAsync(ctx->d_bins, hb, (size_t)nb * sizeof(int4), cudaMemcpyHostToDevice, ctx->stream));
+                ctx->bins_key[0] = bin_px; ctx->bins_key[1] = n_pix; ctx->bins_key[2] = nb;
             }
-            LYA_CUDA(ctx, cudaMemcpyAsync(ctx->d_bins, hb, (size_t)nb * sizeof(int4), cudaMemcpyHostToDevice, ctx->stream));
             a.bins = (const int4 *)ctx->d_bins;
         }
         // LT: the smallest instantiated multiple of 4 that is >= L (every multiple of 4 up to 64, then 96, 124)
