@@ -208,7 +208,33 @@ __global__ void __launch_bounds__(256) observe_rows_kernel(const ObsArgs a)
 // immediate offset (17 instructions per 16 FFMA instead of 26); and the bin geometry of the rebinning, which
 // is the same for every row, comes from a table built once on the host (bins[m] = first pixel, last pixel,
 // weight of the first and of the last pixel) and kept in shared memory.
-struct ObsTaps { float wp[136]; };                       // wp[t + 3] = g(KO - t); zero outside the real taps
+// packed FP32 pairs (sm_100a: fma.rn.f32x2 = FFMA2, one issue slot for two fused multiply-adds)
+constexpr int OBS_PACKED_LT = 40;                        // beyond this the weight pairs no longer fit in registers
+__device__ __forceinline__ unsigned long long pack2(float lo, float hi)
+{
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ unsigned long long ffma2(unsigned long long a, unsigned long long b, unsigned long long c)
+{
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ float sum2(unsigned long long v)
+{
+    float lo, hi;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+    return lo + hi;
+}
+
+struct __align__(16) ObsTaps {
+    float wp[136];                                       // wp[t + 3] = g(KO - t); zero outside the real taps
+    float wq[136];                                       // wq[k] = wp[k + 1]: every (wp[k], wp[k + 1]) pair is 8-byte aligned in one of the two
+};
+// (wp[k], wp[k + 1]) as one 64-bit operand, k known at compile time
+#define OBS_WPAIR(k) (((k) & 1) ? pack2(tp.wq[(k) - 1], tp.wq[(k)]) : pack2(tp.wp[(k)], tp.wp[(k) + 1]))
 
 template <int LT, int NV>                                // LT >= L, multiple of 4: taps t = 0 .. LT; NV float4 per thread
 __global__ void __launch_bounds__(256) observe_rows_lean_kernel(const ObsArgs a, const __grid_constant__ ObsTaps tp)
@@ -260,13 +286,30 @@ __global__ void __launch_bounds__(256) observe_rows_lean_kernel(const ObsArgs a,
             if (p < n) {
                 const float *si = s_in + p;
                 float acc0 = 0.f, acc1 = 0.f, acc2 = 0.f, acc3 = 0.f;
+                if constexpr (LT <= OBS_PACKED_LT) {
+                    // packed FP32 (FFMA2): output r keeps an (even inputs, odd inputs) pair of partial sums, the
+                    // input pairs (x, y) and (z, w) come straight out of the LDS.128 and the weight pairs
+                    // (wp[k], wp[k + 1]) are loop-invariant registers: 8 FFMA2 per LDS.128 instead of 16 FFMA
+                    unsigned long long c0 = 0ull, c1 = 0ull, c2 = 0ull, c3 = 0ull;
 #pragma unroll
-                for (int u = 0; u < LT + 4; u += 4) {    // input u and output r use wp[u - r + 3]
-                    const float4 x = *reinterpret_cast<const float4 *>(si + u);
-                    acc0 = fmaf(tp.wp[u + 3], x.x, acc0); acc0 = fmaf(tp.wp[u + 4], x.y, acc0); acc0 = fmaf(tp.wp[u + 5], x.z, acc0); acc0 = fmaf(tp.wp[u + 6], x.w, acc0);
-                    acc1 = fmaf(tp.wp[u + 2], x.x, acc1); acc1 = fmaf(tp.wp[u + 3], x.y, acc1); acc1 = fmaf(tp.wp[u + 4], x.z, acc1); acc1 = fmaf(tp.wp[u + 5], x.w, acc1);
-                    acc2 = fmaf(tp.wp[u + 1], x.x, acc2); acc2 = fmaf(tp.wp[u + 2], x.y, acc2); acc2 = fmaf(tp.wp[u + 3], x.z, acc2); acc2 = fmaf(tp.wp[u + 4], x.w, acc2);
-                    acc3 = fmaf(tp.wp[u + 0], x.x, acc3); acc3 = fmaf(tp.wp[u + 1], x.y, acc3); acc3 = fmaf(tp.wp[u + 2], x.z, acc3); acc3 = fmaf(tp.wp[u + 3], x.w, acc3);
+                    for (int u = 0; u < LT + 4; u += 4) {
+                        const float4 x = *reinterpret_cast<const float4 *>(si + u);
+                        const unsigned long long xy = pack2(x.x, x.y), zw = pack2(x.z, x.w);
+                        c0 = ffma2(xy, OBS_WPAIR(u + 3), c0); c0 = ffma2(zw, OBS_WPAIR(u + 5), c0);
+                        c1 = ffma2(xy, OBS_WPAIR(u + 2), c1); c1 = ffma2(zw, OBS_WPAIR(u + 4), c1);
+                        c2 = ffma2(xy, OBS_WPAIR(u + 1), c2); c2 = ffma2(zw, OBS_WPAIR(u + 3), c2);
+                        c3 = ffma2(xy, OBS_WPAIR(u + 0), c3); c3 = ffma2(zw, OBS_WPAIR(u + 2), c3);
+                    }
+                    acc0 = sum2(c0); acc1 = sum2(c1); acc2 = sum2(c2); acc3 = sum2(c3);
+                } else {
+#pragma unroll
+                    for (int u = 0; u < LT + 4; u += 4) {    // input u and output r use wp[u - r + 3]
+                        const float4 x = *reinterpret_cast<const float4 *>(si + u);
+                        acc0 = fmaf(tp.wp[u + 3], x.x, acc0); acc0 = fmaf(tp.wp[u + 4], x.y, acc0); acc0 = fmaf(tp.wp[u + 5], x.z, acc0); acc0 = fmaf(tp.wp[u + 6], x.w, acc0);
+                        acc1 = fmaf(tp.wp[u + 2], x.x, acc1); acc1 = fmaf(tp.wp[u + 3], x.y, acc1); acc1 = fmaf(tp.wp[u + 4], x.z, acc1); acc1 = fmaf(tp.wp[u + 5], x.w, acc1);
+                        acc2 = fmaf(tp.wp[u + 1], x.x, acc2); acc2 = fmaf(tp.wp[u + 2], x.y, acc2); acc2 = fmaf(tp.wp[u + 3], x.z, acc2); acc2 = fmaf(tp.wp[u + 4], x.w, acc2);
+                        acc3 = fmaf(tp.wp[u + 0], x.x, acc3); acc3 = fmaf(tp.wp[u + 1], x.y, acc3); acc3 = fmaf(tp.wp[u + 2], x.z, acc3); acc3 = fmaf(tp.wp[u + 3], x.w, acc3);
+                    }
                 }
                 *reinterpret_cast<float4 *>(s_c + p) = make_float4(acc0, acc1, acc2, acc3);
             }
@@ -275,36 +318,34 @@ __global__ void __launch_bounds__(256) observe_rows_lean_kernel(const ObsArgs a,
 
         float *dst = a.out + row * (size_t)a.nb;
         const float *nz = a.noise ? a.noise + row * (size_t)a.nb : nullptr;
-        int k = 0;
-        for (int m = tid; m < a.nb; m += T, ++k) {
-            float v;
+        auto rebinned = [&](int m) -> float {
             if (a.bins3) {                                                        // bins <= 2 pixels wide: at most three
                 const int4 e = s_b[m];                                            // pixels overlap -> {i0, w0, w1, w2}
-                v = fmaf(__int_as_float(e.w), s_c[e.x + 2],
-                         fmaf(__int_as_float(e.z), s_c[e.x + 1], __int_as_float(e.y) * s_c[e.x]));
-            } else if (a.rebin) {
+                return fmaf(__int_as_float(e.w), s_c[e.x + 2],
+                            fmaf(__int_as_float(e.z), s_c[e.x + 1], __int_as_float(e.y) * s_c[e.x]));
+            }
+            if (a.rebin) {
                 const int4 e = s_b[m];
-                if (e.y <= e.x) {
-                    v = __int_as_float(e.z) * s_c[e.x];                           // bin inside one pixel
-                } else {                                                          // weights carry the 1/B
-                    float mid = 0.0f;
+                if (e.y <= e.x) return __int_as_float(e.z) * s_c[e.x];            // bin inside one pixel
+                float mid = 0.0f;                                                 // weights carry the 1/B
 #pragma unroll 1
-                    for (int i = e.x + 1; i < e.y; ++i) mid += s_c[i];
-                    v = fmaf(__int_as_float(e.w), s_c[e.y], fmaf(mid, a.inv_bin_f, __int_as_float(e.z) * s_c[e.x]));
-                }
-            } else {
-                v = s_c[m];
+                for (int i = e.x + 1; i < e.y; ++i) mid += s_c[i];
+                return fmaf(__int_as_float(e.w), s_c[e.y], fmaf(mid, a.inv_bin_f, __int_as_float(e.z) * s_c[e.x]));
             }
-            if (nz) {
-                float z = 0.0f;
-                if (k < OBS_NBR) {
+            return s_c[m];
+        };
 #pragma unroll
-                    for (int kk = 0; kk < OBS_NBR; ++kk) if (kk == k) z = nzr[kk];
-                } else {
-                    z = __ldcs(nz + m);
-                }
-                v = fmaf(z, a.inv_snr, v);
+        for (int k = 0; k < OBS_NBR; ++k) {                                       // noise of these bins is in registers
+            const int m = tid + k * T;
+            if (m < a.nb) {
+                float v = rebinned(m);
+                if (nz) v = fmaf(nzr[k], a.inv_snr, v);
+                __stcs(dst + m, v);
             }
+        }
+        for (int m = tid + OBS_NBR * T; m < a.nb; m += T) {
+            float v = rebinned(m);
+            if (nz) v = fmaf(__ldcs(nz + m), a.inv_snr, v);
             __stcs(dst + m, v);
         }
     }
@@ -443,6 +484,7 @@ extern "C" lya_status lya_observe_rows(lya_ctx *ctx, size_t n_rows, int32_t n_pi
         ObsTaps tp;
         memset(&tp, 0, sizeof(tp));
         for (int t = 0; t < a.L + 11; ++t) tp.wp[t] = ctx->h_taps[t];
+        for (int t = 0; t < 135; ++t) tp.wq[t] = tp.wp[t + 1];
         if (a.rebin) {
             if (ctx->bins_cap < (size_t)nb) {
                 if (ctx->d_bins) cudaFree(ctx->d_bins);
