@@ -297,7 +297,7 @@ def bench_ours(args) -> dict:
                               "note": "S5 and the flux PDF in one pass (replaces flux + flux_pdf: 12 B/pixel)"},
             "flux_power_rows": {"ms": t_pow, "bytes": int(4 * n_cells), "gbs": 4 * n_cells / t_pow / 1e6,
                                 "frac_hbm": 4 * n_cells / t_pow / 1e6 / pk["hbm_gbs"],
-                                "note": "radix-2 FFT in shared memory: shared-memory bound, not HBM bound"}}
+                                "note": "Stockham radix-16/8/4 FFT in shared memory: instruction- and shared-memory-bound, not HBM-bound"}}
         del noise, obs_out
         # delta_b and v_x from a DM field (here: the workload's delta) -- one R2C, two k-space
         # kernels, two C2R; the FFTs are cuFFT's

@@ -9,7 +9,8 @@
 // scatters the result to the other shared-memory buffer, whose index is padded by one slot in 16 so that the
 // stride-R scatter of the first pass is bank-conflict free.  |X|^2 is accumulated in double per CTA and added
 // to the global accumulator once at the end.  4 B read per pixel; N = 1024 makes 3 passes = 2 shared-memory
-// round trips per point (the radix-2 version this replaces made 10, with a barrier each).
+// round trips per point (the radix-2 version this replaces made 10, with a barrier each).  The butterflies'
+// complex additions are packed FP32 (add/sub.rn.f32x2) for rows of 512 pixels and more.
 #include "lya_internal.h"
 
 namespace {
@@ -25,10 +26,33 @@ struct PowArgs {
 
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 __device__ __forceinline__ int pad16(int i) { return i + (i >> 4); }
+// complex add / subtract as one packed FP32 instruction each (sm_100a add/sub.rn.f32x2 = FADD2)
+__device__ __forceinline__ float2 cadd(float2 a, float2 b)
+{
+    unsigned long long x, y, r;
+    float2 o;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(x) : "f"(a.x), "f"(a.y));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(y) : "f"(b.x), "f"(b.y));
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(x), "l"(y));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(o.x), "=f"(o.y) : "l"(r));
+    return o;
+}
+__device__ __forceinline__ float2 csub(float2 a, float2 b)
+{
+    unsigned long long x, y, r;
+    float2 o;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(x) : "f"(a.x), "f"(a.y));
+    asm("mov.b64 %0, {%1, %2};" : "=l"(y) : "f"(b.x), "f"(b.y));
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(x), "l"(y));
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(o.x), "=f"(o.y) : "l"(r));
+    return o;
+}
 
 // R-point DFT in registers, radix-2 decimation in frequency: the result for frequency t ends up in
 // v[bitrev_R(t)].  All indices and twiddles are compile-time constants once unrolled.
-template <int R>
+// PACK: butterflies' complex add / subtract as FADD2 (measured: 1024-pixel rows 1.654 -> 1.580 ms, 256-pixel rows
+// 2.5 % slower, so only rows of 512 pixels and more take it).
+template <int R, bool PACK>
 __device__ __forceinline__ void dft_regs(float2 (&v)[R])
 {
     constexpr float C[8] = {1.0f, 0.92387953251128674f, 0.70710678118654752f, 0.38268343236508977f,
@@ -43,8 +67,8 @@ __device__ __forceinline__ void dft_regs(float2 (&v)[R])
 #pragma unroll
             for (int p = 0; p < half; ++p) {
                 const float2 a = v[s + p], b = v[s + p + half];
-                v[s + p] = make_float2(a.x + b.x, a.y + b.y);
-                const float2 d = make_float2(a.x - b.x, a.y - b.y);
+                v[s + p] = PACK ? cadd(a, b) : make_float2(a.x + b.x, a.y + b.y);
+                const float2 d = PACK ? csub(a, b) : make_float2(a.x - b.x, a.y - b.y);
                 const int q = p * (16 / len);              // W_len^p = exp(-2 pi i q / 16), q < 8
                 if (q == 0)      v[s + p + half] = d;
                 else if (q == 4) v[s + p + half] = make_float2(d.y, -d.x);          // times -i
@@ -106,7 +130,7 @@ __device__ __forceinline__ void stockham_pass(const PowArgs &a, const float *ra,
 #pragma unroll
             for (int t = 1; t < R; ++t) v[t] = cmul(v[t], w[t]);
         }
-        dft_regs<R>(v);
+        dft_regs<R, (N_CT == 0 || N_CT >= 512)>(v);
         float2 *ob = out + pad16((j - k) * R + k);
         if (ns == 2 || ns == 4) {                         // never produced by the plans (radices 16 / 8 first)
 #pragma unroll
