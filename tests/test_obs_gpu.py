@@ -59,7 +59,9 @@ def test_observe_rows_parity(ctx, obs, flux_rows, fwhm, dlam, snr):
     assert err < 1e-5, f"observed flux max abs err {err:.2e}"
 
 
-@pytest.mark.parametrize("n,fwhm", [(5, 3.0), (13, 40.0), (100, 9.0), (257, 300.0), (1000, 55.0), (2048, 100.0), (3000, 30.0), (4096, 224.0)])
+# (512, 30.0) and (1024, 53.5): 25 and 41 tap slots, the packed-FP32 (FFMA2) convolution up to its last
+# instantiation; (1000, 55.0) is the first size past it (scalar FFMA)
+@pytest.mark.parametrize("n,fwhm", [(5, 3.0), (13, 40.0), (100, 9.0), (257, 300.0), (512, 30.0), (1024, 53.5), (1000, 55.0), (2048, 100.0), (3000, 30.0), (4096, 224.0)])
 def test_observe_rows_ragged_and_wide_kernels(ctx, obs, n, fwhm):
     """Ragged row lengths, a Gaussian as wide as the row (every nearest image contributes), bins that do not
     divide the row."""
