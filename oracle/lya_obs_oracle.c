@@ -15,8 +15,9 @@
  * direct O(N^2) DFT.  Readings: O1 the Gaussian is circular (nearest periodic image) and
  * normalised by the discrete sum of its weights; O2 a pixel is the velocity interval [i dv, (i+1) dv) and
  * "resample" is the flux-conserving overlap-weighted mean onto bins [m B, (m+1) B), m < floor(V/B); O3 the
- * noise is N(0,1)/(S/N) relative to the continuum F = 1, its N(0,1) draws passed in; O4 fluxes outside the
- * PDF range fall into the first / last bin, the bin decision is taken in fp32 as the kernel takes it; O5 the
+ * noise is N(0,1)/(S/N) relative to the continuum F = 1, its N(0,1) draws passed in; O4 the PDF bins
+ * are the paper's real-number intervals [f_lo + b dF, f_lo + (b+1) dF), decided in double against the edges;
+ * fluxes outside the range fall into the first / last bin; O5 the
  * power is P(k_m) = (V/N^2) <|sum_i dF_i exp(-2 pi i m i / N)|^2> with dF = F/<F> - 1, k_m = 2 pi m / V.
  *
  * Pins (tests/test_obs_oracle_pins.py): constant in -> constant out; a single spike -> the normalised Gaussian;
@@ -96,23 +97,31 @@ int obs_add_noise(size_t n, double snr, const double *Fb, const float *unit_nois
     return 0;
 }
 
-/* O4.  counts[b] over the fp32 fluxes; bin = floor((F - f_lo) * (1/width)) in fp32 (the kernel's precision,
- * this file is compiled with -ffp-contract=off so the two roundings are the kernel's), clamped to
- * [0, n_bins-1]; pdf[b] = counts[b] / (n * width).  NaN goes to bin 0. */
+/* O4.  The paper's bins are real-number intervals: "21 equally spaced flux bins of width dF = 0.05 ... the first
+ * data point contains flux from -0.025 <= F < 0.025", i.e. bin b = [e_b, e_{b+1}) with the lower
+ * edge inclusive, e_b = f_lo + b width.  Each fp32 flux is promoted to double (exact) and compared with the
+ * edges e_b = fma(b, width, f_lo): the correctly rounded double of f_lo + b width.  Rounding an edge is monotone,
+ * so "F >= e_b" here equals the real-number comparison for every fp32 F except an F that IS the rounded edge;
+ * for the paper's bins the rounded edges are the correctly rounded (2b-1)/40 -- exactly 0.125, 0.375, 0.625,
+ * 0.875 where those are dyadic -- which tests/test_obs_oracle_pins.py pins.  The bin is found by counting edges,
+ * no arithmetic on F.  Fluxes below the first / above the last edge fall into the first / last bin; NaN compares
+ * false with every edge and goes to bin 0.  pdf[b] = counts[b] / (n width). */
 int obs_flux_pdf(const float *F, size_t n, int32_t n_bins, double f_lo, double width, uint64_t *counts, double *pdf)
 {
     if (!F || n_bins < 1 || !(width > 0.0) || !counts || !pdf) return 1;
-    const float lo = (float)f_lo, iw = (float)(1.0 / width);
     for (int32_t b = 0; b < n_bins; ++b) counts[b] = 0;
     for (size_t i = 0; i < n; ++i) {
-        const float d = F[i] - lo;
-        const float t = floorf(d * iw);
-        int32_t b = (t >= (float)n_bins) ? n_bins - 1 : (t > 0.0f ? (int32_t)t : 0);
+        const double f = (double)F[i];
+        int32_t b = 0;
+        while (b + 1 < n_bins && f >= fma((double)(b + 1), width, f_lo)) ++b;
         counts[b] += 1;
     }
     for (int32_t b = 0; b < n_bins; ++b) pdf[b] = n ? (double)counts[b] / ((double)n * width) : 0.0;
     return 0;
 }
+
+/* the edge e_b itself, for the pins */
+double obs_flux_pdf_edge(int32_t b, double f_lo, double width) { return fma((double)b, width, f_lo); }
 
 /* O5.  P[m], m = 0 .. n_pix/2, by direct summation of the DFT of dF = F/mean_flux - 1, averaged over rows. */
 int obs_flux_power(int32_t n_pix, size_t n_rows, double dv_kms, const double *F, double mean_flux, double *P)

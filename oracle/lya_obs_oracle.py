@@ -40,6 +40,8 @@ def lib():
         L.obs_add_noise.argtypes = [C.c_size_t, C.c_double, dp, fp, dp]
         L.obs_flux_pdf.argtypes = [fp, C.c_size_t, C.c_int32, C.c_double, C.c_double,
                                    C.POINTER(C.c_uint64), dp]
+        L.obs_flux_pdf_edge.argtypes = [C.c_int32, C.c_double, C.c_double]
+        L.obs_flux_pdf_edge.restype = C.c_double
         L.obs_flux_power.argtypes = [C.c_int32, C.c_size_t, C.c_double, dp, C.c_double, dp]
         _lib = L
     return _lib
@@ -103,6 +105,11 @@ def flux_pdf(F, nbins: int = 21, f_lo: float = -0.025, width: float = 0.05):
                             _p(pdf, C.c_double))
     assert rc == 0
     return counts, pdf
+
+
+def flux_pdf_edge(b: int, f_lo: float = -0.025, width: float = 0.05) -> float:
+    """Lower edge of bin b as the oracle compares against it."""
+    return float(lib().obs_flux_pdf_edge(b, f_lo, width))
 
 
 def flux_power(F, dv_kms: float, mean_flux: float) -> np.ndarray:

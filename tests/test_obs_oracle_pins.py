@@ -114,6 +114,77 @@ def test_pdf_of_uniform_fluxes_is_flat(obs):
     assert pdf[0] == pytest.approx(0.5, rel=5e-3) and pdf[20] == pytest.approx(0.5, rel=5e-3)   # half bins
 
 
+def _exact_bin(f32, n_bins=21, lo=(-1, 40), width=(1, 20)):
+    """Bin of one fp32 flux by EXACT rational arithmetic against the paper's real edges (2b-1)/40."""
+    from fractions import Fraction
+    f = float(f32)
+    if f != f:
+        return 0
+    if f in (float("inf"), float("-inf")):
+        return n_bins - 1 if f > 0 else 0
+    x, b = Fraction(f), 0
+    while b + 1 < n_bins and x >= Fraction(*lo) + (b + 1) * Fraction(*width):
+        b += 1
+    return b
+
+
+def test_pdf_edges_are_the_papers_real_edges(obs):
+    """bins of width 0.05 starting at -0.025, i.e. real edges (2b-1)/40.  The oracle's edges (built
+    from the doubles nearest -0.025 and 0.05) must sit within 2^-52 of them -- six orders of magnitude closer
+    than any fp32 flux that is not the edge itself can come (>= 2^-32 away from a non-dyadic edge here) -- and the
+    four edges an fp32 flux CAN equal, the dyadic 0.125, 0.375, 0.625, 0.875, must be exact."""
+    from fractions import Fraction
+    for b in range(0, 22):
+        e = obs.flux_pdf_edge(b)
+        exact = Fraction(2 * b - 1, 40)
+        assert abs(Fraction(e) - exact) <= Fraction(1, 2 ** 52)
+        f32 = Fraction(float(np.float32(float(exact))))                 # nearest fp32 to the real edge
+        assert f32 == exact or abs(f32 - exact) >= Fraction(1, 2 ** 32)
+    assert [obs.flux_pdf_edge(b) for b in (3, 8, 13, 18)] == [0.125, 0.375, 0.625, 0.875]
+
+
+def test_pdf_decisions_at_every_edge_and_its_fp32_neighbours(obs):
+    """Fluxes AT each of the 20 interior edges' nearest fp32 and one ulp either side, judged by exact rational
+    comparison with the real edges (lower edge inclusive: "-0.025 <= F < 0.025"), plus values
+    outside the range, infinities and NaN.  A bin decision taken in fp32 arithmetic fails this pin."""
+    vals = []
+    for b in range(1, 21):
+        e = np.float32((2 * b - 1) / 40.0)
+        vals += [np.nextafter(e, np.float32(-9)), e, np.nextafter(e, np.float32(9))]
+    vals += [np.float32(x) for x in (-0.025, -0.0250001, 1.025, 1.0250001, -3.0, 7.0, 0.0, 1.0)]
+    vals += [np.float32("inf"), np.float32("-inf"), np.float32("nan")]
+    F = np.array(vals, dtype=np.float32)
+    expect = np.zeros(21, dtype=np.uint64)
+    for f in F:
+        expect[_exact_bin(f)] += 1
+    counts, pdf = obs.flux_pdf(F)
+    assert np.array_equal(counts, expect)
+    # each value on its own too (a compensating pair of errors cannot hide)
+    for f in F:
+        c, _ = obs.flux_pdf(np.array([f], dtype=np.float32))
+        assert c[_exact_bin(f)] == 1, float(f)
+    # the dyadic edges are inclusive lower edges
+    for b, e in ((3, 0.125), (8, 0.375), (13, 0.625), (18, 0.875)):
+        assert obs.flux_pdf(np.array([e], dtype=np.float32))[0][b] == 1
+        assert obs.flux_pdf(np.array([np.nextafter(np.float32(e), np.float32(0))]))[0][b - 1] == 1
+
+
+def test_pdf_general_bins_against_exact_rationals(obs):
+    """Other (n_bins, f_lo, width): random fp32 fluxes, exact rational bins of the given doubles' real values --
+    the oracle's fma-rounded edge can differ from the real one only for an F that equals the rounded edge."""
+    from fractions import Fraction
+    rng = np.random.default_rng(156)
+    F = rng.uniform(-0.7, 1.7, 4000).astype(np.float32)
+    for nb, lo, w in ((100, -0.5, 0.02), (40, 0.0, 0.025), (7, 0.1, 0.13)):
+        expect = np.zeros(nb, dtype=np.uint64)
+        for f in F:
+            x, b = Fraction(float(f)), 0
+            while b + 1 < nb and x >= Fraction(lo) + (b + 1) * Fraction(w):
+                b += 1
+            expect[b] += 1
+        assert np.array_equal(obs.flux_pdf(F, nb, lo, w)[0], expect)
+
+
 # ---------------------------------------------------------------- 1D power
 def test_power_of_one_cosine_mode(obs):
     n, dv, m0, eps, fbar = 64, 3.0, 5, 0.2, 0.7
