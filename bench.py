@@ -3,11 +3,14 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--cfg C] [--impl ours|reference]
 
-A step is one pass of the whole hot path over one synthetic grid.  Default workload: BASELINE.json
-configs[1] (256^3, 65,536 sightlines x 256 px, fp32).  `value` = tau pixel-pair evaluations per second
-over the whole step, inputs resident in HBM; `e2e` = the same through lya_forest_host with pinned HOST buffers
-(H2D of delta and v_pec, D2H of F inside the timed region).  N > 1 (torchrun): every rank owns a z-slab of
-256 planes of an N*256-plane grid (weak scaling); the only exchange is S4's all-reduce of five doubles per pass.
+A step is one pass of the whole hot path over one synthetic grid.  Default workload: the LARGEST single-GPU
+configuration of BASELINE.json that this box can hold -- configs[4] (2048^3, 4.19M sightlines x 2048 px, processed
+in 64-plane z-slabs with delta, v_pec and tau resident: 96 GiB of HBM, and 96 GiB of pinned host memory for the
+e2e leg), else configs[3] (1024^3); `--cfg` picks any of the five.  `value` = tau pixel-pair evaluations per second
+over the whole step, inputs resident in HBM; `e2e` = the same through lya_forest_host with pinned HOST buffers (H2D
+of delta and v_pec, D2H of F inside the timed region).  N > 1 (torchrun): every rank owns its own seeded grid of
+complete x-rows (weak scaling: slabs of one N-times-taller grid); the only exchange is S4's all-reduce of five
+doubles per pass, in the resident leg and in the e2e leg alike (one GLOBAL A).
 `--impl reference` times the CPU oracle (oracle/, as it stands) on a bounded sample of the same workload.
 """
 from __future__ import annotations
@@ -33,9 +36,29 @@ from paper_1105_4747_b200.workloads import WORKLOADS, Workload
 METRIC = "tau_pixel_pair_evals_per_s"
 UNIT = "pair-evals/s"
 SM_COUNT_B200, MUFU_PER_CLK_SM = 148, 16          # MUFU.EX2 results / clk / SM
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE tau-kernel launch (x pass), from the committed
-# `ncu --set full` captures in profiles/r1_ncu_full_final.md; algorithmic traffic is 16 B per cell
-TAU_TRAFFIC_BYTES = {2: 201.476864e6 + 35.543552e6, 3: 1.611410e9 + 0.504592e9}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE tau-kernel launch in this bench's launch shape, copied from the
+# committed `ncu --set full` captures named beside each figure (NOT measured in this run: a number printed under a
+# profiler is never a bench value, so the capture is a separate command).  Algorithmic traffic is 16 B per cell.
+TAU_TRAFFIC = {
+    2: (201.476864e6 + 35.543552e6, "profiles/r1_ncu_full_final.md"),
+    3: (1.611410e9 + 0.504592e9, "profiles/r1_ncu_full_final.md"),
+}
+
+
+def default_cfg() -> int:
+    """Largest single-GPU config this box holds: 5 needs ~105 GiB of HBM and, for the e2e leg, 96 GiB of pinned host
+    memory; otherwise 4.  Both arms (ours / reference) call this, so they name the same workload."""
+    try:
+        import psutil
+        world = int(os.environ.get("WORLD_SIZE", "1"))
+        host_ok = psutil.virtual_memory().available >= (100 * world + 30) * 2 ** 30
+    except Exception:
+        host_ok = False
+    gpu_ok = False
+    if torch.cuda.is_available():
+        free, total = torch.cuda.mem_get_info(int(os.environ.get("LOCAL_RANK", "0")))
+        gpu_ok = free >= 120 * 2 ** 30
+    return 5 if (host_ok and gpu_ok) else 4
 
 
 def peaks() -> dict:
@@ -115,8 +138,16 @@ def bench_ours(args) -> dict:
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if world > 1:
+        os.environ.setdefault("NCCL_DEBUG", "INFO")            # communicator lines stay on: the driver counts ranks
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     torch.cuda.set_device(local)
+    if args.cfg is None:
+        args.cfg = default_cfg()
+        if world > 1:                                          # every rank must run the same workload
+            c = torch.tensor([args.cfg], device="cuda")
+            dist.all_reduce(c, op=dist.ReduceOp.MIN)
+            args.cfg = int(c.item())
     w: Workload = WORKLOADS[args.cfg]
     n = w.n
     pk = peaks()
@@ -143,6 +174,9 @@ def bench_ours(args) -> dict:
     ctx = lya.Context(local)
     n_hi, b = (torch.empty((slab_nz, n, n), dtype=torch.float32, device="cuda") for _ in range(2))
     tau = torch.empty_like(delta)
+    # per-sightline plain moments of tau, written by the tau kernels' epilogue: S4's first pass reads these 40 B per
+    # sightline instead of tau (lya_tau_sightlines_opt row_moments / lya_normalize_mean_flux_rows)
+    rowm = torch.empty((n * n, 5), dtype=torch.float64, device="cuda")
     flux = tau if w.cfg == 5 else torch.empty_like(delta)
     n_cells = delta.numel()
     n_slabs = n // slab_nz
@@ -172,13 +206,16 @@ def bench_ours(args) -> dict:
                 run = timed if sl == 0 else (lambda name, fn: fn())
                 if k == 0 or n_slabs > 1:
                     run("gas", lambda: ctx.gas_from_density(p, delta[z0:z1], n_hi, b))
-                run("tau", lambda: ctx.tau_sightlines(p, ax, n_hi, b, vels[k][z0:z1], tau[z0:z1]))
+                # sightline index of the moments: axis 0 iz n + iy, axis 1 iz n + ix (slabs are whole planes); axis 2
+                # needs the whole grid (one slab)
+                run("tau", lambda: ctx.tau_sightlines_opt(p, ax, vels[k][z0:z1], n_hi=n_hi, b_kms=b, tau=tau[z0:z1],
+                                                          row_moments=rowm[z0 * n:z1 * n]))
             if world == 1:
                 A, f, it, _ = timed("normalize", lambda: ctx.normalize_mean_flux(tau, w.f_target, rel_tol=1e-7,
-                                                                                 max_iter=60))
+                                                                                 max_iter=60, row_moments=rowm))
             else:
                 A, f, it = timed("normalize", lambda: lya.normalize_mean_flux_sharded(
-                    ctx, tau, w.f_target, n_cells * world, rel_tol=1e-7))
+                    ctx, tau, w.f_target, n_cells * world, rel_tol=1e-7, row_moments=rowm))
             timed("flux", lambda: ctx.flux(tau, A, flux))
             results.update(A=A, f=f, passes=it)
         if timers is not None:
@@ -239,12 +276,15 @@ def bench_ours(args) -> dict:
     if not args.no_next:
         tau_variants = {}
         z1 = slab_nz
+        ctx.gas_from_density(p, delta[:z1], n_hi, b)
+        full = ctx.tau_sightlines(p, w.axes[0], n_hi, b, vels[0][:z1]).clone()      # the full sum of this slab
         for name, kw in (("fused_gas", dict(delta=delta[:z1])),
                          ("windowed", dict(n_hi=n_hi, b_kms=b, windowed=True)),
                          ("windowed_fused_gas", dict(delta=delta[:z1], windowed=True))):
             if "n_hi" in kw:
                 ctx.gas_from_density(p, delta[:z1], n_hi, b)
             _, pairs_ev = ctx.tau_sightlines_opt(p, w.axes[0], vels[0][:z1], tau=tau[:z1], count_pairs=True, **kw)
+            same = bool(torch.equal(tau[:z1], full))                                # measured, every pixel of the slab
             spans = []
             for _ in range(4):
                 flush.zero_()
@@ -258,13 +298,26 @@ def bench_ours(args) -> dict:
             tau_variants[name] = {"ms": ms, "sightline_pixels_per_s": slab_nz * n * n / (ms * 1e-3),
                                   "pairs_evaluated": pairs_ev, "pairs_fraction_of_full": pairs_ev / (float(slab_nz) * n ** 3),
                                   "pair_evals_per_s": pairs_ev / (ms * 1e-3),
-                                  "bit_identical_to_full_sum": True}
+                                  "bit_identical_to_full_sum": same}
+        del full
 
     # ---- the rows after F, timed per kernel on this workload's F; not part of `value`
     next_rows = None
-    if not args.no_next and w.cfg != 5 and (n & (n - 1)) == 0:
+    if not args.no_next and (n & (n - 1)) == 0:
         dv = lya.scalars(p, 0)["dv_kms"]
-        Frows = flux.reshape(-1, n)
+        # config 5 keeps F in tau's storage and the variants above overwrote its first slab: rebuild tau and F of the
+        # first 256 planes (1.07e9 pixels, as many as the whole of config 4) and time the rows after F on those
+        nr_z = n if w.cfg != 5 else 256
+        if w.cfg == 5:
+            for z0 in range(0, nr_z, slab_nz):
+                ctx.gas_from_density(p, delta[z0:z0 + slab_nz], n_hi, b)
+                ctx.tau_sightlines(p, w.axes[0], n_hi, b, vels[0][z0:z0 + slab_nz], tau[z0:z0 + slab_nz])
+            tau_nr = tau[:nr_z]
+            flux_nr = ctx.flux(tau_nr, results["A"])
+        else:
+            tau_nr, flux_nr = tau, flux
+        nr_cells = flux_nr.numel()
+        Frows = flux_nr.reshape(-1, n)
         bin_kms = lya.bin_kms_from_angstrom(w.z, 1.0375)                   # BOSS-like instrument
         nb = lya.lib().lya_instrument_bins(n, dv, lya.C.byref(lya.CInstrument(224.0, bin_kms, 5.0)))
         noise = torch.randn((Frows.shape[0], nb), device="cuda")
@@ -283,22 +336,21 @@ def bench_ours(args) -> dict:
             return sum(spans[1:]) / reps
 
         t_obs = timed_ms(lambda: ctx.observe_rows(Frows, dv, 224.0, bin_kms, 5.0, noise, obs_out))
-        t_pdf = timed_ms(lambda: ctx.flux_pdf(flux))
+        t_pdf = timed_ms(lambda: ctx.flux_pdf(flux_nr))
         t_pow = timed_ms(lambda: ctx.flux_power_rows(Frows, dv, results["f"]))
-        t_fpdf = timed_ms(lambda: ctx.flux_with_pdf(tau, results["A"], out=flux)) if flux is not tau else None
-        b_obs = 4 * n_cells + 8 * obs_out.numel()
+        t_fpdf = timed_ms(lambda: ctx.flux_with_pdf(tau_nr, results["A"], out=flux_nr))
+        b_obs = 4 * nr_cells + 8 * obs_out.numel()
+        row = lambda ms, nbytes, **kw: {"ms": ms, "bytes": int(nbytes), "gbs": nbytes / ms / 1e6,
+                                        "frac_hbm": nbytes / ms / 1e6 / pk["hbm_gbs"], **kw}
         next_rows = {
-            "observe_rows": {"instrument": "FWHM 224 km/s, 1.0375 A bins, S/N 5 (PAPER.md:130)", "bins_per_row": int(nb),
-                             "ms": t_obs, "bytes": int(b_obs), "gbs": b_obs / t_obs / 1e6, "frac_hbm": b_obs / t_obs / 1e6 / pk["hbm_gbs"]},
-            "flux_pdf": {"ms": t_pdf, "bytes": int(4 * n_cells), "gbs": 4 * n_cells / t_pdf / 1e6,
-                         "frac_hbm": 4 * n_cells / t_pdf / 1e6 / pk["hbm_gbs"]},
-            "flux_with_pdf": {"ms": t_fpdf, "bytes": int(8 * n_cells), "gbs": 8 * n_cells / t_fpdf / 1e6,
-                              "frac_hbm": 8 * n_cells / t_fpdf / 1e6 / pk["hbm_gbs"],
-                              "note": "S5 and the flux PDF in one pass (replaces flux + flux_pdf: 12 B/pixel)"},
-            "flux_power_rows": {"ms": t_pow, "bytes": int(4 * n_cells), "gbs": 4 * n_cells / t_pow / 1e6,
-                                "frac_hbm": 4 * n_cells / t_pow / 1e6 / pk["hbm_gbs"],
-                                "note": "Stockham radix-16/8/4 FFT in shared memory: instruction- and shared-memory-bound, not HBM-bound"}}
+            "on": f"{Frows.shape[0]} rows of {n} pixels" + (" (the first 256 planes)" if w.cfg == 5 else ""),
+            "observe_rows": row(t_obs, b_obs, instrument="FWHM 224 km/s, 1.0375 A bins, S/N 5 (PAPER.md:130)", bins_per_row=int(nb)),
+            "flux_pdf": row(t_pdf, 4 * nr_cells),
+            "flux_with_pdf": row(t_fpdf, 8 * nr_cells, note="S5 and the flux PDF in one pass (replaces flux + flux_pdf: 12 B/pixel)"),
+            "flux_power_rows": row(t_pow, 4 * nr_cells, note="Stockham FFT in shared memory: instruction- and shared-memory-bound, not HBM-bound")}
         del noise, obs_out
+        if w.cfg == 5:
+            del flux_nr, Frows, tau_nr
         # delta_b and v_x from a DM field (here: the workload's delta) -- one R2C, two k-space
         # kernels, two C2R; the FFTs are cuFFT's
         if w.cfg <= 3 or args.fields:
@@ -316,40 +368,67 @@ def bench_ours(args) -> dict:
     e2e = None
     if not args.no_e2e:
         pinned = lambda src: torch.empty(src.shape, dtype=src.dtype, pin_memory=True).copy_(src)
-        dh = pinned(delta)
-        vh = [pinned(v) for v in vels]
-        fh = torch.empty(dh.shape, dtype=dh.dtype, pin_memory=True)
+        try:
+            dh = pinned(delta)
+            vh = [pinned(v) for v in vels]
+            fh = torch.empty(dh.shape, dtype=dh.dtype, pin_memory=True)
+        except RuntimeError as exc:                     # the host cannot pin 3 grids: say so instead of dying
+            e2e = {"unavailable": "pinned host allocation failed: " + str(exc).splitlines()[0]}
+            args.no_e2e = True
+    if not args.no_e2e:
         if w.cfg == 5:                                  # lya_forest_host keeps its own tau + slab workspace
-            del delta, vels, tau, flux, n_hi, b
+            del delta, vels, tau, flux, n_hi, b, rowm
             torch.cuda.empty_cache()
-        for _ in range(1 if w.cfg == 5 else 2):
-            ctx.forest_host(p, w.axes[0], dh, vh[0], w.f_target, flux_h=fh)
+        n_pix_global = n_cells * world
+
+        def e2e_step():
+            for k, ax in enumerate(w.axes):
+                if world == 1:
+                    ctx.forest_host(p, ax, dh, vh[k], w.f_target, flux_h=fh)
+                else:                                   # one GLOBAL A over all ranks' pixels
+                    lya.forest_host_sharded(ctx, p, ax, dh, vh[k], w.f_target, n_pix_global, flux_h=fh)
+
+        t0 = time.perf_counter()
+        e2e_step()                                      # warm-up (allocates the workspace); also sizes the leg
+        torch.cuda.synchronize()
+        est = time.perf_counter() - t0
+        if w.cfg != 5:
+            e2e_step()
+        # every step moves the whole grid over PCIe: at most ~40 s of them, never fewer than 2 (the count is reported)
+        e2e_steps = max(2, min(args.steps, int(40.0 / max(est, 1e-3))))
         if world > 1:
+            c = torch.tensor([e2e_steps], device="cuda")
+            dist.all_reduce(c, op=dist.ReduceOp.MIN)
+            e2e_steps = int(c.item())
             dist.barrier()
         torch.cuda.synchronize()
         t0 = time.perf_counter()
-        for _ in range(args.steps):
-            for k, ax in enumerate(w.axes):
-                ctx.forest_host(p, ax, dh, vh[k], w.f_target, flux_h=fh)
+        for _ in range(e2e_steps):
+            e2e_step()
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
         if world > 1:
             tt = torch.tensor([dt], dtype=torch.float64, device="cuda")
             dist.all_reduce(tt, op=dist.ReduceOp.MAX)
             dt = float(tt.item())
-        e2e = {"value": pairs_per_step * args.steps / dt, "unit": UNIT,
+        e2e = {"value": pairs_per_step * e2e_steps / dt, "unit": UNIT,
                "h2d_bytes_per_step": int(2 * 4 * n_cells * n_ax), "d2h_bytes_per_step": int(4 * n_cells * n_ax),
-               "ms_per_step": 1e3 * dt / args.steps,
-               "note": "lya_forest_host: S1 is recomputed per axis pass; multi-rank runs normalise per rank here"}
+               "ms_per_step": 1e3 * dt / e2e_steps, "steps": e2e_steps,
+               "note": "lya_forest_host from pinned host buffers (S1 fused into S3 per axis pass), F copied back; "
+                       "bytes are per rank" + ("; S4 all-reduced over ranks: one global A" if world > 1 else "")}
+        del dh, vh, fh
     sampler.stop()
 
     clocks = sampler.summary(pk["sm_max_mhz"])
     mufu_measured = ctx.measure_mufu_peak()                                   # pure ex2 micro-kernel, this device
+    torch.cuda.empty_cache()
+    hbm_own = ctx.measure_hbm_peak(1 << 32)                                   # the library's own streaming copy, 4 GiB
     f_peak = MUFU_PER_CLK_SM * ctx.sm_count * pk["sm_max_mhz"] * 1e6          # pair-evals/s at max SM clock
     tau_rate = float(slab_cells) * n / (k_ms["tau"] * 1e-3)      # pairs of one launch / its duration
     hbm = pk["hbm_gbs"]
     gbs = lambda bytes_, ms: bytes_ / (ms * 1e-3) / 1e9
     passes = results["passes"]
+    norm_bytes = 4 * n_cells * (passes - 1) + 40 * n * n
     out = {
         "metric": METRIC, "value": pairs_per_step / (ms_per_step * 1e-3), "unit": UNIT,
         "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step,
@@ -364,19 +443,27 @@ def bench_ours(args) -> dict:
         "A": results["A"], "mean_flux": results["f"], "normalize_passes": passes,
         "kernel_ms": k_ms, "wall_s_timed_region_incl_flush": wall,
         "roofline": {"bound": "alu", "kernel": "tau_kernel", "achieved": tau_rate / 1e9, "peak": f_peak / 1e9,
-                     "unit": "Gpair-evals/s", "frac": tau_rate / f_peak, "traffic": TAU_TRAFFIC_BYTES.get(w.cfg),
-                     "traffic_unit": "bytes per launch (ncu dram read+write, profiles/r1_ncu_full_final.md); algorithmic %d" % (16 * n_cells),
+                     "unit": "Gpair-evals/s", "frac": tau_rate / f_peak,
+                     "traffic": TAU_TRAFFIC[w.cfg][0] if w.cfg in TAU_TRAFFIC else None,
+                     "traffic_src": ("ncu dram__bytes_read.sum + dram__bytes_write.sum of one launch, copied from "
+                                     + TAU_TRAFFIC[w.cfg][1] + " (a separate run under ncu, not this one)")
+                                    if w.cfg in TAU_TRAFFIC else None,
+                     "traffic_algorithmic": 16 * slab_cells, "launch": "%d planes of %d x %d" % (slab_nz, n, n),
                      "peak_measured": mufu_measured / 1e9, "frac_of_measured_peak": tau_rate / mufu_measured,
                      "peak_def": "16 MUFU.EX2/clk/SM x %d SMs x %.0f MHz (max SM clock, %s)" %
                                  (ctx.sm_count, pk["sm_max_mhz"], pk["src"]),
                      "frac_at_measured_clock": (tau_rate / (MUFU_PER_CLK_SM * ctx.sm_count * clocks["sm_mhz"] * 1e6))
                      if clocks["sm_mhz"] else None},
         "roofline_hbm": {
-            "peak_gbs": hbm, "peak_src": pk["src"],
+            "peak_gbs": hbm, "peak_src": pk["src"] + " (MEASURED_PEAKS.json: torch copy_)" if pk["src"] == "measured" else pk["src"],
+            "own_copy_gbs": hbm_own, "own_copy_def": "lya_measure_hbm_peak: 128-bit streaming copy kernel, 4 GiB of traffic, best of 5",
+            "frac_def": "algorithmic bytes / event time / peak_gbs; a frac slightly above 1 means the 1:1 streaming "
+                        "pattern beats the torch copy_ the driver measured -- compare with own_copy_gbs",
             "gas": {"bytes": 12 * slab_cells, "gbs": gbs(12 * slab_cells, k_ms["gas"]), "frac": gbs(12 * slab_cells, k_ms["gas"]) / hbm},
-            "normalize": {"bytes": 4 * n_cells * passes, "passes": passes,
-                          "gbs": gbs(4 * n_cells * passes, k_ms["normalize"]),
-                          "frac": gbs(4 * n_cells * passes, k_ms["normalize"]) / hbm},
+            "normalize": {"bytes": norm_bytes, "passes": passes,
+                          "passes_def": "the first (A = 0) reads the tau kernels' per-sightline moments, 40 B per sightline; "
+                                        "the others 4 B per pixel",
+                          "gbs": gbs(norm_bytes, k_ms["normalize"]), "frac": gbs(norm_bytes, k_ms["normalize"]) / hbm},
             "flux": {"bytes": 8 * n_cells, "gbs": gbs(8 * n_cells, k_ms["flux"]), "frac": gbs(8 * n_cells, k_ms["flux"]) / hbm}},
         "clocks": clocks, "e2e": e2e, "tau_variants": tau_variants, "next_rows": next_rows, "gpu_launches": int(launches), "sm_count": ctx.sm_count,
     }
@@ -425,10 +512,12 @@ def bench_reference(args) -> dict:
     if int(os.environ.get("RANK", "0")) != 0:
         return {}
     from oracle import lya_oracle as orc
+    if args.cfg is None:
+        args.cfg = default_cfg()
     w = WORKLOADS[args.cfg]
     n = w.n
     # the same seeded fields as our arm, only the planes the sample needs (generated on the CPU)
-    nz_need = 8
+    nz_need = max(1, min(8, 2048 // n))
     f = inputs.make_fields(w, device="cpu", z0=0, z1=nz_need)
     d = f["delta"].reshape(-1, n).numpy()
     v = f["v_pec"][w.axes[0]].reshape(-1, n).numpy()
@@ -455,7 +544,8 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--cfg", type=int, default=2, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--cfg", type=int, default=None, choices=[1, 2, 3, 4, 5],
+                    help="BASELINE.json configs[cfg-1]; default: 5 if this box holds it (HBM and pinned host memory), else 4")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")

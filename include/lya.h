@@ -108,23 +108,43 @@ lya_status lya_tau_sightlines(lya_ctx *ctx, const lya_params *p, int axis, int32
  *                         cell with the arithmetic of lya_gas_from_density, so tau is bit-identical to the
  *                         two-call path); b_kms is ignored and may be NULL.
  * pairs_evaluated: HOST, receives the number of (i,j) pairs actually evaluated, or NULL; non-NULL
- * synchronises the stream. */
+ * synchronises the stream.
+ * row_moments: DEVICE, [sightlines of this call][5] doubles (8-byte aligned), or NULL: receives per sightline the
+ * plain moments sum_i tau_i^k, k = 0..4 (k = 0: the pixel count), summed in the kernels' epilogue while tau is
+ * still in registers / shared memory (fp32 within a tile of 128 pixels, double above; fixed order: reproducible).
+ * They are S4's first pass (A = 0: PAPER.md:92's mean over "all generated spectra" needs sum tau^k only) --
+ * lya_normalize_mean_flux_rows / lya_row_moment_sums -- so tau is read one time fewer.  Sightline index: axis 0
+ * iz ny + iy; axis 1 iz nx + ix; axis 2 iy nx + ix (iz local to the slab of this call). */
 #define LYA_TAU_WINDOWED     1u
 #define LYA_TAU_FROM_DENSITY 2u
 lya_status lya_tau_sightlines_opt(lya_ctx *ctx, const lya_params *p, int axis, int32_t nz_local, unsigned flags,
                                   const float *n_hi_or_delta, const float *b_kms, const float *v_pec_kms,
-                                  float *tau, uint64_t *pairs_evaluated);
+                                  float *tau, uint64_t *pairs_evaluated, double *row_moments);
 
 /* S4.  tau: DEVICE, n_pix floats in any layout (the mean runs over all of them).  Finds the unique A > 0
  * with mean(exp(-A tau)) = f_target by an iteration that runs entirely on the device (one cooperative
  * kernel): every pass over tau yields five tilted moments and a fifth-order step on ln <exp(-A tau)>,
  * safeguarded by Newton's step and a bisection bracket (3-5 passes).  Synchronises the
  * stream because A returns to the HOST.  rel_tol: stop when the step, or the truncation error of the step's
- * model, is below rel_tol * A (suggest 1e-7); max_iter passes over tau (suggest 60).  a_out, f_achieved (the
- * mean flux at A), iters (passes used): HOST, any may be NULL. */
+ * model, is below rel_tol * A (suggest 1e-7); max_iter passes over tau (suggest 60).  a_out, f_achieved, iters
+ * (passes used): HOST, any may be NULL.  f_achieved is the MODEL's value of the mean flux at the returned A (the
+ * iteration stops without a confirming pass when the quartic and cubic cumulant models agree to rel_tol / 10, so
+ * it equals f_target to that order by construction); a caller who wants the measured mean flux at A takes
+ * lya_flux_partial_sums(tau, {A}) / n_pix -- one more pass -- which the parity tests do. */
 lya_status lya_normalize_mean_flux(lya_ctx *ctx, const float *tau, size_t n_pix, double f_target,
                                    double rel_tol, int max_iter,
                                    double *a_out, double *f_achieved, int *iters);
+
+/* S4 started from the per-sightline plain moments lya_tau_sightlines_opt wrote (row_moments DEVICE [n_rows][5], over
+ * exactly the n_pix pixels of tau): the A = 0 pass reads 40 B per sightline instead of 4 B per pixel; everything
+ * else as lya_normalize_mean_flux, whose result it reproduces to the iteration's tolerance (the later passes and
+ * the final step use the tilted moments of tau itself).  row_moments == NULL and n_rows == 0: the plain call. */
+lya_status lya_normalize_mean_flux_rows(lya_ctx *ctx, const float *tau, size_t n_pix, const double *row_moments,
+                                        size_t n_rows, double f_target, double rel_tol, int max_iter,
+                                        double *a_out, double *f_achieved, int *iters);
+/* sums5[k] = sum over the n_rows sightlines of row_moments[.][k] (HOST out; synchronises): the A = 0 sums of a
+ * sharded S4 (= lya_flux_moment_sums(tau, 0) without reading tau). */
+lya_status lya_row_moment_sums(lya_ctx *ctx, const double *row_moments, size_t n_rows, double *sums5);
 
 /* Building block of S4 for slab-wise or multi-GPU normalisation: for k trial values (1 <= k <= 8) returns
  * sums[t] = sum_p exp(-a_trial[t] tau_p) and, if dsums != NULL, dsums[t] = sum_p tau_p exp(-a_trial[t] tau_p).
@@ -170,6 +190,22 @@ lya_status lya_forest_host(lya_ctx *ctx, const lya_params *p, int axis, int32_t 
                            float *tau_h, float *flux_h,
                            double *a_out, double *f_achieved, int *iters);
 
+/* The same path in three steps, for callers that own the reduction of S4 (one rank per GPU, each holding a z-slab
+ * of complete sightlines -- DESIGN.md "Multi-GPU" -- or any other outer loop over A):
+ *   lya_forest_host_begin   S1 + S3 of the local grid from HOST delta_h / v_pec_h, slab-streamed exactly as in
+ *                           lya_forest_host; tau stays resident in the ctx's device workspace (and is copied to
+ *                           tau_h, HOST, if not NULL).  Asynchronous apart from the workspace allocation.
+ *   lya_forest_moment_sums  sums5[k] = sum_p tau_p^k exp(-a_trial tau_p), k = 0..4, over the resident tau (HOST
+ *                           out; synchronises): all-reduce over ranks, then lya_root_update_moments.
+ *   lya_forest_host_finish  S5 with the given A in place on the resident tau, F streamed back to flux_h (HOST, may
+ *                           be NULL); synchronises both streams and releases the resident tau (not the workspace).
+ * LYA_EINVAL if moment_sums / finish are called with no resident tau (also after lya_fields_from_dm, which shares
+ * the workspace).  On any error no copy is left in flight on the caller's buffers. */
+lya_status lya_forest_host_begin(lya_ctx *ctx, const lya_params *p, int axis, int32_t slab_nz,
+                                 const float *delta_h, const float *v_pec_h, float *tau_h);
+lya_status lya_forest_moment_sums(lya_ctx *ctx, double a_trial, double *sums5);
+lya_status lya_forest_host_finish(lya_ctx *ctx, double a, float *flux_h);
+
 /* ---------------------------------------------------------------------------------------------------------
  * After F: the paper's instrument model and its two validation statistics.
  * Spectra are ROWS: n_rows sightlines of n_pix contiguous fp32 pixels of velocity width dv_kms (sightlines
@@ -212,7 +248,7 @@ lya_status lya_flux_with_pdf(lya_ctx *ctx, const float *tau, size_t n_pix, doubl
 
 /* 1D flux power spectrum: P(k_m) = (V/N^2) <|sum_i dF_i exp(-2 pi i m i/N)|^2> over the
  * rows, dF = F/mean_flux - 1, V = n_pix dv, k_m = 2 pi m / V [s/km], m = 0 .. n_pix/2.  n_pix must be a power
- * of two between 8 and 8192 (a radix-2 FFT per row in shared memory).  flux DEVICE [n_rows][n_pix];
+ * of two between 8 and 8192 (a Stockham radix-16/8/4 FFT of two rows at a time in shared memory).  flux DEVICE [n_rows][n_pix];
  * power HOST, n_pix/2 + 1 doubles [km/s].  Synchronises the stream. */
 lya_status lya_flux_power_rows(lya_ctx *ctx, size_t n_rows, int32_t n_pix, double dv_kms, const float *flux,
                                double mean_flux, double *power);
@@ -247,6 +283,11 @@ lya_status lya_fields_from_dm(lya_ctx *ctx, const lya_field_params *p, const flo
  * runs a pure ex2.approx micro-kernel on every SM of ctx's device and returns MUFU.EX2 results per second
  * (HOST double; best of 3 after a warm-up).  Synchronises the stream.  16 / clk / SM on B200. */
 lya_status lya_measure_mufu_peak(lya_ctx *ctx, double *ex2_per_s);
+
+/* The HBM roofline denominator measured with this library's own access pattern: a 128-bit streaming copy kernel
+ * (1 read : 1 write) over n_bytes of traffic (>= 2^20; use >> L2, e.g. 2^32).  gb_per_s: HOST, read + written bytes
+ * per second / 1e9, best of 5.  Allocates and frees n_bytes of device memory; synchronises. */
+lya_status lya_measure_hbm_peak(lya_ctx *ctx, size_t n_bytes, double *gb_per_s);
 
 /* Number of kernels the library has launched on this ctx since creation (bench.py's gpu_launches). */
 uint64_t lya_launch_count(const lya_ctx *ctx);

@@ -135,6 +135,7 @@ extern "C" lya_status lya_fields_from_dm(lya_ctx *ctx, const lya_field_params *p
 
     const int nxh = p->nx / 2 + 1;
     const size_t half = (size_t)p->nz * p->ny * nxh;
+    ctx->forest_total = 0;                               // the shared workspace no longer holds lya_forest_host_begin's tau
     lya_status st = ensure_ws(ctx, 2 * half * sizeof(float2) + 256);
     if (st != LYA_OK) return st;
     float2 *A = (float2 *)ctx->ws, *B = A + half;

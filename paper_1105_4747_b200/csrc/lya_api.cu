@@ -80,7 +80,7 @@ lya_status lya_create(lya_ctx **out, int device, void *cuda_stream)
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->coop_ok, cudaDevAttrCooperativeLaunch, device);
     const size_t part_bytes = (size_t)2 * LYA_MAX_RED_BLOCKS * 2 * LYA_MAX_TRIALS * sizeof(double);
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->d_partials, part_bytes);
-    if (e == cudaSuccess) e = cudaMallocHost((void **)&ctx->h_pinned, 64 * sizeof(double));
+    if (e == cudaSuccess) e = cudaMallocHost((void **)&ctx->h_pinned, (LYA_PINNED_STATS + LYA_STATS_DOUBLES) * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->d_stats, LYA_STATS_DOUBLES * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->d_sched, 4 * sizeof(unsigned int));
     if (e == cudaSuccess) e = cudaMemset(ctx->d_sched, 0, 4 * sizeof(unsigned int));
@@ -145,7 +145,7 @@ lya_status lya_gas_from_density(lya_ctx *ctx, const lya_params *p, const float *
 
 lya_status lya_tau_sightlines_opt(lya_ctx *ctx, const lya_params *p, int axis, int32_t nz_local, unsigned flags,
                                   const float *n_hi, const float *b_kms, const float *v_pec_kms, float *tau,
-                                  uint64_t *pairs_evaluated)
+                                  uint64_t *pairs_evaluated, double *row_moments)
 {
     if (!ctx) return LYA_EINVAL;
     ctx->err[0] = 0;
@@ -162,6 +162,7 @@ lya_status lya_tau_sightlines_opt(lya_ctx *ctx, const lya_params *p, int axis, i
         return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: pointers must be 4-byte aligned");
     if (tau == n_hi || tau == b_kms || tau == v_pec_kms)
         return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: tau may not alias an input");
+    if ((uintptr_t)row_moments & 7) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: row_moments must be 8-byte aligned");
     if (axis_len(p, axis) > (1 << 22))
         return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: more than 2^22 pixels per sightline");
     lya_scalars s;
@@ -177,7 +178,7 @@ lya_status lya_tau_sightlines_opt(lya_ctx *ctx, const lya_params *p, int axis, i
     }
     // amplitude a_j = K nHI / (b[km/s] 1e5 cm/km): K 1e-5 is passed so that fp32 operands stay O(1e11 x 1e-11)
     lya_status st = lya_launch_tau(ctx, axis, p->nx, p->ny, nz_local, n_hi, b_kms, v_pec_kms, tau, s.K * 1.0e-5,
-                                   s.dv_kms, flags, gas5, d_pairs);
+                                   s.dv_kms, flags, gas5, d_pairs, row_moments);
     if (st != LYA_OK || !pairs_evaluated) return st;
     unsigned long long host = 0;
     LYA_CUDA(ctx, cudaMemcpyAsync(&host, d_pairs, sizeof(host), cudaMemcpyDeviceToHost, ctx->stream));
@@ -189,22 +190,42 @@ lya_status lya_tau_sightlines_opt(lya_ctx *ctx, const lya_params *p, int axis, i
 lya_status lya_tau_sightlines(lya_ctx *ctx, const lya_params *p, int axis, int32_t nz_local,
                               const float *n_hi, const float *b_kms, const float *v_pec_kms, float *tau)
 {
-    return lya_tau_sightlines_opt(ctx, p, axis, nz_local, 0u, n_hi, b_kms, v_pec_kms, tau, nullptr);
+    return lya_tau_sightlines_opt(ctx, p, axis, nz_local, 0u, n_hi, b_kms, v_pec_kms, tau, nullptr, nullptr);
 }
 
-lya_status lya_normalize_mean_flux(lya_ctx *ctx, const float *tau, size_t n_pix, double f_target,
-                                   double rel_tol, int max_iter, double *a_out, double *f_achieved, int *iters)
+lya_status lya_normalize_mean_flux_rows(lya_ctx *ctx, const float *tau, size_t n_pix, const double *row_moments,
+                                        size_t n_rows, double f_target, double rel_tol, int max_iter, double *a_out,
+                                        double *f_achieved, int *iters)
 {
     if (!ctx) return LYA_EINVAL;
     ctx->err[0] = 0;
     if (n_pix == 0) return lya_fail(ctx, LYA_EINVAL, "lya_normalize_mean_flux: n_pix == 0");
     if (!tau || ((uintptr_t)tau & 3)) return lya_fail(ctx, LYA_EINVAL, "lya_normalize_mean_flux: bad tau pointer");
+    if ((row_moments != nullptr) != (n_rows > 0) || ((uintptr_t)row_moments & 7))
+        return lya_fail(ctx, LYA_EINVAL, "lya_normalize_mean_flux_rows: row_moments and n_rows go together (8-byte aligned)");
     if (!(f_target > 0.0 && f_target < 1.0))
         return lya_fail(ctx, LYA_EINVAL, "lya_normalize_mean_flux: f_target must lie in (0,1)");
     if (!(rel_tol > 0.0) || max_iter < 2)
         return lya_fail(ctx, LYA_EINVAL, "lya_normalize_mean_flux: rel_tol > 0 and max_iter >= 2 required");
     LYA_CUDA(ctx, cudaSetDevice(ctx->device));
-    return lya_run_normalize(ctx, tau, n_pix, f_target, rel_tol, max_iter, a_out, f_achieved, iters);
+    return lya_run_normalize(ctx, tau, n_pix, row_moments, n_rows, f_target, rel_tol, max_iter, a_out, f_achieved, iters);
+}
+
+lya_status lya_normalize_mean_flux(lya_ctx *ctx, const float *tau, size_t n_pix, double f_target,
+                                   double rel_tol, int max_iter, double *a_out, double *f_achieved, int *iters)
+{
+    return lya_normalize_mean_flux_rows(ctx, tau, n_pix, nullptr, 0, f_target, rel_tol, max_iter, a_out, f_achieved, iters);
+}
+
+lya_status lya_row_moment_sums(lya_ctx *ctx, const double *row_moments, size_t n_rows, double *sums5)
+{
+    if (!ctx) return LYA_EINVAL;
+    ctx->err[0] = 0;
+    if ((n_rows > 0 && (!row_moments || ((uintptr_t)row_moments & 7))) || !sums5)
+        return lya_fail(ctx, LYA_EINVAL, "lya_row_moment_sums: null or misaligned pointer");
+    if (n_rows == 0) { for (int i = 0; i < 5; ++i) sums5[i] = 0.0; return LYA_OK; }
+    LYA_CUDA(ctx, cudaSetDevice(ctx->device));
+    return lya_run_row_moment_sums(ctx, row_moments, n_rows, sums5);
 }
 
 lya_status lya_flux_partial_sums(lya_ctx *ctx, const float *tau, size_t n_pix, const double *a_trial, int k,

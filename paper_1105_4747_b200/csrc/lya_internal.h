@@ -19,8 +19,9 @@ struct lya_ctx {
     uint64_t      launches;
     // reduction scratch (device): per-block partial sums, root state
     double       *d_partials;     // [2 parities][LYA_MAX_RED_BLOCKS][2*LYA_MAX_TRIALS]
-    double       *h_pinned;       // 64 doubles of pinned host memory, written by the kernels directly (UVA)
-    unsigned int *d_sched;        // tau_x_kernel row counter {next row, groups finished}; zero between launches
+    double       *h_pinned;       // pinned host memory: [0, 64) written by the kernels directly (UVA: S4 results,
+                                  // partial sums), [LYA_PINNED_STATS, +LYA_STATS_DOUBLES) DMA target of the statistics
+    unsigned int *d_sched;        // tau kernels' work counter [0..1] (zeroed on the stream before every launch) and pair counter [2..3]
     double       *d_stats;        // 8192 doubles: flux-PDF counts (as uint64) / power-spectrum accumulators
     float        *d_taps, *h_taps; // lya_observe_rows: Gaussian taps (device / host staging), grown on demand
     size_t        taps_cap;
@@ -33,12 +34,16 @@ struct lya_ctx {
     // lya_forest_host / lya_fields_from_dm workspace (device), grown on demand
     void         *ws;
     size_t        ws_bytes;
+    double       *forest_rowm;                 // per-sightline plain moments of that tau (inside ws)
+    size_t        forest_rows;
+    size_t        forest_total, forest_slab;   // cells of the tau lya_forest_host_begin left resident in ws (0: none), chunk size
     char          err[512];
 };
 
 #define LYA_MAX_RED_BLOCKS 2048
 #define LYA_MAX_TRIALS     8
 #define LYA_STATS_DOUBLES   8192
+#define LYA_PINNED_STATS    64
 
 static inline lya_status lya_fail(lya_ctx *ctx, lya_status s, const char *msg)
 {
@@ -82,10 +87,12 @@ lya_status lya_launch_gas(lya_ctx *ctx, const float *delta, size_t n, float *n_h
 lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
                           const float *n_hi, const float *b, const float *v, float *tau,
                           double amp_scale, double dv_kms, unsigned flags, const float *gas5,
-                          unsigned long long *d_pairs);
+                          unsigned long long *d_pairs, double *d_rowm);
 lya_status lya_launch_flux(lya_ctx *ctx, const float *tau, size_t n, double a, float *flux);
-lya_status lya_run_normalize(lya_ctx *ctx, const float *tau, size_t n, double f_target, double rel_tol,
-                             int max_iter, double *a_out, double *f_out, int *iters);
+// rowm / n_rows: per-sightline plain moments of lya_tau_sightlines_opt (pass 0 reads them instead of tau) or NULL / 0
+lya_status lya_run_normalize(lya_ctx *ctx, const float *tau, size_t n, const double *rowm, size_t n_rows,
+                             double f_target, double rel_tol, int max_iter, double *a_out, double *f_out, int *iters);
+lya_status lya_run_row_moment_sums(lya_ctx *ctx, const double *rowm, size_t n_rows, double *sums5);
 lya_status lya_run_flux_with_pdf(lya_ctx *ctx, const float *tau, size_t n, double a, float *flux, int n_bins,
                                  double f_lo, double width, uint64_t *counts, double *pdf);
 lya_status lya_run_moment_sums(lya_ctx *ctx, const float *tau, size_t n, double a_trial, double *sums5);

@@ -12,6 +12,7 @@
 #include <cooperative_groups.h>
 
 #include "lya_internal.h"
+#include "pdf_bin.h"
 #include "root_iter.h"
 
 namespace cg = cooperative_groups;
@@ -167,6 +168,8 @@ __device__ __forceinline__ void block_sum(double (&v)[NV], double *sh /* [NV][wa
 struct NormArgs {
     const float *tau;
     size_t       n;
+    const double *rowm;        // per-sightline plain moments [n_rows][5] written by the tau kernels, or NULL
+    size_t       n_rows;
     double       f_target, rel_tol;
     int          max_iter;
     double      *partials;     // [2][gridDim.x][5], gridDim.x <= SM count
@@ -184,7 +187,17 @@ __global__ void __launch_bounds__(NORM_THREADS, 1) normalize_kernel(const NormAr
     for (int pass = 0;; ++pass) {
         const Trial tr = make_trial(st.a);
         double s[5];
-        accumulate_moments(a.tau, a.n, tr, s);
+        if (pass == 0 && a.rowm) {
+            // A = 0: the tilted moments are the plain moments sum tau^k, which the tau kernels left per sightline
+            // (40 B per sightline instead of 4 B per pixel); fixed thread -> row assignment, so bit-reproducible
+#pragma unroll
+            for (int k = 0; k < 5; ++k) s[k] = 0.0;
+            for (size_t r = (size_t)blockIdx.x * blockDim.x + threadIdx.x; r < a.n_rows; r += (size_t)gridDim.x * blockDim.x)
+#pragma unroll
+                for (int k = 0; k < 5; ++k) s[k] += __ldcs(a.rowm + 5 * r + k);
+        } else {
+            accumulate_moments(a.tau, a.n, tr, s);
+        }
         block_sum<5>(s, sh);
         double *part = a.partials + (size_t)(pass & 1) * gridDim.x * 5;
         if (threadIdx.x == 0)
@@ -244,6 +257,20 @@ __global__ void __launch_bounds__(RED_THREADS) moment_sums_kernel(const float *_
         for (int k = 0; k < 5; ++k) partials[(size_t)blockIdx.x * 5 + k] = s[k];
 }
 
+// per-sightline plain moments -> per-block partials (lya_row_moment_sums: the A = 0 pass of a sharded S4)
+__global__ void __launch_bounds__(RED_THREADS) row_sums_kernel(const double *__restrict__ rowm, size_t n_rows, double *partials)
+{
+    __shared__ double sh[5 * 32];
+    double s[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    for (size_t r = (size_t)blockIdx.x * blockDim.x + threadIdx.x; r < n_rows; r += (size_t)gridDim.x * blockDim.x)
+#pragma unroll
+        for (int k = 0; k < 5; ++k) s[k] += __ldcs(rowm + 5 * r + k);
+    block_sum<5>(s, sh);
+    if (threadIdx.x == 0)
+#pragma unroll
+        for (int k = 0; k < 5; ++k) partials[(size_t)blockIdx.x * 5 + k] = s[k];
+}
+
 // one block: fixed-order sum of the per-block partials -> out[0 .. nv)
 __global__ void __launch_bounds__(RED_THREADS) finish_sums_kernel(const double *partials, int n_blocks, int nv,
                                                                   double *out)
@@ -284,24 +311,23 @@ __global__ void __launch_bounds__(256) flux_kernel(const float *tau, size_t n, T
 
 // S5 and the flux PDF in one pass: F is written as by flux_kernel and binned as by
 // flux_pdf_kernel (observe.cu) -- private per-thread histograms hist[bin][thread] in shared memory, the bin
-// decision taken in fp32 with two separately rounded operations (reading O4) -- so the counts are bit-identical
-// to lya_flux followed by lya_flux_pdf, with 8 B instead of 12 B of traffic per pixel.
+// decision by pdf_bin.h's exact thresholds (reading O4) -- so the counts are bit-identical to lya_flux followed
+// by lya_flux_pdf, with 8 B instead of 12 B of traffic per pixel.
 constexpr int FPDF_THREADS = 128;
 
 __global__ void __launch_bounds__(FPDF_THREADS) flux_pdf_fused_kernel(const float *tau, size_t n, Trial tr, float *flux,
-                                                                      int n_bins, float f_lo, float inv_width,
+                                                                      const __grid_constant__ PdfEdges edges,
                                                                       unsigned long long *__restrict__ counts)
 {
-    extern __shared__ unsigned int hist[];               // [n_bins][FPDF_THREADS]
+    extern __shared__ unsigned int hist[];               // [n_bins][FPDF_THREADS], then n_bins + 1 thresholds
+    const int n_bins = edges.n_bins;
+    float *s_thr = reinterpret_cast<float *>(hist + n_bins * FPDF_THREADS);
     for (int t = threadIdx.x; t < n_bins * FPDF_THREADS; t += FPDF_THREADS) hist[t] = 0u;
+    for (int t = threadIdx.x; t <= n_bins; t += FPDF_THREADS) s_thr[t] = edges.thr[t];
     __syncthreads();
     unsigned int *mine = hist + threadIdx.x;
-    const float top = (float)n_bins;
-    auto bin = [&](float f) {
-        const float t = floorf(__fmul_rn(__fsub_rn(f, f_lo), inv_width));
-        const int b = (t >= top) ? n_bins - 1 : (t > 0.0f ? (int)t : 0);
-        mine[b * FPDF_THREADS] += 1u;
-    };
+    const float f_lo = edges.f_lo, inv_width = edges.inv_width, eps = edges.eps, ome = edges.one_minus_eps;
+    auto bin = [&](float f) { mine[lya_pdf_bin(f, s_thr, n_bins, f_lo, inv_width, eps, ome) * FPDF_THREADS] += 1u; };
     const size_t gtid = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     const size_t gsz  = (size_t)gridDim.x * blockDim.x;
     size_t head = ((16 - ((uintptr_t)tau & 15)) & 15) >> 2;
@@ -348,15 +374,15 @@ int red_grid(lya_ctx *ctx, size_t n, int per_sm)
 
 }  // namespace
 
-lya_status lya_run_normalize(lya_ctx *ctx, const float *tau, size_t n, double f_target, double rel_tol,
-                             int max_iter, double *a_out, double *f_out, int *iters)
+lya_status lya_run_normalize(lya_ctx *ctx, const float *tau, size_t n, const double *rowm, size_t n_rows,
+                             double f_target, double rel_tol, int max_iter, double *a_out, double *f_out, int *iters)
 {
     if (!ctx->coop_ok) return lya_fail(ctx, LYA_ECUDA, "device does not support cooperative launch");
     int per_sm = 0;
     LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, normalize_kernel, NORM_THREADS, 0));
     if (per_sm < 1) return lya_fail(ctx, LYA_ECUDA, "normalize_kernel: zero occupancy");
     // the four result doubles go straight to the pinned host mirror (mapped under UVA): no copy to enqueue
-    NormArgs a{tau, n, f_target, rel_tol, max_iter, ctx->d_partials, ctx->h_pinned};
+    NormArgs a{tau, n, rowm, n_rows, f_target, rel_tol, max_iter, ctx->d_partials, ctx->h_pinned};
     size_t want = (n / 4 + NORM_THREADS - 1) / NORM_THREADS;           // at least one float4 per thread
     if (want < 1) want = 1;
     const int grid = (int)(want < (size_t)ctx->sm_count ? want : (size_t)ctx->sm_count);
@@ -426,13 +452,28 @@ lya_status lya_run_moment_sums(lya_ctx *ctx, const float *tau, size_t n, double 
     return LYA_OK;
 }
 
+lya_status lya_run_row_moment_sums(lya_ctx *ctx, const double *rowm, size_t n_rows, double *sums5)
+{
+    size_t want = (n_rows + RED_THREADS - 1) / RED_THREADS, cap = (size_t)ctx->sm_count * 4;
+    const int grid = (int)(want < cap ? want : cap);
+    row_sums_kernel<<<grid, RED_THREADS, 0, ctx->stream>>>(rowm, n_rows, ctx->d_partials);
+    finish_sums_kernel<<<1, RED_THREADS, 0, ctx->stream>>>(ctx->d_partials, grid, 5, ctx->h_pinned);   // mapped pinned memory
+    ctx->launches += 2;
+    LYA_CUDA(ctx, cudaGetLastError());
+    LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    for (int i = 0; i < 5; ++i) sums5[i] = ctx->h_pinned[i];
+    return LYA_OK;
+}
+
 lya_status lya_run_flux_with_pdf(lya_ctx *ctx, const float *tau, size_t n, double a, float *flux, int n_bins,
                                  double f_lo, double width, uint64_t *counts, double *pdf)
 {
     unsigned long long *d_counts = reinterpret_cast<unsigned long long *>(ctx->d_stats);
     LYA_CUDA(ctx, cudaMemsetAsync(d_counts, 0, (size_t)n_bins * sizeof(unsigned long long), ctx->stream));
     if (n > 0) {
-        const size_t smem = (size_t)n_bins * FPDF_THREADS * sizeof(unsigned int);
+        PdfEdges edges;
+        lya_pdf_edges(n_bins, f_lo, width, &edges);
+        const size_t smem = (size_t)n_bins * FPDF_THREADS * sizeof(unsigned int) + (size_t)(n_bins + 1) * sizeof(float);
         LYA_CUDA(ctx, cudaFuncSetAttribute(flux_pdf_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         int per_sm = 0;
         LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, flux_pdf_fused_kernel, FPDF_THREADS, smem));
@@ -441,11 +482,12 @@ lya_status lya_run_flux_with_pdf(lya_ctx *ctx, const float *tau, size_t n, doubl
         if (want < 1) want = 1;
         const size_t cap = (size_t)ctx->sm_count * per_sm;
         flux_pdf_fused_kernel<<<(int)(want < cap ? want : cap), FPDF_THREADS, smem, ctx->stream>>>(
-            tau, n, make_trial(a), flux, n_bins, (float)f_lo, (float)(1.0 / width), d_counts);
+            tau, n, make_trial(a), flux, edges, d_counts);
         ctx->launches++;
         LYA_CUDA(ctx, cudaGetLastError());
     }
-    uint64_t host[256];
+    // counts come back through the ctx's pinned mirror: a true asynchronous DMA, no pageable staging
+    uint64_t *host = reinterpret_cast<uint64_t *>(ctx->h_pinned + LYA_PINNED_STATS);
     LYA_CUDA(ctx, cudaMemcpyAsync(host, d_counts, (size_t)n_bins * sizeof(uint64_t), cudaMemcpyDeviceToHost, ctx->stream));
     LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     for (int b = 0; b < n_bins; ++b) {

@@ -15,6 +15,7 @@
 #include <math.h>
 
 #include "lya_internal.h"
+#include "pdf_bin.h"
 
 namespace {
 
@@ -354,21 +355,19 @@ __global__ void __launch_bounds__(256) observe_rows_lean_kernel(const ObsArgs a,
 // ---- flux PDF: private per-thread histograms in shared memory (hist[bin][thread]: conflict-free, no atomics)
 constexpr int PDF_THREADS = 128;
 
-__global__ void __launch_bounds__(PDF_THREADS) flux_pdf_kernel(const float *__restrict__ flux, size_t n, int n_bins,
-                                                               float f_lo, float inv_width,
+__global__ void __launch_bounds__(PDF_THREADS) flux_pdf_kernel(const float *__restrict__ flux, size_t n,
+                                                               const __grid_constant__ PdfEdges edges,
                                                                unsigned long long *__restrict__ counts)
 {
-    extern __shared__ unsigned int hist[];               // [n_bins][PDF_THREADS]
+    extern __shared__ unsigned int hist[];               // [n_bins][PDF_THREADS], then n_bins + 1 thresholds
+    const int n_bins = edges.n_bins;
+    float *s_thr = reinterpret_cast<float *>(hist + n_bins * PDF_THREADS);
     for (int t = threadIdx.x; t < n_bins * PDF_THREADS; t += PDF_THREADS) hist[t] = 0u;
+    for (int t = threadIdx.x; t <= n_bins; t += PDF_THREADS) s_thr[t] = edges.thr[t];
     __syncthreads();
     unsigned int *mine = hist + threadIdx.x;
-    const float top = (float)n_bins;
-    auto add = [&](float f) {
-        // the bin decision is taken in fp32 with two separately rounded operations (reading O4)
-        const float t = floorf(__fmul_rn(__fsub_rn(f, f_lo), inv_width));
-        const int b = (t >= top) ? n_bins - 1 : (t > 0.0f ? (int)t : 0);
-        mine[b * PDF_THREADS] += 1u;
-    };
+    const float f_lo = edges.f_lo, inv_width = edges.inv_width, eps = edges.eps, ome = edges.one_minus_eps;
+    auto add = [&](float f) { mine[lya_pdf_bin(f, s_thr, n_bins, f_lo, inv_width, eps, ome) * PDF_THREADS] += 1u; };
     const size_t gtid = (size_t)blockIdx.x * PDF_THREADS + threadIdx.x, gsz = (size_t)gridDim.x * PDF_THREADS;
     size_t head = ((16 - ((uintptr_t)flux & 15)) & 15) >> 2;
     if (head > n) head = n;
@@ -587,7 +586,9 @@ extern "C" lya_status lya_flux_pdf(lya_ctx *ctx, const float *flux, size_t n, in
     unsigned long long *d_counts = reinterpret_cast<unsigned long long *>(ctx->d_stats);
     LYA_CUDA(ctx, cudaMemsetAsync(d_counts, 0, (size_t)n_bins * sizeof(unsigned long long), ctx->stream));
     if (n > 0) {
-        const size_t smem = (size_t)n_bins * PDF_THREADS * sizeof(unsigned int);
+        PdfEdges edges;
+        lya_pdf_edges(n_bins, f_lo, width, &edges);
+        const size_t smem = (size_t)n_bins * PDF_THREADS * sizeof(unsigned int) + (size_t)(n_bins + 1) * sizeof(float);
         LYA_CUDA(ctx, cudaFuncSetAttribute(flux_pdf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         int per_sm = 0;
         LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, flux_pdf_kernel, PDF_THREADS, smem));
@@ -595,12 +596,12 @@ extern "C" lya_status lya_flux_pdf(lya_ctx *ctx, const float *flux, size_t n, in
         size_t want = (n / 4 + PDF_THREADS - 1) / PDF_THREADS;
         if (want < 1) want = 1;
         const size_t cap = (size_t)ctx->sm_count * per_sm;
-        flux_pdf_kernel<<<(int)(want < cap ? want : cap), PDF_THREADS, smem, ctx->stream>>>(
-            flux, n, n_bins, (float)f_lo, (float)(1.0 / width), d_counts);
+        flux_pdf_kernel<<<(int)(want < cap ? want : cap), PDF_THREADS, smem, ctx->stream>>>(flux, n, edges, d_counts);
         ctx->launches++;
         LYA_CUDA(ctx, cudaGetLastError());
     }
-    uint64_t host[256];
+    // counts come back through the ctx's pinned mirror: a true asynchronous DMA, no pageable staging
+    uint64_t *host = reinterpret_cast<uint64_t *>(ctx->h_pinned + LYA_PINNED_STATS);
     LYA_CUDA(ctx, cudaMemcpyAsync(host, d_counts, (size_t)n_bins * sizeof(uint64_t), cudaMemcpyDeviceToHost, ctx->stream));
     LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     for (int b = 0; b < n_bins; ++b) {

@@ -262,9 +262,10 @@ extern "C" lya_status lya_flux_power_rows(lya_ctx *ctx, size_t n_rows, int32_t n
     kern<<<(int)(n_pairs < cap ? n_pairs : cap), threads, smem, ctx->stream>>>(a);
     ctx->launches++;
     LYA_CUDA(ctx, cudaGetLastError());
-    LYA_CUDA(ctx, cudaMemcpyAsync(power, ctx->d_stats, (size_t)nk * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    double *host = ctx->h_pinned + LYA_PINNED_STATS;                       // pinned: a true asynchronous DMA
+    LYA_CUDA(ctx, cudaMemcpyAsync(host, ctx->d_stats, (size_t)nk * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     const double scale = dv_kms / ((double)n_pix * (double)n_rows);        // V / N^2 / n_rows
-    for (int m = 0; m < nk; ++m) power[m] *= scale;
+    for (int m = 0; m < nk; ++m) power[m] = host[m] * scale;
     return LYA_OK;
 }

@@ -42,7 +42,8 @@
 //
 // Variants behind lya_tau_sightlines_opt (template flags, same kernels): FUSED applies S1 (gas_cell.h) to delta
 // while staging, so n_HI and b never exist in memory; WIN (LYA_TAU_WINDOWED) lets every lane walk only the
-// 2 reach + R sources around its own pixels (tile_window) -- bit-identical output, ~3 % of the pairs at N = 1024.
+// 2 reach + R sources around its own pixels (tile_window, over a row staged unwrapped with a periodic halo) --
+// bit-identical output, ~3 % of the pairs at N = 1024.
 #include "gas_cell.h"
 #include "lya_internal.h"
 
@@ -64,7 +65,7 @@ struct TauArgs {
     int          tstride;     // strided: floats per sightline of the tau tile (tiles*32*R + pad)
     long long    n_sl;        // x-axis: number of sightlines (rows)
     long long    n_batches;   // strided: number of gathered batches
-    unsigned int *sched;      // x-axis: [0] next row, [1] groups finished (self-resetting)
+    unsigned int *sched;      // [0] next row / batch to hand out; zeroed by the host before every launch
     // strided modes (axis 1, 2)
     int          nx;          // x extent
     int          nxb;         // ceil(nx / bsl)
@@ -77,6 +78,8 @@ struct TauArgs {
     float        xcut_over_w; // TAU_XCUT / w_scale: TAU_XCUT / w_j = b_j * xcut_over_w
     GasK         gas;         // FUSED (LYA_TAU_FROM_DENSITY): n_hi points at delta, S1 is done while staging
     unsigned long long *pairs; // device counter of (i,j) pairs evaluated
+    double      *rowm;        // [sightline][5] plain moments sum_i tau_i^k, k = 0..4, of every sightline written (or NULL):
+                              // S4's first pass (A = 0) without re-reading tau -- lya_normalize_mean_flux_rows
 };
 
 __device__ __forceinline__ float ex2_ftz(float x)
@@ -127,17 +130,41 @@ __device__ __forceinline__ float stage_from_global(const TauArgs &a, float jf, s
     return stage_cell(a, jf, nh, bb, __ldcs(a.v + g), out);
 }
 
-// Staged cells are stored at cpos(j): plain for the full sum (every lane reads the same cell: broadcast); for
-// LYA_TAU_WINDOWED, where lane k reads cell j0 + R k, one pad slot per R cells, j + j / R: the lanes of an
-// LDS.128 phase then sit (R + 1) float4 apart, and R + 1 being odd the eight of them fall into the eight
-// different 16-byte bank groups whatever j0 is (R = 1 needs no pad: neighbouring cells).
-template <bool PAD, int R> __device__ __forceinline__ int cpos(int j)
+// Staged cells are stored at cpos(j): plain for the full sum (every lane reads the same cell: broadcast).  For
+// LYA_TAU_WINDOWED, where lane k reads cell j0 + R k, the row is stored UNWRAPPED with a periodic halo of TAU_HALO
+// cells on either side (slot j + TAU_HALO holds cell j; the halo copies carry m -/+ N, so a walk across the ends
+// needs no wrap logic at all) and with one pad slot per R cells, s + s / R: the lanes of an LDS.128 phase then sit
+// (R + 1) float4 apart, and R + 1 being odd the eight of them fall into the eight different 16-byte bank groups
+// (R = 1 needs no pad: neighbouring cells).
+constexpr int TAU_HALO = 64;           // multiple of 4; a sightline whose window does not fit takes the full loops
+
+template <bool WIN, int R> __device__ __forceinline__ int cpos(int j)
 {
-    return (PAD && R > 1) ? j + (R == 2 ? (j >> 1) : (j >> 2)) : j;
+    if (!WIN) return j;
+    const int s = j + TAU_HALO;
+    return R > 1 ? s + (R == 2 ? (s >> 1) : (s >> 2)) : s;
 }
-template <int R> __host__ __device__ constexpr int crow_len(int n, bool pad)        // slots of one staged row
+template <int R> __host__ __device__ constexpr int crow_len(int n, bool win)        // slots of one staged row
 {
-    return (pad && R > 1) ? n + (R == 2 ? (n >> 1) : (n >> 2)) + 1 : n;
+    return !win ? n : (R > 1 ? (n + 2 * TAU_HALO) + (R == 2 ? ((n + 2 * TAU_HALO) >> 1) : ((n + 2 * TAU_HALO) >> 2)) + 1
+                             : n + 2 * TAU_HALO);
+}
+
+// LYA_TAU_WINDOWED: after the row is staged (and the group has synchronised), fill the halo: slot of index -t is
+// cell N - t with m - N, slot of index N - 1 + t is cell t - 1 with m + N (t = 1 .. TAU_HALO).  Rows shorter than
+// the halo never take the window (tile_any), so they skip this.
+template <int R>
+__device__ __forceinline__ void fill_halo(float4 *cs, int n, float n_f, int t0, int nthreads)
+{
+    if (n < TAU_HALO) return;
+    for (int t = t0; t < 2 * TAU_HALO; t += nthreads) {
+        const bool left = t < TAU_HALO;
+        const int src = left ? n - TAU_HALO + t : t - TAU_HALO;
+        const int dst = left ? t - TAU_HALO : n + t - TAU_HALO;
+        float4 q = cs[cpos<true, R>(src)];
+        q.x += left ? -n_f : n_f;                         // exact: integer-valued floats far below 2^24
+        cs[cpos<true, R>(dst)] = q;
+    }
 }
 
 // Fast path, full sum: unwrapped walk over all n sources jj = start .. start + n - 1 around the tile centre (at
@@ -173,36 +200,40 @@ __device__ __forceinline__ void tile_fast(const float4 *__restrict__ cs, int n, 
 }
 
 // LYA_TAU_WINDOWED: every LANE walks only its own window jj = il - W .. il + R - 1 + W around its R pixels
-// (il = i0 + lane R), W = the sightline's reach: 2 W + R sources instead of n.  A source outside the window is
-// further than its reach from all R pixels, so it would have added ex2(..) == 0 exactly; the sources kept are
-// added in the same ascending order with the same arithmetic (same reference pixel), so the result is
-// bit-identical to tile_fast.  Lanes read different cells (conflict-free through cpos<true, R>); the wrap is one
-// compare per source cell.
+// (il = i0 + lane R; W = the sightline's reach rounded up to a multiple of R): 2 W + R sources instead of n.  A
+// source outside the window is further than its reach from all R pixels, so it would have added ex2(..) == 0
+// exactly; the sources kept are added in the same ascending order with the same arithmetic (same reference pixel,
+// the same exact integer separation E), so the result is bit-identical to tile_fast.  The row is stored unwrapped
+// with a halo (cpos<true, R>), and il and W being multiples of R the walk is whole pad groups: R consecutive slots,
+// then one pad slot -- every LDS.128 offset is an immediate, there is no wrap test and no index arithmetic in the
+// loop, which is what lets the MUFU pipe set the pace as in the full sum.
 template <int R>
-__device__ __forceinline__ void tile_window(const float4 *__restrict__ cs, int n, float n_f, int i0, int lane, int W,
+__device__ __forceinline__ void tile_window(const float4 *__restrict__ cs, int n, int i0, int lane, int W,
                                             float (&acc)[R])
 {
     constexpr int RH = R / 2;
     const int il = i0 + lane * R;
-    const int jj = il - W;
-    int j = jj % n;
-    if (j < 0) j += n;
-    float cref = (float)(il + RH - (jj - j));
 #pragma unroll
     for (int r = 0; r < R; ++r) acc[r] = 0.0f;
-    const int cnt = 2 * W + R;
-#pragma unroll 4
-    for (int t = 0; t < cnt; ++t) {
-        const float4 q = cs[cpos<true, R>(j)];
-        const float E  = cref - q.x;
-        const float xr = fmaf(E, q.y, q.z);
+    if (il >= n) return;                                  // ragged last tile: this lane owns no pixel
+    const float4 *q4 = cs + cpos<true, R>(il - W);        // slot of the first source; (il - W + TAU_HALO) % R == 0
+    const float cref = (float)(il + RH);
+    const int groups = (2 * W + R) / R;
+#pragma unroll 2
+    for (int g = 0; g < groups; ++g) {
 #pragma unroll
-        for (int r = 0; r < R; ++r) {
-            const float x = (r == RH) ? xr : fmaf((float)(r - RH), q.y, xr);
-            const float e = ex2_ftz(-(x * x));
-            acc[r] = fmaf(q.w, e, acc[r]);
+        for (int k = 0; k < R; ++k) {
+            const float4 q = q4[k];
+            const float E  = cref - q.x;
+            const float xr = fmaf(E, q.y, q.z);
+#pragma unroll
+            for (int r = 0; r < R; ++r) {
+                const float x = (r == RH) ? xr : fmaf((float)(r - RH), q.y, xr);
+                const float e = ex2_ftz(-(x * x));
+                acc[r] = fmaf(q.w, e, acc[r]);
+            }
         }
-        if (++j == n) { j = 0; cref -= n_f; }
+        q4 += R > 1 ? R + 1 : 1;
     }
 }
 
@@ -244,9 +275,11 @@ __device__ __forceinline__ int tile_any(const TauArgs &a, const float4 *cs, floa
         return n;
     }
     if (WIN) {
-        const int W = (int)reach + 1;
-        tile_window<R>(cs, n, a.n_f, i0, lane, W, acc);
-        return 2 * W + R;
+        const int W = (((int)reach + 1) + R - 1) / R * R;   // whole pad groups on either side
+        if (W + R <= TAU_HALO && n >= TAU_HALO) {
+            tile_window<R>(cs, n, i0, lane, W, acc);
+            return 2 * W + R;
+        }
     }
     tile_fast<R, WIN>(cs, n, i0, lane, acc);
     return n;
@@ -274,6 +307,8 @@ __global__ void __launch_bounds__(1024, 1) tau_x_kernel(const TauArgs a, const i
     const int crow = crow_len<R>(n, WIN);                // float4 slots per staged row
     float4 *cells = reinterpret_cast<float4 *>(smem) + (size_t)grp * crow;
     volatile int *ctl = reinterpret_cast<volatile int *>(smem + (size_t)gpc * crow * sizeof(float4)) + 4 * grp;
+    // per warp: four doubles, the running sum_i tau_i^k (k = 1..4) of the warp's tiles of the current row
+    double *mom = reinterpret_cast<double *>(smem + (size_t)gpc * (crow * sizeof(float4) + 16)) + 4 * warp;
     const int bar_id = grp;      // named barrier of the group (G >= 2: at most 16 groups; no __syncthreads here)
     const int gl = wg * 32 + lane, gthreads = G * 32;    // thread index / count inside the group
 
@@ -301,18 +336,38 @@ __global__ void __launch_bounds__(1024, 1) tau_x_kernel(const TauArgs a, const i
         group_sync(G, bar_id);                           // cells complete, ctl[0] read
         if (G > 1 && lane == 0) atomicMax(const_cast<int *>(ctl + 1), __float_as_int(reach));   // reach >= 0
         if (gl == 0) ctl[2] = (int)atomicAdd(&a.sched[0], 1u);   // claim the next row early: latency hidden
-        if (G > 1) {
+        if (WIN) fill_halo<R>(cells, n, a.n_f, gl, gthreads);
+        if (G > 1 || WIN) {
             group_sync(G, bar_id);
-            reach = __int_as_float(ctl[1]);
+            reach = __int_as_float(G > 1 ? ctl[1] : __float_as_int(reach));
         }
 
         // ---- sum: the group's warps take the pixel tiles of the row
         int walked = 0;
+        if (a.rowm && lane < 4) mom[lane] = 0.0;
         for (int tile = wg; tile < a.tiles; tile += G) {
             const int i0 = tile * 32 * R;
             float acc[R];
             walked = tile_any<R, WIN>(a, cells, reach, i0, lane, acc);
             const int i = i0 + lane * R;
+            if (a.rowm) {                                // plain moments of the tile: fp32 over its 32 R pixels, double above
+                float p[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+#pragma unroll
+                for (int r = 0; r < R; ++r) {
+                    const float t = (i + r < n) ? acc[r] : 0.0f;
+                    float q = t;
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) { p[k] += q; q *= t; }
+                }
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) p[k] += __shfl_xor_sync(0xffffffffu, p[k], o);
+                __syncwarp();
+                if (lane == 0)
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) mom[k] += (double)p[k];
+            }
             float *dst = a.tau + g0 + i;
             if (R == 4 && a.vec) {
                 if (i < n) __stcs(reinterpret_cast<float4 *>(dst), make_float4(acc[0], acc[1], acc[2], acc[3]));
@@ -326,19 +381,19 @@ __global__ void __launch_bounds__(1024, 1) tau_x_kernel(const TauArgs a, const i
         }
         group_sync(G, bar_id);                           // cells consumed by every warp of the group
         if (gl == 0 && a.pairs) atomicAdd(a.pairs, (unsigned long long)n * (unsigned long long)walked);
+        if (gl == 0 && a.rowm) {                         // the row's moments: the group's warps in fixed order
+            double m[4] = {0.0, 0.0, 0.0, 0.0};
+            const int nw = G < a.tiles ? G : a.tiles;    // warps that had a tile
+            for (int w2 = 0; w2 < nw; ++w2)
+#pragma unroll
+                for (int k = 0; k < 4; ++k) m[k] += mom[4 * w2 + k];
+            double *dst = a.rowm + 5 * (size_t)row;
+            dst[0] = (double)n;
+#pragma unroll
+            for (int k = 0; k < 4; ++k) dst[1 + k] = m[k];
+        }
         if (gl == 0) ctl[0] = ctl[2];
         group_sync(G, bar_id);
-    }
-
-    // the last group to finish re-arms the row counter for the next launch on this ctx
-    if (gl == 0) {
-        __threadfence();
-        const unsigned int total = gridDim.x * (unsigned int)gpc;
-        if (atomicAdd(&a.sched[1], 1u) == total - 1u) {
-            a.sched[0] = 0u;
-            a.sched[1] = 0u;
-            __threadfence();
-        }
     }
 }
 
@@ -390,6 +445,10 @@ __global__ void __launch_bounds__(TAU_THREADS) tau_strided_kernel(const TauArgs 
         __syncthreads();                                 // cells complete
         reach = __int_as_float(s_reach);
         if (tid == 0) s_batch = atomicAdd(&a.sched[0], 1u);
+        if (WIN) {
+            for (int sl = warp; sl < nb; sl += TAU_WARPS) fill_halo<R>(cells + (size_t)sl * cstride, n, a.n_f, lane, 32);
+            __syncthreads();
+        }
 
         int walked = 0;
         const int items = nb * a.tiles;
@@ -407,6 +466,27 @@ __global__ void __launch_bounds__(TAU_THREADS) tau_strided_kernel(const TauArgs 
         }
         __syncthreads();                                 // cells consumed, tau tile complete, s_batch written
         if (tid == 0 && a.pairs) atomicAdd(a.pairs, (unsigned long long)nb * n * (unsigned long long)walked);
+        if (a.rowm) {                                    // plain moments per sightline, read off the tau tile
+            for (int sl = warp; sl < nb; sl += TAU_WARPS) {
+                double m[4] = {0.0, 0.0, 0.0, 0.0};
+                for (int j = lane; j < n; j += 32) {
+                    const double t = (double)ttile[sl * tstride + j];
+                    double q = t;
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) { m[k] += q; q *= t; }
+                }
+#pragma unroll
+                for (int k = 0; k < 4; ++k)
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) m[k] += __shfl_xor_sync(0xffffffffu, m[k], o);
+                if (lane == 0) {
+                    double *dst = a.rowm + 5 * (size_t)(outer * a.nx + x0 + sl);
+                    dst[0] = (double)n;
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) dst[1 + k] = m[k];
+                }
+            }
+        }
         for (int c = tid; c < (n << a.bshift); c += TAU_THREADS) {
             const int bx = c & (a.bsl - 1), j = c >> a.bshift;
             if (bx < nb) __stcs(a.tau + base + (long long)j * a.stride + bx, ttile[bx * tstride + j]);
@@ -414,14 +494,6 @@ __global__ void __launch_bounds__(TAU_THREADS) tau_strided_kernel(const TauArgs 
         __syncthreads();                                 // tile read out before the next batch's sums
     }
 
-    if (tid == 0) {                                      // the last CTA re-arms the counter
-        __threadfence();
-        if (atomicAdd(&a.sched[1], 1u) == gridDim.x - 1u) {
-            a.sched[0] = 0u;
-            a.sched[1] = 0u;
-            __threadfence();
-        }
-    }
 }
 
 template <int R, bool FUSED, bool WIN>
@@ -430,7 +502,8 @@ lya_status launch_x(lya_ctx *ctx, const TauArgs &a)
     auto kern = tau_x_kernel<R, FUSED, WIN>;
     const size_t cap = (size_t)ctx->max_smem_optin;
     const size_t per_group = (size_t)crow_len<R>(a.n, WIN) * sizeof(float4) + 16;
-    int groups = (int)(cap / per_group);                 // groups that fit in one SM's shared memory
+    const size_t mom_bytes = 32 * 4 * sizeof(double);    // four running moments per warp (a.rowm)
+    int groups = (int)((cap - mom_bytes) / per_group);   // groups that fit in one SM's shared memory
     if (groups < 1) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: sightline too long for shared memory");
     // G warps per group: as few as keep >= 24 warps resident, never more than the row has tiles
     int G = 1;
@@ -440,7 +513,7 @@ lya_status launch_x(lya_ctx *ctx, const TauArgs &a)
     // one persistent CTA per SM; never more groups than rows
     long long want = (a.n_sl + ctx->sm_count - 1) / ctx->sm_count;
     if (groups > want) groups = (int)(want < 1 ? 1 : want);
-    const size_t smem_bytes = (size_t)groups * per_group;
+    const size_t smem_bytes = (size_t)groups * per_group + mom_bytes;
     LYA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
     long long ctas = (a.n_sl + groups - 1) / groups;
     const int grid = (int)(ctas < ctx->sm_count ? ctas : ctx->sm_count);
@@ -471,7 +544,7 @@ lya_status launch_strided(lya_ctx *ctx, const TauArgs &a, size_t smem_bytes)
 lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
                           const float *n_hi, const float *b, const float *v, float *tau,
                           double amp_scale, double dv_kms, unsigned flags, const float *gas5,
-                          unsigned long long *d_pairs)
+                          unsigned long long *d_pairs, double *d_rowm)
 {
     const bool fused = (flags & LYA_TAU_FROM_DENSITY) != 0;
     const bool win = (flags & LYA_TAU_WINDOWED) != 0;
@@ -488,6 +561,10 @@ lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
     a.inv_n = 1.0f / (float)n;
     a.xcut_over_w = TAU_XCUT / a.w_scale;
     a.pairs = d_pairs;
+    a.rowm = d_rowm;
+    // the work counter is zeroed on the stream before EVERY launch: a launch that failed or was killed midway cannot
+    // leave it armed and turn later launches on this ctx into no-ops
+    LYA_CUDA(ctx, cudaMemsetAsync(ctx->d_sched, 0, 2 * sizeof(unsigned int), ctx->stream));
     if (fused) a.gas = GasK{gas5[0], gas5[1], gas5[2], gas5[3], gas5[4]};
     const int R = n >= 128 ? 4 : (n >= 64 ? 2 : 1);
     a.tiles = (n + 32 * R - 1) / (32 * R);
@@ -520,7 +597,7 @@ lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
     auto pad_to = [](int v, int mod, int want) { return v + ((want - v % mod) % mod + mod) % mod; };
     auto strides = [&](int sh, int &cs, int &ts) {
         const int bs = 1 << sh;
-        cs = pad_to(R == 4 ? crow_len<4>(n, win) : (R == 2 ? crow_len<2>(n, win) : n), 8, (8 / bs) % 8);
+        cs = pad_to(R == 4 ? crow_len<4>(n, win) : (R == 2 ? crow_len<2>(n, win) : crow_len<1>(n, win)), 8, (8 / bs) % 8);
         ts = pad_to(a.tiles * 32 * R, 32, (32 / bs) % 32);
     };
     auto need2 = [&](int sh) {

@@ -53,22 +53,32 @@ def philox4x32(c0, c1, c2, c3, k0: int, k1: int):
     return c0, c1, c2, c3
 
 
-def white_noise_plane(seed: int, fid: int, iz: int, n: int, device) -> torch.Tensor:
-    """N(0,1) white noise for one z-plane, float64 [n, n]. Key = (seed, fid), counter = (cell/4, iz)."""
+def white_noise_planes(seed: int, fid: int, izs, n: int, device) -> torch.Tensor:
+    """N(0,1) white noise for the z-planes `izs` (a sequence of plane indices), float64 [len(izs), n, n], all planes
+    in one batch of elementwise launches.  Key = (seed, fid), counter = (cell/4, iz): plane iz depends on nothing
+    but (seed, fid, iz)."""
     m = (n * n + 3) // 4
-    idx = torch.arange(m, dtype=torch.int64, device=device)
-    z = torch.zeros_like(idx)
-    r = philox4x32(idx & _MASK, idx >> 32, z + (iz & _MASK), z,
+    idx = torch.arange(m, dtype=torch.int64, device=device).unsqueeze(0)                      # [1, m]
+    zz = (torch.as_tensor(list(izs), dtype=torch.int64, device=device) & _MASK).unsqueeze(1)  # [P, 1]
+    c0, c1 = (idx & _MASK).expand(zz.shape[0], m), (idx >> 32).expand(zz.shape[0], m)
+    r = philox4x32(c0, c1, zz.expand(-1, m), torch.zeros_like(c0),
                    seed & _MASK, ((seed >> 32) ^ (fid * 0x9E3779B1)) & _MASK)
     u = [(x.to(torch.float64) + 0.5) * (1.0 / 4294967296.0) for x in r]
+    del r
     # Box-Muller on (u0,u1) and (u2,u3): four normals per counter
     r01 = torch.sqrt(-2.0 * torch.log(u[0]))
     r23 = torch.sqrt(-2.0 * torch.log(u[2]))
     t01 = (2.0 * math.pi) * u[1]
     t23 = (2.0 * math.pi) * u[3]
+    del u
     g = torch.stack([r01 * torch.cos(t01), r01 * torch.sin(t01),
-                     r23 * torch.cos(t23), r23 * torch.sin(t23)], dim=1).reshape(-1)
-    return g[: n * n].reshape(n, n)
+                     r23 * torch.cos(t23), r23 * torch.sin(t23)], dim=2).reshape(zz.shape[0], -1)
+    return g[:, : n * n].reshape(zz.shape[0], n, n)
+
+
+def white_noise_plane(seed: int, fid: int, iz: int, n: int, device) -> torch.Tensor:
+    """One plane of white_noise_planes: float64 [n, n]."""
+    return white_noise_planes(seed, fid, [iz], n, device)[0]
 
 
 def smoothing_weights(r_cells: float) -> torch.Tensor:
@@ -93,12 +103,8 @@ def unit_gaussian_field(seed: int, fid: int, n: int, r_cells: float, device="cpu
     out = torch.empty((z1 - z0, n, n), dtype=torch.float64, device=device)
     for c0 in range(z0, z1, chunk):
         c1 = min(c0 + chunk, z1)
-        planes = []
-        for iz in range(c0 - _HALO, c1 + _HALO):
-            p = white_noise_plane(seed, fid, iz % n, n, device)
-            p = _smooth_periodic(_smooth_periodic(p, w, 1), w, 0)      # along x, then y
-            planes.append(p)
-        stack = torch.stack(planes, dim=0)                             # [c1-c0+2H, n, n]
+        stack = white_noise_planes(seed, fid, [iz % n for iz in range(c0 - _HALO, c1 + _HALO)], n, device)
+        stack = _smooth_periodic(_smooth_periodic(stack, w, 2), w, 1)  # along x, then y: [c1-c0+2H, n, n]
         acc = torch.zeros((c1 - c0, n, n), dtype=torch.float64, device=device)
         for t in range(2 * _HALO + 1):
             # out[z] = sum_t w[t] * x[z - (t - H)]  (same convention as torch.roll above)

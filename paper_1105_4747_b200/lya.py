@@ -86,7 +86,8 @@ EXPORTS = ("lya_version", "lya_status_string", "lya_scalars_from_params", "lya_c
            "lya_flux", "lya_forest_host", "lya_launch_count", "lya_measure_mufu_peak",
            "lya_bin_kms_from_angstrom", "lya_instrument_bins", "lya_observe_rows", "lya_flux_pdf",
            "lya_flux_power_rows", "lya_tau_sightlines_opt", "lya_growth_rate", "lya_fields_from_dm", "lya_flux_moment_sums",
-           "lya_root_update_moments", "lya_flux_with_pdf")
+           "lya_root_update_moments", "lya_flux_with_pdf", "lya_forest_host_begin", "lya_forest_moment_sums",
+           "lya_forest_host_finish", "lya_measure_hbm_peak", "lya_normalize_mean_flux_rows", "lya_row_moment_sums")
 
 _lib = None
 
@@ -114,7 +115,9 @@ def lib() -> C.CDLL:
     L.lya_launch_count.restype = C.c_uint64
     L.lya_gas_from_density.argtypes = [vp, pp, fp, C.c_size_t, fp, fp]
     L.lya_tau_sightlines.argtypes = [vp, pp, C.c_int, C.c_int32, fp, fp, fp, fp]
-    L.lya_tau_sightlines_opt.argtypes = [vp, pp, C.c_int, C.c_int32, C.c_uint, fp, fp, fp, fp, C.POINTER(C.c_uint64)]
+    L.lya_tau_sightlines_opt.argtypes = [vp, pp, C.c_int, C.c_int32, C.c_uint, fp, fp, fp, fp, C.POINTER(C.c_uint64), vp]
+    L.lya_normalize_mean_flux_rows.argtypes = [vp, fp, C.c_size_t, vp, C.c_size_t, C.c_double, C.c_double, C.c_int, dp, dp, ip]
+    L.lya_row_moment_sums.argtypes = [vp, vp, C.c_size_t, dp]
     L.lya_normalize_mean_flux.argtypes = [vp, fp, C.c_size_t, C.c_double, C.c_double, C.c_int, dp, dp, ip]
     L.lya_flux_partial_sums.argtypes = [vp, fp, C.c_size_t, dp, C.c_int, dp, dp]
     L.lya_root_init.argtypes = [C.POINTER(CRootState), C.c_double, C.c_double, C.c_double]
@@ -124,7 +127,11 @@ def lib() -> C.CDLL:
     L.lya_flux.argtypes = [vp, fp, C.c_size_t, C.c_double, fp]
     L.lya_forest_host.argtypes = [vp, pp, C.c_int, C.c_int32, fp, fp, C.c_double, C.c_double, C.c_int,
                                   fp, fp, dp, dp, ip]
+    L.lya_forest_host_begin.argtypes = [vp, pp, C.c_int, C.c_int32, fp, fp, fp]
+    L.lya_forest_moment_sums.argtypes = [vp, C.c_double, dp]
+    L.lya_forest_host_finish.argtypes = [vp, C.c_double, fp]
     L.lya_measure_mufu_peak.argtypes = [vp, dp]
+    L.lya_measure_hbm_peak.argtypes = [vp, C.c_size_t, dp]
     L.lya_growth_rate.argtypes = [C.c_double, C.c_double, dp]
     L.lya_fields_from_dm.argtypes = [vp, C.POINTER(CFieldParams), fp, fp, fp, fp, fp]
     L.lya_bin_kms_from_angstrom.argtypes = [C.c_double, C.c_double]
@@ -213,6 +220,12 @@ class Context:
         self._check(lib().lya_measure_mufu_peak(self._h, C.byref(r)))
         return r.value
 
+    def measure_hbm_peak(self, n_bytes: int = 1 << 32) -> float:
+        """GB/s (read + written bytes) of the library's own 128-bit streaming copy kernel over n_bytes."""
+        r = C.c_double()
+        self._check(lib().lya_measure_hbm_peak(self._h, n_bytes, C.byref(r)))
+        return r.value
+
     # S1
     def gas_from_density(self, p: Params, delta: torch.Tensor, n_hi=None, b_kms=None):
         n_hi = torch.empty_like(delta) if n_hi is None else n_hi
@@ -235,8 +248,9 @@ class Context:
         return tau
 
     def tau_sightlines_opt(self, p: Params, axis: int, v_pec, n_hi=None, b_kms=None, delta=None, windowed=False,
-                           tau=None, nz_local=None, count_pairs=False):
+                           tau=None, nz_local=None, count_pairs=False, row_moments=None):
         """delta given -> S1 fused into the staging; windowed -> only contributing sources.
+        row_moments: float64 CUDA tensor [sightlines][5] that receives the per-sightline plain moments of tau.
         Returns tau, or (tau, pairs evaluated) with count_pairs."""
         first = delta if delta is not None else n_hi
         flags = (TAU_WINDOWED if windowed else 0) | (TAU_FROM_DENSITY if delta is not None else 0)
@@ -244,22 +258,39 @@ class Context:
         nz_local = first.shape[0] if nz_local is None else nz_local
         if first.numel() != nz_local * p.ny * p.nx or v_pec.numel() != first.numel() or tau.numel() != first.numel():
             raise ValueError("tau_sightlines_opt: arrays must be [nz_local][ny][nx]")
+        if row_moments is not None:
+            n_ax = (p.nx, p.ny, p.nz)[axis]
+            if not (row_moments.is_cuda and row_moments.dtype == torch.float64 and row_moments.is_contiguous()
+                    and row_moments.numel() == 5 * (first.numel() // n_ax)):
+                raise ValueError("row_moments: contiguous float64 CUDA tensor [sightlines][5] required")
         cp = p.c()
         pairs = C.c_uint64()
         self._check(lib().lya_tau_sightlines_opt(
             self._h, C.byref(cp), axis, nz_local, flags, _dev(first, "n_hi/delta"),
             None if delta is not None else _dev(b_kms, "b_kms"), _dev(v_pec, "v_pec"), _dev(tau, "tau"),
-            C.byref(pairs) if count_pairs else None))
+            C.byref(pairs) if count_pairs else None, None if row_moments is None else row_moments.data_ptr()))
         return (tau, int(pairs.value)) if count_pairs else tau
 
     # S4
     def normalize_mean_flux(self, tau, f_target: float, rel_tol: float = 1e-7, max_iter: int = 60,
-                            allow_noconv: bool = False):
+                            allow_noconv: bool = False, row_moments=None):
+        """row_moments: what tau_sightlines_opt(row_moments=...) wrote for exactly this tau -- the A = 0 pass then
+        reads them instead of tau.  Returns (A, f at A (model value), passes, status)."""
         a, f, it = C.c_double(), C.c_double(), C.c_int()
-        st = self._check(lib().lya_normalize_mean_flux(self._h, _dev(tau, "tau"), tau.numel(), f_target,
-                                                       rel_tol, max_iter, C.byref(a), C.byref(f), C.byref(it)),
-                         allow=(ENOCONV,) if allow_noconv else ())
+        if row_moments is None:
+            rc = lib().lya_normalize_mean_flux(self._h, _dev(tau, "tau"), tau.numel(), f_target,
+                                               rel_tol, max_iter, C.byref(a), C.byref(f), C.byref(it))
+        else:
+            rc = lib().lya_normalize_mean_flux_rows(self._h, _dev(tau, "tau"), tau.numel(), row_moments.data_ptr(),
+                                                    row_moments.numel() // 5, f_target, rel_tol, max_iter,
+                                                    C.byref(a), C.byref(f), C.byref(it))
+        st = self._check(rc, allow=(ENOCONV,) if allow_noconv else ())
         return a.value, f.value, it.value, st
+
+    def row_moment_sums(self, row_moments):
+        s5 = (C.c_double * 5)()
+        self._check(lib().lya_row_moment_sums(self._h, row_moments.data_ptr() or None, row_moments.numel() // 5, s5))
+        return list(s5)
 
     def flux_partial_sums(self, tau, a_trials):
         k = len(a_trials)
@@ -346,13 +377,34 @@ class Context:
         return a.value, f.value, it.value
 
 
+def forest_host_sharded(ctx: Context, p: Params, axis: int, delta_h, v_pec_h, f_target: float, n_pix_global: int,
+                        rel_tol: float = 1e-7, max_iter: int = 60, slab_nz: int = 0, tau_h=None, flux_h=None, group=None):
+    """S1..S5 from HOST buffers when every rank holds a z-slab of complete sightlines: lya_forest_host_begin on the
+    local slab, S4 over ALL ranks' pixels (five moments per pass, one all-reduce, lya_root_update_moments -- the
+    GLOBAL A of PAPER.md:92), lya_forest_host_finish.  Returns (A, f at A (model), passes)."""
+    cp = p.c()
+    ctx._check(lib().lya_forest_host_begin(ctx._h, C.byref(cp), axis, slab_nz, _host(delta_h, "delta_h"),
+                                           _host(v_pec_h, "v_pec_h"), _host(tau_h, "tau_h")))
+
+    def sums(a):
+        s5 = (C.c_double * 5)()
+        ctx._check(lib().lya_forest_moment_sums(ctx._h, a, s5))
+        return list(s5)
+
+    A, f, it = normalize_mean_flux_sharded(ctx, None, f_target, n_pix_global, rel_tol, max_iter, group, partial_sums=sums)
+    ctx._check(lib().lya_forest_host_finish(ctx._h, A, _host(flux_h, "flux_h")))
+    return A, f, it
+
+
 def normalize_mean_flux_sharded(ctx: Context, tau_local, f_target: float, n_pix_global: int,
-                                rel_tol: float = 1e-7, max_iter: int = 60, group=None, partial_sums=None):
+                                rel_tol: float = 1e-7, max_iter: int = 60, group=None, partial_sums=None,
+                                row_moments=None):
     """S4 when the pixels are sharded over ranks (z-slabs per GPU).
 
     Each pass: the five local tilted moments from lya_flux_moment_sums, one all-reduce of five doubles, then the
     library's scalar update lya_root_update_moments -- identical on every rank, so all ranks hold the same A.
     `partial_sums` lets a CPU test (gloo) stand in for the kernel; the product path leaves it None.
+    `row_moments`: the local tau's per-sightline plain moments (tau_sightlines_opt) -- the A = 0 pass sums those.
     """
     import torch.distributed as dist
     L = lib()
@@ -360,7 +412,12 @@ def normalize_mean_flux_sharded(ctx: Context, tau_local, f_target: float, n_pix_
     if L.lya_root_init(C.byref(st), f_target, rel_tol, float(n_pix_global)) != OK:
         raise LyaError(EINVAL, "lya_root_init: bad arguments")
     # per pass: five local tilted moments (or, with the two-sum stand-in of a CPU test, sum e and sum tau e)
-    sums_fn = partial_sums if partial_sums is not None else (lambda a: ctx.flux_moment_sums(tau_local, a))
+    def kernel_sums(a):
+        if a == 0.0 and row_moments is not None:
+            return ctx.row_moment_sums(row_moments)
+        return ctx.flux_moment_sums(tau_local, a)
+
+    sums_fn = partial_sums if partial_sums is not None else kernel_sums
     while not st.done:
         got = sums_fn(st.a)
         vals = list(got) if len(got) == 5 else [got[0][0], got[1][0]]

@@ -1,6 +1,6 @@
 """GPU parity of the instrument model, flux PDF and 1D flux power against
 oracle/lya_obs_oracle.c, through the C ABI.  Tolerances: observed flux 1e-5 absolute (the north_star's bar for
-F); PDF counts bit-exact (the bin decision is taken in fp32 on both sides); power 1e-4 relative plus 1e-9 of
+F); PDF counts bit-exact against the oracle's double-precision decision at the real edges (reading O4); power 1e-4 relative plus 1e-9 of
 the largest mode (fp32 FFT of dF)."""
 import numpy as np
 import pytest
@@ -97,6 +97,36 @@ def test_flux_pdf_bit_exact(ctx, obs, flux_rows):
         assert counts.sum() == arr.numel()
     counts, _ = ctx.flux_pdf(noisy, n_bins=100, f_lo=-0.5, width=0.02)
     assert np.array_equal(counts, obs.flux_pdf(noisy.cpu().numpy(), 100, -0.5, 0.02)[0])
+
+
+def test_flux_pdf_edge_decisions_match_the_real_number_bins(ctx, obs):
+    """PAPER.md:156 (reading O4): fluxes AT every interior edge's nearest fp32 and one ulp either side, the dyadic
+    edges, out-of-range values, infinities and NaN -- the kernel's counts must equal the oracle's double-precision
+    decision against the real edges, both for lya_flux_pdf and for the fused S5 + PDF pass."""
+    vals = []
+    for b in range(1, 21):
+        e = np.float32((2 * b - 1) / 40.0)
+        vals += [np.nextafter(e, np.float32(-9)), e, np.nextafter(e, np.float32(9))]
+    vals += [np.float32(x) for x in (-0.025, -0.0250001, 1.025, 1.0250001, -3.0, 7.0, 0.0, 1.0, 0.125, 0.375, 0.625, 0.875)]
+    vals += [np.float32("inf"), np.float32("-inf"), np.float32("nan")]
+    base = np.array(vals, dtype=np.float32)
+    F = torch.from_numpy(np.tile(base, 997)[:-1].copy()).cuda()           # ragged length, every thread sees edges
+    counts, _ = ctx.flux_pdf(F)
+    assert np.array_equal(counts, obs.flux_pdf(F.cpu().numpy())[0])
+    one_each = [ctx.flux_pdf(torch.from_numpy(np.array([v], dtype=np.float32)).cuda())[0] for v in base]
+    for v, c in zip(base, one_each):
+        assert np.array_equal(c, obs.flux_pdf(np.array([v], dtype=np.float32))[0]), float(v)
+    # the fused pass bins the F it writes: tau = -ln F / A reproduces fluxes close to the edges; whatever F
+    # comes out, its counts must equal the oracle's on that same F
+    tau = (-torch.log(F[torch.isfinite(F) & (F > 0)]) / 0.7).contiguous()
+    F2, c2, _ = ctx.flux_with_pdf(tau, 0.7)
+    assert np.array_equal(c2, obs.flux_pdf(F2.cpu().numpy())[0])
+    # other bin layouts, including one whose edges are all fp32-representable
+    g = torch.Generator(device="cuda").manual_seed(5)
+    R = (torch.rand(300_001, device="cuda", generator=g) * 2.4 - 0.7).contiguous()
+    R[:4096] = torch.arange(4096, device="cuda") / 64.0 - 8.0              # multiples of 1/64: on the edges below
+    for nb, lo, w in ((100, -0.5, 0.02), (64, -0.5, 0.03125), (7, 0.1, 0.13), (256, -1.0, 0.01)):
+        assert np.array_equal(ctx.flux_pdf(R, nb, lo, w)[0], obs.flux_pdf(R.cpu().numpy(), nb, lo, w)[0]), (nb, lo, w)
 
 
 @pytest.mark.parametrize("n_rows", [1, 2, 333])
