@@ -310,7 +310,9 @@ def test_forest_host_matches_stepwise_path(ctx, oracle):
     # the three-step form with the caller owning S4 (what a rank of a sharded run does)
     A3, f3, it3 = lya.forest_host_sharded(ctx, p, 0, dh, vh, w.f_target, tau.numel(), tau_h=tau_h, flux_h=flux_h)
     assert torch.equal(tau_h, tau.cpu()) and abs(A3 / A - 1) < 1e-9 and it3 == it
-    assert np.abs(flux_h.numpy() - F.cpu().numpy()).max() < 1e-7
+    # A3 differs from A in the last digits (host-side sum of per-call partials instead of the cooperative kernel's
+    # order), so ex2.approx's argument does too: F may move by a couple of fp32 ulps (6e-8 each below 1)
+    assert np.abs(flux_h.numpy() - F.cpu().numpy()).max() < 5e-7
     with pytest.raises(lya.LyaError):                                  # no resident tau any more
         ctx._check(lya.lib().lya_forest_host_finish(ctx._h, A, None))
 
