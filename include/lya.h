@@ -135,6 +135,22 @@ lya_status lya_normalize_mean_flux(lya_ctx *ctx, const float *tau, size_t n_pix,
                                    double rel_tol, int max_iter,
                                    double *a_out, double *f_achieved, int *iters);
 
+/* S4's nested iteration.  For n_pix >= min_pix the device loop first finds the root of the mean over a SUBSAMPLE of
+ * tau -- of its 16-byte aligned body cut into 4 KiB chunks, every `every`-th chunk; 1 / every of the bytes per pass --
+ * to 1e-3, and only then streams all of tau, starting from that root: the first full pass's fifth-order step lands on
+ * the root of the FULL mean and its truncation estimate proves it, so tau is normally streamed ONCE instead of 3-5
+ * times.  The returned A is the root of the mean over all pixels either way (same stopping rule; the subsample only
+ * supplies the starting point).  every <= 1 disables; defaults 32 and 2^24.  lya_last_normalize_stats says how the
+ * last call spent its passes; `iters` of lya_normalize_mean_flux counts tau_passes (incl. the row-moment pass). */
+typedef struct {
+    int32_t  tau_passes;   /* passes over ALL pixels: the full passes plus, if row moments were given, the A = 0 pass */
+    int32_t  sub_passes;   /* passes over the subsample                                                          */
+    int32_t  row_pass;     /* 1: the A = 0 pass read the per-sightline moments, not tau                           */
+    uint64_t n_sub;        /* pixels in the subsample (0: none)                                                   */
+} lya_normalize_stats;
+lya_status lya_set_normalize_subsample(lya_ctx *ctx, int32_t every, size_t min_pix);
+lya_status lya_last_normalize_stats(const lya_ctx *ctx, lya_normalize_stats *out);
+
 /* S4 started from the per-sightline plain moments lya_tau_sightlines_opt wrote (row_moments DEVICE [n_rows][5], over
  * exactly the n_pix pixels of tau): the A = 0 pass reads 40 B per sightline instead of 4 B per pixel; everything
  * else as lya_normalize_mean_flux, whose result it reproduces to the iteration's tolerance (the later passes and
@@ -175,6 +191,11 @@ lya_status lya_root_update(lya_root_state *s, double sum_exp, double sum_tau_exp
  * f_at_a is the model's value at the final a).  Feed the GLOBAL sums.  tau DEVICE; sums5 HOST. */
 lya_status lya_flux_moment_sums(lya_ctx *ctx, const float *tau, size_t n_pix, double a_trial, double *sums5);
 lya_status lya_root_update_moments(lya_root_state *s, const double *sums5);
+/* The same sums over the subsample of lya_set_normalize_subsample (every `every`-th 4 KiB chunk of the aligned body of
+ * tau; every == 1: all of tau), for callers that run the nested iteration themselves (slabs, ranks); n_sub (HOST, may be
+ * NULL) receives the number of pixels summed over -- the n_pix of the subsample's own lya_root_init. */
+lya_status lya_flux_moment_sums_sub(lya_ctx *ctx, const float *tau, size_t n_pix, double a_trial, int32_t every,
+                                    double *sums5, uint64_t *n_sub);
 
 /* S5.  tau, flux: DEVICE, n_pix floats; flux == tau (in place) allowed.  Asynchronous. */
 lya_status lya_flux(lya_ctx *ctx, const float *tau, size_t n_pix, double a, float *flux);
@@ -204,6 +225,8 @@ lya_status lya_forest_host(lya_ctx *ctx, const lya_params *p, int axis, int32_t 
 lya_status lya_forest_host_begin(lya_ctx *ctx, const lya_params *p, int axis, int32_t slab_nz,
                                  const float *delta_h, const float *v_pec_h, float *tau_h);
 lya_status lya_forest_moment_sums(lya_ctx *ctx, double a_trial, double *sums5);
+/* ... over the subsample of the resident tau (as lya_flux_moment_sums_sub; every == 1: all of it) */
+lya_status lya_forest_moment_sums_sub(lya_ctx *ctx, double a_trial, int32_t every, double *sums5, uint64_t *n_sub);
 lya_status lya_forest_host_finish(lya_ctx *ctx, double a, float *flux_h);
 
 /* ---------------------------------------------------------------------------------------------------------

@@ -111,13 +111,21 @@ extern "C" lya_status lya_forest_host_begin(lya_ctx *ctx, const lya_params *p, i
     return LYA_OK;
 }
 
-extern "C" lya_status lya_forest_moment_sums(lya_ctx *ctx, double a_trial, double *sums5)
+extern "C" lya_status lya_forest_moment_sums_sub(lya_ctx *ctx, double a_trial, int32_t every, double *sums5, uint64_t *n_sub)
 {
     if (!ctx) return LYA_EINVAL;
     ctx->err[0] = 0;
     if (!ctx->forest_total) return lya_fail(ctx, LYA_EINVAL, "lya_forest_moment_sums: no resident tau (call lya_forest_host_begin)");
-    if (a_trial == 0.0) return lya_row_moment_sums(ctx, ctx->forest_rowm, ctx->forest_rows, sums5);   // tau not re-read
-    return lya_flux_moment_sums(ctx, (const float *)ctx->ws, ctx->forest_total, a_trial, sums5);
+    if (a_trial == 0.0 && every <= 1) {                    // the A = 0 sums over all pixels: tau is not re-read
+        if (n_sub) *n_sub = ctx->forest_total;
+        return lya_row_moment_sums(ctx, ctx->forest_rowm, ctx->forest_rows, sums5);
+    }
+    return lya_flux_moment_sums_sub(ctx, (const float *)ctx->ws, ctx->forest_total, a_trial, every, sums5, n_sub);
+}
+
+extern "C" lya_status lya_forest_moment_sums(lya_ctx *ctx, double a_trial, double *sums5)
+{
+    return lya_forest_moment_sums_sub(ctx, a_trial, 1, sums5, nullptr);
 }
 
 extern "C" lya_status lya_forest_host_finish(lya_ctx *ctx, double a, float *flux_h)

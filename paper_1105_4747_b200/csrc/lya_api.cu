@@ -73,6 +73,8 @@ lya_status lya_create(lya_ctx **out, int device, void *cuda_stream)
     memset(ctx, 0, sizeof(*ctx));
     ctx->device = device;
     ctx->taps_key[0] = ctx->bins_key[0] = -1.0;
+    ctx->norm_sub_every = 32;                              // S4's nested iteration (lya_set_normalize_subsample)
+    ctx->norm_sub_min = (size_t)1 << 24;
     ctx->stream = (cudaStream_t)cuda_stream;
     cudaError_t e = cudaSetDevice(device);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, device);
@@ -217,6 +219,26 @@ lya_status lya_normalize_mean_flux(lya_ctx *ctx, const float *tau, size_t n_pix,
     return lya_normalize_mean_flux_rows(ctx, tau, n_pix, nullptr, 0, f_target, rel_tol, max_iter, a_out, f_achieved, iters);
 }
 
+lya_status lya_set_normalize_subsample(lya_ctx *ctx, int32_t every, size_t min_pix)
+{
+    if (!ctx) return LYA_EINVAL;
+    ctx->err[0] = 0;
+    if (every < 0 || every > 65536) return lya_fail(ctx, LYA_EINVAL, "lya_set_normalize_subsample: 0 <= every <= 65536 required");
+    ctx->norm_sub_every = every < 2 ? 1 : (size_t)every;
+    ctx->norm_sub_min = min_pix;
+    return LYA_OK;
+}
+
+lya_status lya_last_normalize_stats(const lya_ctx *ctx, lya_normalize_stats *out)
+{
+    if (!ctx || !out) return LYA_EINVAL;
+    out->tau_passes = (int32_t)ctx->norm_stats[0];
+    out->sub_passes = (int32_t)ctx->norm_stats[1];
+    out->row_pass   = (int32_t)ctx->norm_stats[2];
+    out->n_sub      = (uint64_t)ctx->norm_stats[3];
+    return LYA_OK;
+}
+
 lya_status lya_row_moment_sums(lya_ctx *ctx, const double *row_moments, size_t n_rows, double *sums5)
 {
     if (!ctx) return LYA_EINVAL;
@@ -268,15 +290,26 @@ lya_status lya_root_init(lya_root_state *s, double f_target, double rel_tol, dou
     return LYA_OK;
 }
 
-lya_status lya_flux_moment_sums(lya_ctx *ctx, const float *tau, size_t n_pix, double a_trial, double *sums5)
+lya_status lya_flux_moment_sums_sub(lya_ctx *ctx, const float *tau, size_t n_pix, double a_trial, int32_t every,
+                                    double *sums5, uint64_t *n_sub)
 {
     if (!ctx) return LYA_EINVAL;
     ctx->err[0] = 0;
     if ((n_pix > 0 && (!tau || ((uintptr_t)tau & 3))) || !sums5) return lya_fail(ctx, LYA_EINVAL, "lya_flux_moment_sums: null or misaligned pointer");
     if (!(a_trial >= 0.0) || !(a_trial < 1.0e30)) return lya_fail(ctx, LYA_EINVAL, "lya_flux_moment_sums: trial A must be finite and >= 0");
-    if (n_pix == 0) { for (int i = 0; i < 5; ++i) sums5[i] = 0.0; return LYA_OK; }
+    if (every < 1 || every > 65536) return lya_fail(ctx, LYA_EINVAL, "lya_flux_moment_sums_sub: 1 <= every <= 65536 required");
+    if (n_pix == 0) {
+        for (int i = 0; i < 5; ++i) sums5[i] = 0.0;
+        if (n_sub) *n_sub = 0;
+        return LYA_OK;
+    }
     LYA_CUDA(ctx, cudaSetDevice(ctx->device));
-    return lya_run_moment_sums(ctx, tau, n_pix, a_trial, sums5);
+    return lya_run_moment_sums(ctx, tau, n_pix, a_trial, (size_t)every, sums5, n_sub);
+}
+
+lya_status lya_flux_moment_sums(lya_ctx *ctx, const float *tau, size_t n_pix, double a_trial, double *sums5)
+{
+    return lya_flux_moment_sums_sub(ctx, tau, n_pix, a_trial, 1, sums5, nullptr);
 }
 
 lya_status lya_root_update_moments(lya_root_state *s, const double *sums5)

@@ -37,6 +37,9 @@ struct lya_ctx {
     double       *forest_rowm;                 // per-sightline plain moments of that tau (inside ws)
     size_t        forest_rows;
     size_t        forest_total, forest_slab;   // cells of the tau lya_forest_host_begin left resident in ws (0: none), chunk size
+    size_t        norm_sub_every, norm_sub_min;  // S4's nested iteration: subsample stride [4 KiB chunks], smallest n_pix that uses it
+    int           norm_occ;                      // CTAs of normalize_kernel per SM (0: not asked yet, -1: none)
+    double        norm_stats[4];                 // last lya_normalize_mean_flux: passes over tau, subsample passes, row pass, n_sub
     char          err[512];
 };
 
@@ -95,6 +98,8 @@ lya_status lya_run_normalize(lya_ctx *ctx, const float *tau, size_t n, const dou
 lya_status lya_run_row_moment_sums(lya_ctx *ctx, const double *rowm, size_t n_rows, double *sums5);
 lya_status lya_run_flux_with_pdf(lya_ctx *ctx, const float *tau, size_t n, double a, float *flux, int n_bins,
                                  double f_lo, double width, uint64_t *counts, double *pdf);
-lya_status lya_run_moment_sums(lya_ctx *ctx, const float *tau, size_t n, double a_trial, double *sums5);
+// every > 1: over the subsample (every `every`-th 4 KiB chunk of tau); n_sub receives the pixels summed over (or NULL)
+lya_status lya_run_moment_sums(lya_ctx *ctx, const float *tau, size_t n, double a_trial, size_t every, double *sums5,
+                               uint64_t *n_sub);
 lya_status lya_run_partial_sums(lya_ctx *ctx, const float *tau, size_t n, const double *a_trial, int k,
                                 double *sums, double *dsums);

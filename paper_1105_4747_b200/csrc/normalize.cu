@@ -87,8 +87,15 @@ __device__ __forceinline__ void accumulate(const float *__restrict__ tau, size_t
     }
 }
 
-// the same stream, five tilted moments sum tau^k e, k = 0..4, for one trial (lya_root_step_moments)
-__device__ __forceinline__ void accumulate_moments(const float *__restrict__ tau, size_t n, const Trial &tr, double (&s)[5])
+// the same stream, five tilted moments sum tau^k e, k = 0..4, for one trial (lya_root_step_moments).
+// SUB: only the SUBSAMPLE of tau -- of the 16-byte aligned body, cut into chunks of 256 float4 (4 KiB), every
+// `every`-th chunk; `items` = float4 in the subsample (the host counts them: sub_items()).  The subsample passes of
+// normalize_kernel's nested iteration read 1 / every of the bytes.
+constexpr int SUB_CHUNK_LOG2 = 8;
+
+template <bool SUB>
+__device__ __forceinline__ void accumulate_moments(const float *__restrict__ tau, size_t n, const Trial &tr, double (&s)[5],
+                                                   size_t every = 1, size_t items = 0)
 {
 #pragma unroll
     for (int k = 0; k < 5; ++k) s[k] = 0.0;
@@ -96,8 +103,12 @@ __device__ __forceinline__ void accumulate_moments(const float *__restrict__ tau
     const size_t gsz  = (size_t)gridDim.x * blockDim.x;
     size_t head = ((16 - ((uintptr_t)tau & 15)) & 15) >> 2;
     if (head > n) head = n;
-    const size_t n4 = (n - head) >> 2;
+    const size_t n4 = SUB ? items : (n - head) >> 2;
     const float4 *t4 = reinterpret_cast<const float4 *>(tau + head);
+    // item -> float4 index: the identity, or chunk (x >> 8) of the subsample = chunk (x >> 8) * every of tau
+    auto at = [&](size_t x) -> size_t {
+        return SUB ? ((((x >> SUB_CHUNK_LOG2) * every) << SUB_CHUNK_LOG2) | (x & ((1u << SUB_CHUNK_LOG2) - 1))) : x;
+    };
     // fp32 inside a group of up to four float4 (16 pixels), double above: one cvt + DADD per moment and group
     float q[5] = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f};
     auto add4 = [&](const float4 &t) {
@@ -111,7 +122,8 @@ __device__ __forceinline__ void accumulate_moments(const float *__restrict__ tau
     };
     size_t i = gtid;
     for (; i + 3 * gsz < n4; i += 4 * gsz) {
-        const float4 t0 = __ldg(t4 + i), t1 = __ldg(t4 + i + gsz), t2 = __ldg(t4 + i + 2 * gsz), t3 = __ldg(t4 + i + 3 * gsz);
+        const float4 t0 = __ldg(t4 + at(i)), t1 = __ldg(t4 + at(i + gsz)), t2 = __ldg(t4 + at(i + 2 * gsz)),
+                     t3 = __ldg(t4 + at(i + 3 * gsz));
 #pragma unroll
         for (int k = 0; k < 5; ++k) q[k] = 0.0f;
         add4(t0); add4(t1); add4(t2); add4(t3);
@@ -119,13 +131,14 @@ __device__ __forceinline__ void accumulate_moments(const float *__restrict__ tau
         for (int k = 0; k < 5; ++k) s[k] += (double)q[k];
     }
     for (; i < n4; i += gsz) {
-        const float4 t0 = __ldg(t4 + i);
+        const float4 t0 = __ldg(t4 + at(i));
 #pragma unroll
         for (int k = 0; k < 5; ++k) q[k] = 0.0f;
         add4(t0);
 #pragma unroll
         for (int k = 0; k < 5; ++k) s[k] += (double)q[k];
     }
+    if (SUB) return;                                     // the unaligned edges are not part of the subsample
     const size_t tail0 = head + (n4 << 2);
     const size_t n_edge = head + (n - tail0);
     for (size_t e = gtid; e < n_edge; e += gsz) {
@@ -170,24 +183,49 @@ struct NormArgs {
     size_t       n;
     const double *rowm;        // per-sightline plain moments [n_rows][5] written by the tau kernels, or NULL
     size_t       n_rows;
+    size_t       sub_every;    // > 1: nested iteration -- converge on every sub_every-th 4 KiB chunk of tau first
+    size_t       sub_items;    // float4 in that subsample
+    double       sub_tol;      // relative tolerance of the subsample's own root
     double       f_target, rel_tol;
     int          max_iter;
     double      *partials;     // [2][gridDim.x][5], gridDim.x <= SM count
-    double      *result;       // [0] A, [1] <F> at A, [2] passes, [3] status
+    double      *result;       // [0] A, [1] <F> at A, [2] passes over all of tau (incl. the row-moment pass), [3] status,
+                               // [4] subsample passes, [5] 1 if the A = 0 pass read the row moments
 };
+
+// The iteration, nested (reading C14):
+//   ROWS  the A = 0 pass from the tau kernels' per-sightline moments, if the caller has them (40 B per sightline);
+//   SUB   the whole root iteration on a SUBSAMPLE of tau (1 / sub_every of the bytes per pass) to sub_tol: the mean flux
+//         of 1/32 of 1e9 pixels already fixes A to ~1e-4, and a heavy-tailed tau (max 1e6 x mean on the lognormal fields)
+//         makes the first steps from A = 0 short, so this is where most passes go;
+//   FULL  passes over ALL of tau from the subsample's root: the first one's fifth-order step lands within ~1e-15 of the
+//         root of the FULL mean (|h| ~ 1e-4 A), its quartic-vs-cubic truncation estimate proves it, and the iteration
+//         stops -- normally ONE pass over tau instead of 3-5.
+// The result is the root of the mean over all pixels in every case: the subsample only supplies the starting point,
+// the stopping rule is the full iteration's own.
+constexpr int NORM_SUB_MAX = 12;                         // subsample passes before giving up on its convergence
+enum { PH_ROWS = 0, PH_SUB = 1, PH_FULL = 2 };
 
 __global__ void __launch_bounds__(NORM_THREADS, 1) normalize_kernel(const NormArgs a)
 {
     cg::grid_group grid = cg::this_grid();
     __shared__ double sh[5 * 32];
     __shared__ lya_root_state st;
-    if (threadIdx.x == 0) lya_root_reset(&st, a.f_target, a.rel_tol, (double)a.n);
+    __shared__ int s_phase, s_full, s_sub, s_finished;
+    if (threadIdx.x == 0) {
+        const bool sub = a.sub_every > 1 && a.sub_items > 0;
+        s_phase = a.rowm ? PH_ROWS : (sub ? PH_SUB : PH_FULL);
+        s_full = s_sub = s_finished = 0;
+        if (s_phase == PH_SUB) lya_root_reset(&st, a.f_target, a.sub_tol, 4.0 * (double)a.sub_items);
+        else                   lya_root_reset(&st, a.f_target, a.rel_tol, (double)a.n);
+    }
     __syncthreads();
 
     for (int pass = 0;; ++pass) {
+        const int phase = s_phase;
         const Trial tr = make_trial(st.a);
         double s[5];
-        if (pass == 0 && a.rowm) {
+        if (phase == PH_ROWS) {
             // A = 0: the tilted moments are the plain moments sum tau^k, which the tau kernels left per sightline
             // (40 B per sightline instead of 4 B per pixel); fixed thread -> row assignment, so bit-reproducible
 #pragma unroll
@@ -195,8 +233,10 @@ __global__ void __launch_bounds__(NORM_THREADS, 1) normalize_kernel(const NormAr
             for (size_t r = (size_t)blockIdx.x * blockDim.x + threadIdx.x; r < a.n_rows; r += (size_t)gridDim.x * blockDim.x)
 #pragma unroll
                 for (int k = 0; k < 5; ++k) s[k] += __ldcs(a.rowm + 5 * r + k);
+        } else if (phase == PH_SUB) {
+            accumulate_moments<true>(a.tau, a.n, tr, s, a.sub_every, a.sub_items);
         } else {
-            accumulate_moments(a.tau, a.n, tr, s);
+            accumulate_moments<false>(a.tau, a.n, tr, s);
         }
         block_sum<5>(s, sh);
         double *part = a.partials + (size_t)(pass & 1) * gridDim.x * 5;
@@ -211,17 +251,43 @@ __global__ void __launch_bounds__(NORM_THREADS, 1) normalize_kernel(const NormAr
             for (int k = 0; k < 5; ++k) t[k] += __ldcg(part + 5 * b + k);
         block_sum<5>(t, sh);
         if (threadIdx.x == 0) {
+            const double a_before = st.a;
             lya_root_step_moments(&st, t);
-            if (!st.done && st.iters >= a.max_iter) { st.status = LYA_ENOCONV; st.done = 1; }
+            const bool sub = a.sub_every > 1 && a.sub_items > 0;
+            if (phase == PH_SUB) {
+                s_sub += 1;
+                if (st.done || s_sub >= NORM_SUB_MAX) {  // the subsample's root (or the best it got): start of the full passes
+                    const double a0 = (st.status == LYA_OK && st.a > 0.0 && st.a < 1.0e30) ? st.a : a_before;
+                    lya_root_reset(&st, a.f_target, a.rel_tol, (double)a.n);
+                    st.a = a0;
+                    s_phase = PH_FULL;
+                }
+            } else {
+                s_full += 1;
+                if (st.done) {
+                    s_finished = 1;
+                } else if (s_full >= a.max_iter) {
+                    st.status = LYA_ENOCONV; st.done = 1; s_finished = 1;
+                } else if (phase == PH_ROWS) {
+                    s_phase = sub ? PH_SUB : PH_FULL;
+                    if (sub) {                           // the subsample has its own pixel count and tolerance
+                        const double a0 = st.a;
+                        lya_root_reset(&st, a.f_target, a.sub_tol, 4.0 * (double)a.sub_items);
+                        st.a = a0;
+                    }
+                }
+            }
         }
         __syncthreads();
-        if (st.done) break;
+        if (s_finished) break;
     }
     if (blockIdx.x == 0 && threadIdx.x == 0) {
         a.result[0] = st.a;
         a.result[1] = st.f_at_a;
-        a.result[2] = (double)st.iters;
+        a.result[2] = (double)s_full;
         a.result[3] = (double)st.status;
+        a.result[4] = (double)s_sub;
+        a.result[5] = a.rowm ? 1.0 : 0.0;
     }
 }
 
@@ -246,11 +312,12 @@ __global__ void __launch_bounds__(RED_THREADS) partial_sums_kernel(const float *
 }
 
 __global__ void __launch_bounds__(RED_THREADS) moment_sums_kernel(const float *__restrict__ tau, size_t n, const Trial tr,
-                                                                 double *partials)
+                                                                 double *partials, size_t sub_every, size_t sub_items)
 {
     __shared__ double sh[5 * 32];
     double s[5];
-    accumulate_moments(tau, n, tr, s);
+    if (sub_every > 1) accumulate_moments<true>(tau, n, tr, s, sub_every, sub_items);
+    else               accumulate_moments<false>(tau, n, tr, s);
     block_sum<5>(s, sh);
     if (threadIdx.x == 0)
 #pragma unroll
@@ -363,6 +430,19 @@ __global__ void __launch_bounds__(FPDF_THREADS) flux_pdf_fused_kernel(const floa
     }
 }
 
+// float4 in the subsample "every `every`-th chunk of 256 float4 of the aligned body of tau" (0: no subsample)
+size_t sub_items_of(const float *tau, size_t n, size_t every)
+{
+    size_t head = ((16 - ((uintptr_t)tau & 15)) & 15) >> 2;
+    if (head > n) head = n;
+    const size_t n4 = (n - head) >> 2;
+    if (every <= 1 || n4 == 0) return 0;
+    const size_t n_ch = (n4 + 255) >> SUB_CHUNK_LOG2, k_sub = (n_ch + every - 1) / every;
+    const size_t last = ((k_sub - 1) * every) << SUB_CHUNK_LOG2;          // first float4 of the last subsample chunk
+    const size_t len_last = n4 - last < 256 ? n4 - last : 256;
+    return ((k_sub - 1) << SUB_CHUNK_LOG2) + len_last;
+}
+
 int red_grid(lya_ctx *ctx, size_t n, int per_sm)
 {
     size_t want = (n / 4 + RED_THREADS - 1) / RED_THREADS;
@@ -378,11 +458,19 @@ lya_status lya_run_normalize(lya_ctx *ctx, const float *tau, size_t n, const dou
                              double f_target, double rel_tol, int max_iter, double *a_out, double *f_out, int *iters)
 {
     if (!ctx->coop_ok) return lya_fail(ctx, LYA_ECUDA, "device does not support cooperative launch");
-    int per_sm = 0;
-    LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, normalize_kernel, NORM_THREADS, 0));
-    if (per_sm < 1) return lya_fail(ctx, LYA_ECUDA, "normalize_kernel: zero occupancy");
+    if (ctx->norm_occ == 0) {                              // asked once per ctx: the answer cannot change
+        int per_sm = 0;
+        LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, normalize_kernel, NORM_THREADS, 0));
+        ctx->norm_occ = per_sm < 1 ? -1 : per_sm;
+    }
+    if (ctx->norm_occ < 1) return lya_fail(ctx, LYA_ECUDA, "normalize_kernel: zero occupancy");
     // the four result doubles go straight to the pinned host mirror (mapped under UVA): no copy to enqueue
-    NormArgs a{tau, n, rowm, n_rows, f_target, rel_tol, max_iter, ctx->d_partials, ctx->h_pinned};
+    // nested iteration for grids beyond norm_sub_min pixels (lya_set_normalize_subsample); the subsample's own root is
+    // only a starting point, so its tolerance is loose: its statistical distance from the full root is ~1e-4 anyway
+    const size_t every = (ctx->norm_sub_every > 1 && n >= ctx->norm_sub_min) ? ctx->norm_sub_every : 1;
+    const size_t items = sub_items_of(tau, n, every);
+    NormArgs a{tau, n, rowm, n_rows, items ? every : 1, items, 1.0e-3 > rel_tol ? 1.0e-3 : rel_tol,
+               f_target, rel_tol, max_iter, ctx->d_partials, ctx->h_pinned};
     size_t want = (n / 4 + NORM_THREADS - 1) / NORM_THREADS;           // at least one float4 per thread
     if (want < 1) want = 1;
     const int grid = (int)(want < (size_t)ctx->sm_count ? want : (size_t)ctx->sm_count);
@@ -394,6 +482,10 @@ lya_status lya_run_normalize(lya_ctx *ctx, const float *tau, size_t n, const dou
     if (a_out) *a_out = ctx->h_pinned[0];
     if (f_out) *f_out = ctx->h_pinned[1];
     if (iters) *iters = (int)ctx->h_pinned[2];
+    ctx->norm_stats[0] = ctx->h_pinned[2];                 // lya_last_normalize_stats
+    ctx->norm_stats[1] = ctx->h_pinned[4];
+    ctx->norm_stats[2] = ctx->h_pinned[5];
+    ctx->norm_stats[3] = 4.0 * (double)items;
     lya_status st = (lya_status)(int)ctx->h_pinned[3];
     if (st == LYA_ENOROOT) return lya_fail(ctx, st, "lya_normalize_mean_flux: no A > 0 reaches f_target");
     if (st == LYA_ENOCONV) return lya_fail(ctx, st, "lya_normalize_mean_flux: max_iter reached");
@@ -440,10 +532,17 @@ lya_status lya_launch_flux(lya_ctx *ctx, const float *tau, size_t n, double a, f
     return LYA_OK;
 }
 
-lya_status lya_run_moment_sums(lya_ctx *ctx, const float *tau, size_t n, double a_trial, double *sums5)
+lya_status lya_run_moment_sums(lya_ctx *ctx, const float *tau, size_t n, double a_trial, size_t every, double *sums5,
+                               uint64_t *n_sub)
 {
-    const int grid = red_grid(ctx, n, 8);
-    moment_sums_kernel<<<grid, RED_THREADS, 0, ctx->stream>>>(tau, n, make_trial(a_trial), ctx->d_partials);
+    const size_t items = sub_items_of(tau, n, every);
+    if (n_sub) *n_sub = every > 1 ? 4 * items : n;
+    if (every > 1 && items == 0) {                         // nothing in the subsample (fewer than 4 aligned pixels)
+        for (int i = 0; i < 5; ++i) sums5[i] = 0.0;
+        return LYA_OK;
+    }
+    const int grid = red_grid(ctx, every > 1 ? 4 * items : n, 8);
+    moment_sums_kernel<<<grid, RED_THREADS, 0, ctx->stream>>>(tau, n, make_trial(a_trial), ctx->d_partials, every, items);
     finish_sums_kernel<<<1, RED_THREADS, 0, ctx->stream>>>(ctx->d_partials, grid, 5, ctx->h_pinned);   // mapped pinned memory
     ctx->launches += 2;
     LYA_CUDA(ctx, cudaGetLastError());

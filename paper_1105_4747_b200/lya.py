@@ -46,6 +46,10 @@ class CFieldParams(C.Structure):
                 ("h", C.c_double), ("z", C.c_double), ("omega_m", C.c_double), ("k_filter_mpc", C.c_double)]
 
 
+class CNormalizeStats(C.Structure):
+    _fields_ = [("tau_passes", C.c_int32), ("sub_passes", C.c_int32), ("row_pass", C.c_int32), ("n_sub", C.c_uint64)]
+
+
 class CRootState(C.Structure):
     _fields_ = [("f_target", C.c_double), ("rel_tol", C.c_double), ("n_pix", C.c_double),
                 ("lo", C.c_double), ("hi", C.c_double), ("a", C.c_double), ("f_at_a", C.c_double),
@@ -87,7 +91,9 @@ EXPORTS = ("lya_version", "lya_status_string", "lya_scalars_from_params", "lya_c
            "lya_bin_kms_from_angstrom", "lya_instrument_bins", "lya_observe_rows", "lya_flux_pdf",
            "lya_flux_power_rows", "lya_tau_sightlines_opt", "lya_growth_rate", "lya_fields_from_dm", "lya_flux_moment_sums",
            "lya_root_update_moments", "lya_flux_with_pdf", "lya_forest_host_begin", "lya_forest_moment_sums",
-           "lya_forest_host_finish", "lya_measure_hbm_peak", "lya_normalize_mean_flux_rows", "lya_row_moment_sums")
+           "lya_forest_host_finish", "lya_measure_hbm_peak", "lya_normalize_mean_flux_rows", "lya_row_moment_sums",
+           "lya_set_normalize_subsample", "lya_last_normalize_stats", "lya_flux_moment_sums_sub",
+           "lya_forest_moment_sums_sub")
 
 _lib = None
 
@@ -124,6 +130,10 @@ def lib() -> C.CDLL:
     L.lya_root_update.argtypes = [C.POINTER(CRootState), C.c_double, C.c_double]
     L.lya_flux_moment_sums.argtypes = [vp, fp, C.c_size_t, C.c_double, dp]
     L.lya_root_update_moments.argtypes = [C.POINTER(CRootState), dp]
+    L.lya_flux_moment_sums_sub.argtypes = [vp, fp, C.c_size_t, C.c_double, C.c_int32, dp, C.POINTER(C.c_uint64)]
+    L.lya_forest_moment_sums_sub.argtypes = [vp, C.c_double, C.c_int32, dp, C.POINTER(C.c_uint64)]
+    L.lya_set_normalize_subsample.argtypes = [vp, C.c_int32, C.c_size_t]
+    L.lya_last_normalize_stats.argtypes = [vp, C.POINTER(CNormalizeStats)]
     L.lya_flux.argtypes = [vp, fp, C.c_size_t, C.c_double, fp]
     L.lya_forest_host.argtypes = [vp, pp, C.c_int, C.c_int32, fp, fp, C.c_double, C.c_double, C.c_int,
                                   fp, fp, dp, dp, ip]
@@ -287,6 +297,15 @@ class Context:
         st = self._check(rc, allow=(ENOCONV,) if allow_noconv else ())
         return a.value, f.value, it.value, st
 
+    def set_normalize_subsample(self, every: int, min_pix: int):
+        """S4's nested iteration: subsample stride in 4 KiB chunks (<= 1: off) and the smallest n_pix that uses it."""
+        self._check(lib().lya_set_normalize_subsample(self._h, every, min_pix))
+
+    def last_normalize_stats(self) -> dict:
+        st = CNormalizeStats()
+        self._check(lib().lya_last_normalize_stats(self._h, C.byref(st)))
+        return {k: int(getattr(st, k)) for k, _ in CNormalizeStats._fields_}
+
     def row_moment_sums(self, row_moments):
         s5 = (C.c_double * 5)()
         self._check(lib().lya_row_moment_sums(self._h, row_moments.data_ptr() or None, row_moments.numel() // 5, s5))
@@ -303,6 +322,12 @@ class Context:
         s5 = (C.c_double * 5)()
         self._check(lib().lya_flux_moment_sums(self._h, _dev(tau, "tau"), tau.numel(), a_trial, s5))
         return list(s5)
+
+    def flux_moment_sums_sub(self, tau, a_trial: float, every: int):
+        """The five tilted moments over every `every`-th 4 KiB chunk of tau; returns (sums5, pixels summed over)."""
+        s5, ns = (C.c_double * 5)(), C.c_uint64()
+        self._check(lib().lya_flux_moment_sums_sub(self._h, _dev(tau, "tau"), tau.numel(), a_trial, every, s5, C.byref(ns)))
+        return list(s5), int(ns.value)
 
     # S5
     def flux(self, tau, a: float, out=None):
@@ -378,61 +403,114 @@ class Context:
 
 
 def forest_host_sharded(ctx: Context, p: Params, axis: int, delta_h, v_pec_h, f_target: float, n_pix_global: int,
-                        rel_tol: float = 1e-7, max_iter: int = 60, slab_nz: int = 0, tau_h=None, flux_h=None, group=None):
+                        rel_tol: float = 1e-7, max_iter: int = 60, slab_nz: int = 0, tau_h=None, flux_h=None, group=None,
+                        sub_every: int = 32):
     """S1..S5 from HOST buffers when every rank holds a z-slab of complete sightlines: lya_forest_host_begin on the
     local slab, S4 over ALL ranks' pixels (five moments per pass, one all-reduce, lya_root_update_moments -- the
-    GLOBAL A of PAPER.md:92), lya_forest_host_finish.  Returns (A, f at A (model), passes)."""
+    GLOBAL A of PAPER.md:92), lya_forest_host_finish.  Returns (A, f at A (model), passes over all of tau)."""
     cp = p.c()
     ctx._check(lib().lya_forest_host_begin(ctx._h, C.byref(cp), axis, slab_nz, _host(delta_h, "delta_h"),
                                            _host(v_pec_h, "v_pec_h"), _host(tau_h, "tau_h")))
 
-    def sums(a):
-        s5 = (C.c_double * 5)()
-        ctx._check(lib().lya_forest_moment_sums(ctx._h, a, s5))
-        return list(s5)
+    def sums(a, every):
+        s5, ns = (C.c_double * 5)(), C.c_uint64()
+        ctx._check(lib().lya_forest_moment_sums_sub(ctx._h, a, every, s5, C.byref(ns)))
+        return list(s5), int(ns.value)
 
-    A, f, it = normalize_mean_flux_sharded(ctx, None, f_target, n_pix_global, rel_tol, max_iter, group, partial_sums=sums)
+    A, f, it = normalize_mean_flux_sharded(ctx, None, f_target, n_pix_global, rel_tol, max_iter, group,
+                                           kernel_sums=sums, sub_every=sub_every)
     ctx._check(lib().lya_forest_host_finish(ctx._h, A, _host(flux_h, "flux_h")))
     return A, f, it
 
 
 def normalize_mean_flux_sharded(ctx: Context, tau_local, f_target: float, n_pix_global: int,
                                 rel_tol: float = 1e-7, max_iter: int = 60, group=None, partial_sums=None,
-                                row_moments=None):
+                                row_moments=None, sub_every: int = 32, sub_min_pix: int = 1 << 24, kernel_sums=None,
+                                stats: dict | None = None):
     """S4 when the pixels are sharded over ranks (z-slabs per GPU).
 
-    Each pass: the five local tilted moments from lya_flux_moment_sums, one all-reduce of five doubles, then the
-    library's scalar update lya_root_update_moments -- identical on every rank, so all ranks hold the same A.
-    `partial_sums` lets a CPU test (gloo) stand in for the kernel; the product path leaves it None.
-    `row_moments`: the local tau's per-sightline plain moments (tau_sightlines_opt) -- the A = 0 pass sums those.
+    Each pass: the five local tilted moments from lya_flux_moment_sums[_sub], one all-reduce of six doubles (the
+    moments and the number of pixels they run over), then the library's scalar update lya_root_update_moments --
+    identical on every rank, so all ranks hold the same A.  The passes are nested as in lya_normalize_mean_flux: the
+    A = 0 pass from `row_moments` (the local tau's per-sightline plain moments, tau_sightlines_opt) if given; for
+    n_pix_global >= sub_min_pix the whole iteration on every sub_every-th 4 KiB chunk of each rank's tau to 1e-3;
+    then passes over all of tau from there until the full iteration's own stopping rule holds (normally one).
+    `partial_sums` lets a CPU test (gloo) stand in for the kernel (no subsample then); the product path leaves it None.
+    `kernel_sums(a, every) -> (sums5, pixels)` replaces lya_flux_moment_sums_sub (forest_host_sharded's resident tau).
+    Returns (A, f at A (model value), passes over all of tau); `stats` receives the pass counts.
     """
     import torch.distributed as dist
     L = lib()
-    st = CRootState()
-    if L.lya_root_init(C.byref(st), f_target, rel_tol, float(n_pix_global)) != OK:
-        raise LyaError(EINVAL, "lya_root_init: bad arguments")
-    # per pass: five local tilted moments (or, with the two-sum stand-in of a CPU test, sum e and sum tau e)
-    def kernel_sums(a):
-        if a == 0.0 and row_moments is not None:
-            return ctx.row_moment_sums(row_moments)
-        return ctx.flux_moment_sums(tau_local, a)
 
-    sums_fn = partial_sums if partial_sums is not None else kernel_sums
-    while not st.done:
-        got = sums_fn(st.a)
-        vals = list(got) if len(got) == 5 else [got[0][0], got[1][0]]
+    def all_reduce(vals):
         buf = torch.tensor(vals, dtype=torch.float64)
         if dist.is_available() and dist.is_initialized():
             if dist.get_backend(group) == "nccl":
                 buf = buf.cuda()
             dist.all_reduce(buf, op=dist.ReduceOp.SUM, group=group)
             buf = buf.cpu()
-        if len(vals) == 5:
-            rc = L.lya_root_update_moments(C.byref(st), (C.c_double * 5)(*[float(x) for x in buf]))
-        else:
-            rc = L.lya_root_update(C.byref(st), float(buf[0]), float(buf[1]))
+        return [float(x) for x in buf]
+
+    def local_sums(a, every):
+        if kernel_sums is not None:
+            return kernel_sums(a, every)
+        if a == 0.0 and every <= 1 and row_moments is not None:
+            return ctx.row_moment_sums(row_moments), tau_local.numel()
+        return ctx.flux_moment_sums_sub(tau_local, a, every)
+
+    def new_state(tol, n_pix, a0=0.0):
+        st = CRootState()
+        if L.lya_root_init(C.byref(st), f_target, tol, float(n_pix)) != OK:
+            raise LyaError(EINVAL, "lya_root_init: bad arguments")
+        st.a = a0
+        return st
+
+    def update(st, sums5):
+        rc = L.lya_root_update_moments(C.byref(st), (C.c_double * 5)(*sums5))
         if rc == ENOROOT:
             raise LyaError(rc, "no A > 0 reaches f_target")
-        if not st.done and st.iters >= max_iter:
-            break
-    return st.a, st.f_at_a, st.iters
+
+    st = new_state(rel_tol, n_pix_global)
+    n_full = n_sub_passes = n_sub_local = 0
+    if partial_sums is not None:                         # CPU stand-in: plain loop, five moments or the two-sum rule
+        while not st.done and st.iters < max_iter:
+            got = partial_sums(st.a)
+            if len(got) == 5:
+                update(st, all_reduce(list(got)))
+            else:
+                s = all_reduce([got[0][0], got[1][0]])
+                if L.lya_root_update(C.byref(st), s[0], s[1]) == ENOROOT:
+                    raise LyaError(ENOROOT, "no A > 0 reaches f_target")
+        return st.a, st.f_at_a, st.iters
+
+    use_sub = sub_every > 1 and n_pix_global >= sub_min_pix
+    if row_moments is not None or kernel_sums is not None or not use_sub:
+        s5, _ = local_sums(0.0, 1)                       # the A = 0 pass (row moments when there are some)
+        update(st, all_reduce(s5))
+        n_full += 1
+    if use_sub and not st.done:
+        a0, ss = st.a, None
+        while n_sub_passes < 12:
+            s5, npx = local_sums(a0 if ss is None else ss.a, sub_every)
+            n_sub_local = npx
+            red = all_reduce(s5 + [float(npx)])
+            if ss is None:
+                if red[5] < 1.0:
+                    break                                 # nothing in the subsample
+                ss = new_state(max(1e-3, rel_tol), red[5], a0)
+            rc = L.lya_root_update_moments(C.byref(ss), (C.c_double * 5)(*red[:5]))
+            n_sub_passes += 1
+            if rc != OK:
+                ss = None
+                break
+            if ss.done:
+                break
+        if ss is not None and 0.0 < ss.a < 1e30:
+            st = new_state(rel_tol, n_pix_global, ss.a)
+    while not st.done and n_full < max_iter:
+        s5, _ = local_sums(st.a, 1)
+        update(st, all_reduce(s5))
+        n_full += 1
+    if stats is not None:
+        stats.update(tau_passes=n_full, sub_passes=n_sub_passes, n_sub=n_sub_local)
+    return st.a, st.f_at_a, n_full

@@ -275,6 +275,63 @@ def test_normalize_closed_forms_and_errors(ctx):
         assert abs(si / e_.sum() - 1) < 1e-6 and abs(di / (t * e_).sum() - 1) < 1e-6
 
 
+def test_nested_normalisation_subsample_then_full(ctx, oracle):
+    """S4's nested iteration forced on a small, heavy-tailed, ragged tau: the subsample (every 4th 4 KiB chunk of the
+    aligned body) only supplies the starting point, so A must equal the oracle's root of the mean over ALL pixels, and
+    the plain iteration's A, to the iteration's tolerance; tau is then streamed once or twice instead of 4-5 times.  The
+    subsample sums themselves are checked against a float64 numpy sum over the chunks of the definition in lya.h."""
+    rng = np.random.default_rng(92)
+    n = 3_000_017
+    t = np.exp(rng.normal(-0.4, 2.3, n)).astype(np.float32)               # max ~ 1e5 x median
+    t[rng.integers(0, n, 50)] = 0.0
+    tau = torch.from_numpy(t).cuda()
+    A_ref, _, _ = oracle.normalize_mean_flux(t.astype(np.float64), 0.8)
+    try:
+        for view, off in ((tau, 0), (tau[3:], 3)):                        # aligned and unaligned (head scalars)
+            ctx.set_normalize_subsample(0, 0)
+            A0, _, it0, _ = ctx.normalize_mean_flux(view, 0.8)
+            st0 = ctx.last_normalize_stats()
+            assert st0 == dict(tau_passes=it0, sub_passes=0, row_pass=0, n_sub=0)
+            ctx.set_normalize_subsample(4, 0)
+            A1, f1, it1, _ = ctx.normalize_mean_flux(view, 0.8)
+            st1 = ctx.last_normalize_stats()
+            assert abs(A1 / A0 - 1) < 2e-7 and st1["sub_passes"] >= 2 and it1 == st1["tau_passes"] <= 2 < it0
+            if off == 0:
+                assert abs(A1 / A_ref - 1) < 1e-6
+            s, _ = ctx.flux_partial_sums(view, [A1])
+            assert abs(s[0] / view.numel() - 0.8) < 1e-6
+            # the subsample: float4 body after the head, chunks of 256 float4, every 4th
+            tv = t[off:].astype(np.float64)
+            head = (-(tau.data_ptr() + 4 * off) % 16) // 4
+            body = tv[head: head + ((tv.size - head) // 4) * 4]
+            chunks = [body[c: c + 1024] for c in range(0, body.size, 4096)]
+            sub = np.concatenate(chunks)
+            assert st1["n_sub"] == sub.size
+            sums, npx = ctx.flux_moment_sums_sub(view, 0.37, 4)
+            assert npx == sub.size
+            e = np.exp(-0.37 * sub)
+            for k in range(5):
+                assert abs(sums[k] / (sub ** k * e).sum() - 1) < 2e-6
+            full, npx1 = ctx.flux_moment_sums_sub(view, 0.37, 1)
+            assert npx1 == view.numel() and full == ctx.flux_moment_sums(view, 0.37)
+        # the sharded loop nests the same way and lands on the same root
+        ctx.set_normalize_subsample(0, 0)
+        stats = {}
+        A2, _, it2 = lya.normalize_mean_flux_sharded(ctx, tau, 0.8, n, sub_every=4, sub_min_pix=0, stats=stats)
+        assert abs(A2 / A_ref - 1) < 1e-6 and stats["sub_passes"] >= 2 and it2 <= 2
+        # a subsample of zeros (every chunk it holds is empty) must not derail the full iteration
+        z = tau.clone()
+        zb = z[(-z.data_ptr() % 16) // 4:]
+        for c in range(0, zb.numel(), 4096):
+            zb[c: c + 1024] = 0.0
+        ctx.set_normalize_subsample(4, 0)
+        A3, _, _, _ = ctx.normalize_mean_flux(z, 0.8)
+        A3_ref, _, _ = oracle.normalize_mean_flux(z.cpu().numpy().astype(np.float64), 0.8)
+        assert abs(A3 / A3_ref - 1) < 1e-6
+    finally:
+        ctx.set_normalize_subsample(32, 1 << 24)
+
+
 def test_flux_in_place_and_ragged(ctx, oracle):
     rng = np.random.default_rng(3)
     t = np.exp(rng.normal(-0.5, 1.5, 100_003)).astype(np.float32)

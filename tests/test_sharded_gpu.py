@@ -59,7 +59,8 @@ def _worker(rank: int, world: int, port: int, out_dir: str):
     # (2) the same shard from host buffers (global A again)
     dp, vp = dh.pin_memory(), vh.pin_memory()
     tau_h, flux_h = torch.empty_like(dp).pin_memory(), torch.empty_like(dp).pin_memory()
-    A2, fa2, it2 = lya.forest_host_sharded(ctx, p, 0, dp, vp, w.f_target, N ** 3, rel_tol=1e-9, slab_nz=16,
+    p_loc = lya.Params(**{**p.__dict__, "nz": nzl})               # lya_forest_host_begin takes the LOCAL grid
+    A2, fa2, it2 = lya.forest_host_sharded(ctx, p_loc, 0, dp, vp, w.f_target, N ** 3, rel_tol=1e-9, slab_nz=16,
                                            tau_h=tau_h, flux_h=flux_h)
     torch.cuda.synchronize()
     assert torch.equal(tau_h, tau.cpu())
