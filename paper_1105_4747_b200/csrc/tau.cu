@@ -58,7 +58,8 @@ struct TauArgs {
     float       *tau;
     int          n;           // pixels per sightline
     int          tiles;       // pixel tiles of 32*R per sightline
-    int          vec;         // x-axis: rows are 16-byte aligned and n % 4 == 0
+    int          vec;         // x-axis: tau rows are 16-byte aligned and n % 4 == 0
+    int          vec_in;      // x-axis: the input rows are (128-bit staging loads)
     int          bsl;         // strided: x-width of a gathered batch (power of 2)
     int          bshift;      // log2(bsl)
     int          cstride;     // strided: float4 cells per staged sightline (n + pad)
@@ -89,6 +90,14 @@ __device__ __forceinline__ float ex2_ftz(float x)
     return y;
 }
 
+// 1 / x to 1 ulp (MUFU.RCP) -- the IEEE division's slow-path branch kept the staging loop's loads from being batched
+__device__ __forceinline__ float rcp_approx(float x)
+{
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
 // round to nearest integer on the FP32 pipe (valid for |x| < 2^22; MUFU/XU-pipe FRND would compete with ex2)
 __device__ __forceinline__ float round_magic(float x)
 {
@@ -104,14 +113,14 @@ __device__ __forceinline__ float round_magic(float x)
 // below 1, so f carries an absolute error < 1e-7 pixel however large P is.  Precondition |v_pec| < 2^22 dv
 // (4e6 pixels; beyond it P is no longer an integer: the reach is set to +inf, which sends the sightline to the
 // general path with a meaningless but finite displacement).  No FP64 and, apart from one reciprocal, no
-// XU-pipe instruction.  jf = (float)j.  Reading C11: +v -> higher pixel index.
+// XU-pipe instruction (MUFU.RCP: 1 / b to 1 ulp).  jf = (float)j.  Reading C11: +v -> higher pixel index.
 __device__ __forceinline__ float stage_cell(const TauArgs &a, float jf, float nh, float bb, float vv, float4 &out)
 {
     const float P  = round_magic(vv * a.inv_dv_hi);
     const float f  = fmaf(vv, a.inv_dv_lo, fmaf(vv, a.inv_dv_hi, -P));
     // integer displacement reduced to [-N/2, N/2]; at an exact half-way point either image is nearest
     const float Pr = fmaf(-a.n_f, round_magic(P * a.inv_n), P);
-    const float ib = 1.0f / bb;
+    const float ib = rcp_approx(bb);
     const float w  = a.w_scale * ib;
     out.x = jf + Pr;
     out.y = w;
@@ -128,6 +137,30 @@ __device__ __forceinline__ float stage_from_global(const TauArgs &a, float jf, s
     if (FUSED) gas_cell(a.gas, __ldcs(a.n_hi + g), nh, bb);            // n_hi points at delta
     else { nh = __ldcs(a.n_hi + g); bb = __ldcs(a.b + g); }
     return stage_cell(a, jf, nh, bb, __ldcs(a.v + g), out);
+}
+
+// Four consecutive cells j .. j + 3 from 128-bit loads (rows 16-byte aligned, n % 4 == 0): a quarter of the load and
+// address instructions, and -- with no branch in stage_cell -- the compiler issues all loads of an unrolled batch before
+// the first conversion, so a thread waits for global memory once per batch instead of once per cell.
+template <bool FUSED>
+__device__ __forceinline__ void load4(const TauArgs &a, size_t g, float4 &nh, float4 &bb, float4 &vv)
+{
+    nh = __ldcs(reinterpret_cast<const float4 *>(a.n_hi + g));         // FUSED: delta
+    if (!FUSED) bb = __ldcs(reinterpret_cast<const float4 *>(a.b + g));
+    vv = __ldcs(reinterpret_cast<const float4 *>(a.v + g));
+}
+template <bool FUSED>
+__device__ __forceinline__ float stage4(const TauArgs &a, float jf, float4 nh, float4 bb, const float4 &vv, float4 (&out)[4])
+{
+    if (FUSED) {
+        const float4 d = nh;
+        gas_cell(a.gas, d.x, nh.x, bb.x); gas_cell(a.gas, d.y, nh.y, bb.y);
+        gas_cell(a.gas, d.z, nh.z, bb.z); gas_cell(a.gas, d.w, nh.w, bb.w);
+    }
+    float reach = stage_cell(a, jf, nh.x, bb.x, vv.x, out[0]);
+    reach = fmaxf(reach, stage_cell(a, jf + 1.0f, nh.y, bb.y, vv.y, out[1]));
+    reach = fmaxf(reach, stage_cell(a, jf + 2.0f, nh.z, bb.z, vv.z, out[2]));
+    return fmaxf(reach, stage_cell(a, jf + 3.0f, nh.w, bb.w, vv.w, out[3]));
 }
 
 // Staged cells are stored at cpos(j): plain for the full sum (every lane reads the same cell: broadcast).  For
@@ -322,13 +355,35 @@ __global__ void __launch_bounds__(1024, 1) tau_x_kernel(const TauArgs a, const i
 
         // ---- stage the row: (nHI, b, v_pec) [or delta, v_pec] -> (m, w, g, a) per cell; 128-byte coalesced loads
         float reach = 0.0f;
-        float jf = (float)gl;
+        if (a.vec_in) {                                  // four consecutive cells per thread and step, two steps in flight
+            int j = 4 * gl;
+            for (; j + 4 * gthreads < n; j += 8 * gthreads) {
+                float4 nh0, bb0, vv0, nh1, bb1, vv1, q[4];
+                load4<FUSED>(a, g0 + j, nh0, bb0, vv0);
+                load4<FUSED>(a, g0 + j + 4 * gthreads, nh1, bb1, vv1);
+                reach = fmaxf(reach, stage4<FUSED>(a, (float)j, nh0, bb0, vv0, q));
+#pragma unroll
+                for (int k = 0; k < 4; ++k) cells[cpos<WIN, R>(j + k)] = q[k];
+                reach = fmaxf(reach, stage4<FUSED>(a, (float)(j + 4 * gthreads), nh1, bb1, vv1, q));
+#pragma unroll
+                for (int k = 0; k < 4; ++k) cells[cpos<WIN, R>(j + 4 * gthreads + k)] = q[k];
+            }
+            if (j < n) {
+                float4 nh0, bb0, vv0, q[4];
+                load4<FUSED>(a, g0 + j, nh0, bb0, vv0);
+                reach = fmaxf(reach, stage4<FUSED>(a, (float)j, nh0, bb0, vv0, q));
+#pragma unroll
+                for (int k = 0; k < 4; ++k) cells[cpos<WIN, R>(j + k)] = q[k];
+            }
+        } else {
+            float jf = (float)gl;
 #pragma unroll 4
-        for (int j = gl; j < n; j += gthreads) {
-            float4 q;
-            reach = fmaxf(reach, stage_from_global<FUSED>(a, jf, g0 + j, q));
-            cells[cpos<WIN, R>(j)] = q;
-            jf += (float)gthreads;
+            for (int j = gl; j < n; j += gthreads) {
+                float4 q;
+                reach = fmaxf(reach, stage_from_global<FUSED>(a, jf, g0 + j, q));
+                cells[cpos<WIN, R>(j)] = q;
+                jf += (float)gthreads;
+            }
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) reach = fmaxf(reach, __shfl_xor_sync(0xffffffffu, reach, o));
@@ -574,6 +629,7 @@ lya_status lya_launch_tau(lya_ctx *ctx, int axis, int nx, int ny, int nz_local,
         a.n_sl = (long long)ny * nz_local;
         if (a.n_sl >= (1LL << 31)) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: more than 2^31 sightlines");
         a.vec = (n % 4 == 0) && (((uintptr_t)tau & 15) == 0);
+        a.vec_in = (n % 4 == 0) && ((((uintptr_t)n_hi | (uintptr_t)v | (fused ? 0 : (uintptr_t)b)) & 15) == 0);
         a.sched = ctx->d_sched;
 #define LYA_TAU_X(RR)                                                                                       \
     return win ? (fused ? launch_x<RR, true, true>(ctx, a) : launch_x<RR, false, true>(ctx, a))             \
