@@ -101,9 +101,10 @@ lya_status lya_tau_sightlines(lya_ctx *ctx, const lya_params *p, int axis, int32
 /* Work-efficient variants of S2 + S3, same arrays and conventions as
  * lya_tau_sightlines.  flags:
  *   LYA_TAU_WINDOWED      walk only the source cells that can contribute: a cell further from a pixel than
- *                         12.5 b_j sqrt(ln 2)/dv + |v_pec,j|/dv + 1 pixels adds ex2(-x^2) == 0 exactly in fp32, so
- *                         the result is BIT-IDENTICAL to the full sum while ~N / (128 + 2 reach) times fewer
- *                         pairs are evaluated.  Sightlines whose reach does not fit take the full loops.
+ *                         11.3 b_j sqrt(ln 2)/dv + |v_pec,j|/dv + 1 pixels adds ex2(-x^2) == 0 exactly in fp32 (the
+ *                         result, below 2^-127, is flushed; it is < 2^-127 of the cell's line-centre depth in exact
+ *                         arithmetic), so the result is BIT-IDENTICAL to the full sum while ~N / (4 + 2 reach) times
+ *                         fewer pairs are evaluated.  Sightlines whose reach does not fit take the full loops.
  *   LYA_TAU_FROM_DENSITY  S1 fused into the staging: n_hi_or_delta is delta (Eq.4/5 are applied per staged
  *                         cell with the arithmetic of lya_gas_from_density, so tau is bit-identical to the
  *                         two-call path); b_kms is ignored and may be NULL.

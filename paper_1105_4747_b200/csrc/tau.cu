@@ -24,8 +24,8 @@
 // Periodic wrap without per-pair work: a warp owns a tile of 32*R consecutive pixels and walks the sources
 // in UNWRAPPED order jj = c - N/2 ... c + N/2 - 1 around the tile centre c (two contiguous index segments),
 // so i - jj is already the nearest image for every pair that can contribute.  That is valid when, for every
-// source of the sightline, (N/2 - 16R - |P_j| - 1) w_j >= 12.5, i.e. a pair whose chosen image is not the
-// nearest has ex2(-x^2) == 0 in fp32 (and < 2^-156 of a_j in the oracle's double).  The staging pass checks
+// source of the sightline, (N/2 - 16R - |P_j| - 1/2) w_j >= 11.3, i.e. a pair whose chosen image is not the
+// nearest has ex2(-x^2) == 0 in fp32 (and < 2^-127 of a_j in the oracle's double).  The staging pass checks
 // the condition; a sightline that fails it (tiny N, |v_pec| of order V) takes the general loop with a
 // per-pair image choice.  Both loops evaluate all N^2 pairs.
 //
@@ -51,7 +51,7 @@ namespace {
 
 constexpr int   TAU_WARPS   = 8;       // strided kernel: warps per CTA
 constexpr int   TAU_THREADS = TAU_WARPS * 32;
-constexpr float TAU_XCUT    = 12.5f;   // ex2(-12.5^2) = 2^-156: exactly 0 in fp32 (ftz)
+constexpr float TAU_XCUT    = 11.3f;   // ex2.approx.ftz(-11.3^2) = 2^-127.7 is below 2^-126: flushed to exactly 0
 
 struct TauArgs {
     const float *n_hi, *b, *v;
@@ -105,7 +105,7 @@ __device__ __forceinline__ float round_magic(float x)
     return __fsub_rn(__fadd_rn(x, big), big);
 }
 
-// One source cell -> staged float4 (m, w, g, a).  Returns the cell's REACH in pixels, 12.5 / w_j + |P_j| + 1:
+// One source cell -> staged float4 (m, w, g, a).  Returns the cell's REACH in pixels, 11.3 / w_j + |P_j| + 1/2:
 // a pixel further than that from the (unwrapped) cell index gets ex2(-x^2) == 0 exactly from it.  The maximum
 // over a sightline decides between the fast and the general loop and sets the window of LYA_TAU_WINDOWED.
 // All fp32: p = v_pec/dv is split as P + f with P = round(v * inv_dv_hi) and f = fma(v, inv_dv_hi, -P) +
@@ -126,7 +126,7 @@ __device__ __forceinline__ float stage_cell(const TauArgs &a, float jf, float nh
     out.y = w;
     out.z = -f * w;
     out.w = (a.amp_scale * nh) * ib;
-    const float reach = fmaf(bb, a.xcut_over_w, fabsf(Pr) + 1.0f);
+    const float reach = fmaf(bb, a.xcut_over_w, fabsf(Pr) + 0.5078125f);   // 1/2 for |f|, 2^-7 for the roundings here
     return (fabsf(P) < 4194304.0f && reach >= 0.0f) ? reach : __int_as_float(0x7f800000);   // NaN -> +inf
 }
 
@@ -308,7 +308,7 @@ __device__ __forceinline__ int tile_any(const TauArgs &a, const float4 *cs, floa
         return n;
     }
     if (WIN) {
-        const int W = (((int)reach + 1) + R - 1) / R * R;   // whole pad groups on either side
+        const int W = ((int)reach + R - 1) / R * R;         // floor(reach), then whole pad groups on either side
         if (W + R <= TAU_HALO && n >= TAU_HALO) {
             tile_window<R>(cs, n, i0, lane, W, acc);
             return 2 * W + R;
