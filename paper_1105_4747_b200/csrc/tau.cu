@@ -163,13 +163,30 @@ __device__ __forceinline__ float stage4(const TauArgs &a, float jf, float4 nh, f
     return fmaxf(reach, stage_cell(a, jf + 3.0f, nh.w, bb.w, vv.w, out[3]));
 }
 
-// Staged cells are stored at cpos(j): plain for the full sum (every lane reads the same cell: broadcast).  For
-// LYA_TAU_WINDOWED, where lane k reads cell j0 + R k, the row is stored UNWRAPPED with a periodic halo of TAU_HALO
-// cells on either side (slot j + TAU_HALO holds cell j; the halo copies carry m -/+ N, so a walk across the ends
-// needs no wrap logic at all) and with one pad slot per R cells, s + s / R: the lanes of an LDS.128 phase then sit
+// ---- the staged layout: sources in PAIRS.  Cells 2p and 2p + 1 of a row share two float4 slots,
+//     slot 2p     A = (m_2p, m_2p+1, w_2p, w_2p+1)        slot 2p + 1   B = (g_2p, g_2p+1, a_2p, a_2p+1)
+// so that an LDS.128 of A and one of B hand the pair loop (m, m'), (w, w'), (g, g'), (a, a') as aligned 64-bit register
+// pairs: the loop body is packed FP32 (sub/fma/mul.rn.f32x2: FADD2, FFMA2, FMUL2) on two SOURCES at a time -- for four
+// pixels per lane 23 issue slots per 8 pairs instead of 36, which is what the windowed variant, short of issue slots,
+// needs (profiles/r2_ncu_tau_windowed.md); each f32x2 lane is the scalar operation, bit for bit.  Every pixel keeps an
+// (even sources, odd sources) pair of partial sums, added at the end; the full and the windowed walks both start at an
+// even unwrapped source index, so they add the same terms in the same order and stay bit-identical.  The fast walks
+// need n % 4 == 0 (even segment ends for any tile); other rows take the general loop.
+// Slots are stored at cpos(slot): plain for the full sum (every lane reads the same slot: broadcast).  For
+// LYA_TAU_WINDOWED, where lane k reads slot s0 + R k, the row is stored UNWRAPPED with a periodic halo of TAU_HALO
+// cells on either side (slot j + TAU_HALO holds slot j; the halo copies carry m -/+ N, so a walk across the ends
+// needs no wrap logic at all) and with one pad slot per R slots, s + s / R: the lanes of an LDS.128 phase then sit
 // (R + 1) float4 apart, and R + 1 being odd the eight of them fall into the eight different 16-byte bank groups
-// (R = 1 needs no pad: neighbouring cells).
+// (R = 1 needs no pad: neighbouring lanes share a pair).
 constexpr int TAU_HALO = 64;           // multiple of 4; a sightline whose window does not fit takes the full loops
+
+typedef unsigned long long f32x2;      // two packed floats (lo, hi) in one 64-bit register pair
+__device__ __forceinline__ f32x2 pk(float lo, float hi) { f32x2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ void unpk(f32x2 v, float &lo, float &hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) { f32x2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b)); return r; }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c)); return r; }
 
 template <bool WIN, int R> __device__ __forceinline__ int cpos(int j)
 {
@@ -179,29 +196,84 @@ template <bool WIN, int R> __device__ __forceinline__ int cpos(int j)
 }
 template <int R> __host__ __device__ constexpr int crow_len(int n, bool win)        // slots of one staged row
 {
-    return !win ? n : (R > 1 ? (n + 2 * TAU_HALO) + (R == 2 ? ((n + 2 * TAU_HALO) >> 1) : ((n + 2 * TAU_HALO) >> 2)) + 1
-                             : n + 2 * TAU_HALO);
+    const int ne = (n + 1) & ~1;                          // an odd row gets a dummy last cell (amplitude 0)
+    return !win ? ne : (R > 1 ? (ne + 2 * TAU_HALO) + (R == 2 ? ((ne + 2 * TAU_HALO) >> 1) : ((ne + 2 * TAU_HALO) >> 2)) + 1
+                              : ne + 2 * TAU_HALO);
 }
 
-// LYA_TAU_WINDOWED: after the row is staged (and the group has synchronised), fill the halo: slot of index -t is
-// cell N - t with m - N, slot of index N - 1 + t is cell t - 1 with m + N (t = 1 .. TAU_HALO).  Rows shorter than
-// the halo never take the window (tile_any), so they skip this.
+// one staged cell -> its half of the pair's two slots (scalar stores: the strided gather and unaligned rows)
+template <bool WIN, int R>
+__device__ __forceinline__ void put_cell(float4 *cs, int j, const float4 &q)
+{
+    float *fa = reinterpret_cast<float *>(cs + cpos<WIN, R>(j & ~1)) + (j & 1);
+    float *fb = reinterpret_cast<float *>(cs + cpos<WIN, R>((j & ~1) + 1)) + (j & 1);
+    fa[0] = q.x; fa[2] = q.y; fb[0] = q.z; fb[2] = q.w;
+}
+// four consecutive cells j .. j + 3 (j % 4 == 0) -> four slots, 128-bit stores
+template <bool WIN, int R>
+__device__ __forceinline__ void put_cells4(float4 *cs, int j, const float4 (&q)[4])
+{
+    cs[cpos<WIN, R>(j)]     = make_float4(q[0].x, q[1].x, q[0].y, q[1].y);
+    cs[cpos<WIN, R>(j + 1)] = make_float4(q[0].z, q[1].z, q[0].w, q[1].w);
+    cs[cpos<WIN, R>(j + 2)] = make_float4(q[2].x, q[3].x, q[2].y, q[3].y);
+    cs[cpos<WIN, R>(j + 3)] = make_float4(q[2].z, q[3].z, q[2].w, q[3].w);
+}
+// an odd row's dummy cell n: amplitude 0, finite width, so the pair it shares with cell n - 1 is harmless
+template <bool WIN, int R>
+__device__ __forceinline__ void put_dummy(float4 *cs, int n)
+{
+    if (n & 1) put_cell<WIN, R>(cs, n, make_float4(0.0f, 1.0f, 0.0f, 0.0f));
+}
+template <bool WIN, int R>
+__device__ __forceinline__ float4 get_cell(const float4 *cs, int j)
+{
+    const float *fa = reinterpret_cast<const float *>(cs + cpos<WIN, R>(j & ~1)) + (j & 1);
+    const float *fb = reinterpret_cast<const float *>(cs + cpos<WIN, R>((j & ~1) + 1)) + (j & 1);
+    return make_float4(fa[0], fa[2], fb[0], fb[2]);
+}
+
+// LYA_TAU_WINDOWED: after the row is staged (and the group has synchronised), fill the halo: slot -t is slot N - t
+// with m - N, slot N - 1 + t is slot t - 1 with m + N (t = 1 .. TAU_HALO); only the A slots (even) carry m.  N % 4 == 0
+// here (tile_any), so source and destination slots have the same parity.  Rows shorter than the halo never take
+// the window, so they skip this.
 template <int R>
 __device__ __forceinline__ void fill_halo(float4 *cs, int n, float n_f, int t0, int nthreads)
 {
-    if (n < TAU_HALO) return;
+    if (n < TAU_HALO || (n & 3)) return;
     for (int t = t0; t < 2 * TAU_HALO; t += nthreads) {
         const bool left = t < TAU_HALO;
         const int src = left ? n - TAU_HALO + t : t - TAU_HALO;
         const int dst = left ? t - TAU_HALO : n + t - TAU_HALO;
         float4 q = cs[cpos<true, R>(src)];
-        q.x += left ? -n_f : n_f;                         // exact: integer-valued floats far below 2^24
+        if (!(t & 1)) {                                   // exact: integer-valued floats far below 2^24
+            q.x += left ? -n_f : n_f;
+            q.y += left ? -n_f : n_f;
+        }
         cs[cpos<true, R>(dst)] = q;
     }
 }
 
+// Two sources (one pair of slots) against the R pixels of a lane: cref2 = (c, c) with c the reference pixel's
+// (unwrapped) index, so E = c - m is the exact integer separation; acc2[r] = (sum over even, sum over odd sources).
+template <int R>
+__device__ __forceinline__ void pair_step(const float4 &A, const float4 &B, f32x2 cref2, f32x2 (&acc2)[R])
+{
+    constexpr int RH = R / 2;
+    const f32x2 m2 = pk(A.x, A.y), w2 = pk(A.z, A.w), g2 = pk(B.x, B.y), a2 = pk(B.z, B.w);
+    const f32x2 xr = fma2(sub2(cref2, m2), w2, g2);
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        // x_r = (r - RH) w + x_ref, one rounding: +-1 as a packed add / subtract, the others as a packed fma
+        const f32x2 x = (r == RH) ? xr : (r == RH + 1) ? add2(xr, w2) : (r == RH - 1) ? sub2(xr, w2)
+                                       : fma2(pk((float)(r - RH), (float)(r - RH)), w2, xr);
+        float t0, t1;
+        unpk(mul2(x, x), t0, t1);
+        acc2[r] = fma2(a2, pk(ex2_ftz(-t0), ex2_ftz(-t1)), acc2[r]);
+    }
+}
+
 // Fast path, full sum: unwrapped walk over all n sources jj = start .. start + n - 1 around the tile centre (at
-// most one wrap), no per-pair image logic.  Lane owns pixels i0 + lane*R + r.
+// most one wrap), no per-pair image logic.  Lane owns pixels i0 + lane*R + r.  n % 4 == 0: start, j0 and n are even.
 template <int R, bool PAD>
 __device__ __forceinline__ void tile_fast(const float4 *__restrict__ cs, int n, int i0, int lane, float (&acc)[R])
 {
@@ -211,66 +283,67 @@ __device__ __forceinline__ void tile_fast(const float4 *__restrict__ cs, int n, 
     if (j0 < 0) j0 += n;                               // slot holding jj = start
     const int off = start - j0;                        // jj = j + off on [j0, n), jj = j + off + n on [0, j0)
     float cref = (float)(i0 + lane * R + RH - off);
+    f32x2 acc2[R];
 #pragma unroll
-    for (int r = 0; r < R; ++r) acc[r] = 0.0f;
+    for (int r = 0; r < R; ++r) acc2[r] = 0ull;
 #pragma unroll 1
     for (int seg = 0; seg < 2; ++seg) {
         const int lo = seg ? 0 : j0, hi = seg ? j0 : n;
-#pragma unroll 8
-        for (int j = lo; j < hi; ++j) {
-            const float4 q = cs[cpos<PAD, R>(j)];
-            const float E  = cref - q.x;
-            const float xr = fmaf(E, q.y, q.z);
-#pragma unroll
-            for (int r = 0; r < R; ++r) {
-                const float x = (r == RH) ? xr : fmaf((float)(r - RH), q.y, xr);
-                const float e = ex2_ftz(-(x * x));
-                acc[r] = fmaf(q.w, e, acc[r]);
-            }
-        }
+        const f32x2 cref2 = pk(cref, cref);
+#pragma unroll 4
+        for (int j = lo; j < hi; j += 2) pair_step<R>(cs[cpos<PAD, R>(j)], cs[cpos<PAD, R>(j + 1)], cref2, acc2);
         cref -= (float)n;
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        float lo, hi;
+        unpk(acc2[r], lo, hi);
+        acc[r] = lo + hi;
     }
 }
 
-// LYA_TAU_WINDOWED: every LANE walks only its own window jj = il - W .. il + R - 1 + W around its R pixels
-// (il = i0 + lane R; W = the sightline's reach rounded up to a multiple of R): 2 W + R sources instead of n.  A
-// source outside the window is further than its reach from all R pixels, so it would have added ex2(..) == 0
-// exactly; the sources kept are added in the same ascending order with the same arithmetic (same reference pixel,
-// the same exact integer separation E), so the result is bit-identical to tile_fast.  The row is stored unwrapped
-// with a halo (cpos<true, R>), and il and W being multiples of R the walk is whole pad groups: R consecutive slots,
-// then one pad slot -- every LDS.128 offset is an immediate, there is no wrap test and no index arithmetic in the
-// loop, which is what lets the MUFU pipe set the pace as in the full sum.
+// LYA_TAU_WINDOWED: every LANE walks only its own window jj = s0 .. around its R pixels (il = i0 + lane R): from
+// s0 = il - W (W = the sightline's reach rounded up to a multiple of R; R = 1: rounded down to even) up to at least
+// il + R - 1 + W, in whole pairs.  A source outside the window is further than its reach from all R pixels, so it would
+// have added ex2(..) == 0 exactly; the sources kept are added in the same ascending order, into the same (even, odd)
+// partial sums, with the same arithmetic (same reference pixel, the same exact integer separation E), so the result is
+// bit-identical to tile_fast.  The row is stored unwrapped with a halo (cpos<true, R>), and s0 + TAU_HALO being a
+// multiple of R the walk is whole pad groups: R consecutive slots, then one pad slot -- every LDS.128 offset is an
+// immediate, there is no wrap test and no index arithmetic in the loop.  Returns the sources walked.
 template <int R>
-__device__ __forceinline__ void tile_window(const float4 *__restrict__ cs, int n, int i0, int lane, int W,
-                                            float (&acc)[R])
+__device__ __forceinline__ int tile_window(const float4 *__restrict__ cs, int n, int i0, int lane, int W,
+                                           float (&acc)[R])
 {
     constexpr int RH = R / 2;
+    constexpr int PG = R > 1 ? R : 2;                     // slots per pad group (R = 1: one pair, no pad)
     const int il = i0 + lane * R;
 #pragma unroll
     for (int r = 0; r < R; ++r) acc[r] = 0.0f;
-    if (il >= n) return;                                  // ragged last tile: this lane owns no pixel
-    const float4 *q4 = cs + cpos<true, R>(il - W);        // slot of the first source; (il - W + TAU_HALO) % R == 0
-    const float cref = (float)(il + RH);
-    const int groups = (2 * W + R) / R;
+    const int s0l = R > 1 ? il - W : (il - W) - ((il - W) & 1);
+    const int groups = R > 1 ? (2 * W + R) / R : (il + W - s0l + 2) / 2;
+    const int walked = groups * PG;                       // lane 0's count is the tile's (R = 1: +-1 between lanes)
+    if (il >= n) return walked;                           // ragged last tile: this lane owns no pixel
+    const float4 *q4 = cs + cpos<true, R>(s0l);           // slot of the first source; (s0l + TAU_HALO) % PG == 0
+    const f32x2 cref2 = pk((float)(il + RH), (float)(il + RH));
+    f32x2 acc2[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) acc2[r] = 0ull;
 #pragma unroll 2
     for (int g = 0; g < groups; ++g) {
 #pragma unroll
-        for (int k = 0; k < R; ++k) {
-            const float4 q = q4[k];
-            const float E  = cref - q.x;
-            const float xr = fmaf(E, q.y, q.z);
-#pragma unroll
-            for (int r = 0; r < R; ++r) {
-                const float x = (r == RH) ? xr : fmaf((float)(r - RH), q.y, xr);
-                const float e = ex2_ftz(-(x * x));
-                acc[r] = fmaf(q.w, e, acc[r]);
-            }
-        }
-        q4 += R > 1 ? R + 1 : 1;
+        for (int k = 0; k < PG; k += 2) pair_step<R>(q4[k], q4[k + 1], cref2, acc2);
+        q4 += R > 1 ? R + 1 : 2;
     }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        float lo, hi;
+        unpk(acc2[r], lo, hi);
+        acc[r] = lo + hi;
+    }
+    return walked;
 }
 
-// General path: nearest image chosen per pair (tiny N, or |v_pec| comparable to the box).
+// General path: nearest image chosen per pair (tiny N, N % 4 != 0, or |v_pec| comparable to the box).
 template <int R, bool PAD>
 __device__ __forceinline__ void tile_general(const float4 *__restrict__ cs, int n, float n_f, float inv_n, int i0,
                                              int lane, float (&acc)[R])
@@ -283,7 +356,7 @@ __device__ __forceinline__ void tile_general(const float4 *__restrict__ cs, int 
     }
 #pragma unroll 2
     for (int j = 0; j < n; ++j) {
-        const float4 q = cs[cpos<PAD, R>(j)];
+        const float4 q = get_cell<PAD, R>(cs, j);
         const float  f = -q.z / q.y;                    // fractional displacement (only picks the image)
 #pragma unroll
         for (int r = 0; r < R; ++r) {
@@ -303,16 +376,13 @@ __device__ __forceinline__ int tile_any(const TauArgs &a, const float4 *cs, floa
                                         float (&acc)[R])
 {
     const int n = a.n;
-    if (!(reach <= (float)((n >> 1) - 16 * R))) {       // also catches +inf
+    if ((n & 3) || !(reach <= (float)((n >> 1) - 16 * R))) {   // also catches +inf
         tile_general<R, WIN>(cs, n, a.n_f, a.inv_n, i0, lane, acc);
         return n;
     }
     if (WIN) {
         const int W = ((int)reach + R - 1) / R * R;         // floor(reach), then whole pad groups on either side
-        if (W + R <= TAU_HALO && n >= TAU_HALO) {
-            tile_window<R>(cs, n, i0, lane, W, acc);
-            return 2 * W + R;
-        }
+        if (W + R + 2 <= TAU_HALO && n >= TAU_HALO) return tile_window<R>(cs, n, i0, lane, W, acc);
     }
     tile_fast<R, WIN>(cs, n, i0, lane, acc);
     return n;
@@ -362,18 +432,15 @@ __global__ void __launch_bounds__(1024, 1) tau_x_kernel(const TauArgs a, const i
                 load4<FUSED>(a, g0 + j, nh0, bb0, vv0);
                 load4<FUSED>(a, g0 + j + 4 * gthreads, nh1, bb1, vv1);
                 reach = fmaxf(reach, stage4<FUSED>(a, (float)j, nh0, bb0, vv0, q));
-#pragma unroll
-                for (int k = 0; k < 4; ++k) cells[cpos<WIN, R>(j + k)] = q[k];
+                put_cells4<WIN, R>(cells, j, q);
                 reach = fmaxf(reach, stage4<FUSED>(a, (float)(j + 4 * gthreads), nh1, bb1, vv1, q));
-#pragma unroll
-                for (int k = 0; k < 4; ++k) cells[cpos<WIN, R>(j + 4 * gthreads + k)] = q[k];
+                put_cells4<WIN, R>(cells, j + 4 * gthreads, q);
             }
             if (j < n) {
                 float4 nh0, bb0, vv0, q[4];
                 load4<FUSED>(a, g0 + j, nh0, bb0, vv0);
                 reach = fmaxf(reach, stage4<FUSED>(a, (float)j, nh0, bb0, vv0, q));
-#pragma unroll
-                for (int k = 0; k < 4; ++k) cells[cpos<WIN, R>(j + k)] = q[k];
+                put_cells4<WIN, R>(cells, j, q);
             }
         } else {
             float jf = (float)gl;
@@ -381,9 +448,10 @@ __global__ void __launch_bounds__(1024, 1) tau_x_kernel(const TauArgs a, const i
             for (int j = gl; j < n; j += gthreads) {
                 float4 q;
                 reach = fmaxf(reach, stage_from_global<FUSED>(a, jf, g0 + j, q));
-                cells[cpos<WIN, R>(j)] = q;
+                put_cell<WIN, R>(cells, j, q);
                 jf += (float)gthreads;
             }
+            if (gl == 0) put_dummy<WIN, R>(cells, n);
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) reach = fmaxf(reach, __shfl_xor_sync(0xffffffffu, reach, o));
@@ -490,9 +558,10 @@ __global__ void __launch_bounds__(TAU_THREADS) tau_strided_kernel(const TauArgs 
             if (bx < nb) {
                 float4 q;
                 reach = fmaxf(reach, stage_from_global<FUSED>(a, (float)j, (size_t)(base + (long long)j * a.stride + bx), q));
-                cells[bx * cstride + cpos<WIN, R>(j)] = q;
+                put_cell<WIN, R>(cells + bx * cstride, j, q);
             }
         }
+        if (tid < nb) put_dummy<WIN, R>(cells + tid * cstride, n);
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) reach = fmaxf(reach, __shfl_xor_sync(0xffffffffu, reach, o));
         __syncthreads();                                 // s_reach zeroed; s_batch read by everyone
