@@ -3,7 +3,7 @@
 // additive noise N(0,1)/(S/N) from caller-supplied unit draws.  DESIGN.md readings O1-O3.
 //
 //   Fc(i)  = sum_k g(k) F(i-k),  g(k) ~ exp(-(k dv)^2 / 2 sigma^2) over the nearest periodic image,
-//            normalised by the discrete sum; taps below 9e-8 of the peak are dropped (5.7 sigma)
+//            normalised by the discrete sum; taps beyond 5 sigma are dropped (5.7e-7 of the kernel: |error| <= 5.7e-7)
 //   Fb(m)  = (1/B) integral over [m B, (m+1) B) of the piecewise-constant Fc       (B = bin / dv in pixels)
 //   out    = Fb + unit_noise / snr
 //
@@ -253,31 +253,43 @@ __global__ void __launch_bounds__(256) observe_rows_lean_kernel(const ObsArgs a,
 
     float4 reg[NV];                                      // this thread's pixels 4 (tid + q T) .. + 3
     float hreg = 0.0f, nzr[OBS_NBR];
-    auto fetch = [&](size_t row) {
-        const float *src = a.flux + row * (size_t)n;
+    // everything that does not depend on the row is computed once: offsets are 32-bit, the row pointers advance by a
+    // constant stride (the per-row 64-bit multiplies and the lambdas' re-derived addresses were a third of the
+    // instructions: profiles/r2_ncu_next_rows.md)
+    const int nb = a.nb;
+    const bool has_halo = tid < a.L;
+    const int hsrc = tid < a.KO ? n - a.KO + tid : tid - a.KO;       // this thread's halo pixel and where it goes
+    const int hdst = tid < a.KO ? tid : n + tid;
+    const size_t row_step = gridDim.x;
+    const float *src = a.flux + (size_t)blockIdx.x * n;               // row being fetched
+    const float *nz  = a.noise ? a.noise + (size_t)blockIdx.x * nb : nullptr;   // row being written
+    float *dst = a.out + (size_t)blockIdx.x * nb;
+    const size_t src_step = row_step * n, out_step = row_step * nb;
+    auto fetch = [&]() {
 #pragma unroll
         for (int q = 0; q < NV; ++q) {
             const int p = 4 * (tid + q * T);
             reg[q] = p < n ? __ldcs(reinterpret_cast<const float4 *>(src + p)) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
-        if (tid < a.L) hreg = __ldg(src + (tid < a.KO ? n - a.KO + tid : tid - a.KO));
+        if (has_halo) hreg = __ldg(src + hsrc);
+        src += src_step;
     };
     size_t row = blockIdx.x;
-    if (row < a.n_rows) fetch(row);
-    for (; row < a.n_rows; row += gridDim.x) {
+    if (row < a.n_rows) fetch();
+    for (; row < a.n_rows; row += row_step) {
         __syncthreads();                                 // previous row's s_in / s_c consumed
 #pragma unroll
         for (int q = 0; q < NV; ++q) {
             const int p = 4 * (tid + q * T);
             if (p < n) *reinterpret_cast<float4 *>(s_in + a.KO + p) = reg[q];
         }
-        if (tid < a.L) s_in[tid < a.KO ? tid : n + tid] = hreg;
-        if (row + gridDim.x < a.n_rows) fetch(row + gridDim.x);
-        if (a.noise) {
+        if (has_halo) s_in[hdst] = hreg;
+        if (row + row_step < a.n_rows) fetch();
+        if (nz) {
 #pragma unroll
             for (int k = 0; k < OBS_NBR; ++k) {
                 const int m = tid + k * T;
-                nzr[k] = m < a.nb ? __ldcs(a.noise + row * (size_t)a.nb + m) : 0.0f;
+                nzr[k] = m < nb ? __ldcs(nz + m) : 0.0f;
             }
         }
         __syncthreads();
@@ -317,38 +329,52 @@ __global__ void __launch_bounds__(256) observe_rows_lean_kernel(const ObsArgs a,
         }
         __syncthreads();
 
-        float *dst = a.out + row * (size_t)a.nb;
-        const float *nz = a.noise ? a.noise + row * (size_t)a.nb : nullptr;
-        auto rebinned = [&](int m) -> float {
-            if (a.bins3) {                                                        // bins <= 2 pixels wide: at most three
-                const int4 e = s_b[m];                                            // pixels overlap -> {i0, w0, w1, w2}
-                return fmaf(__int_as_float(e.w), s_c[e.x + 2],
-                            fmaf(__int_as_float(e.z), s_c[e.x + 1], __int_as_float(e.y) * s_c[e.x]));
+        // output bins m = tid + k T: the three rebinning modes are uniform over the launch, so each gets its own loop
+        const float inv_snr = nz ? a.inv_snr : 0.0f;
+        auto put = [&](int k, int m, float v) {
+            if (nz) v = fmaf(k < OBS_NBR ? nzr[k < OBS_NBR ? k : 0] : __ldcs(nz + m), inv_snr, v);
+            __stcs(dst + m, v);
+        };
+        if (a.bins3) {                                   // bins <= 2 pixels wide: three pixels {i0, w0, w1, w2}
+#pragma unroll
+            for (int k = 0; k < OBS_NBR; ++k) {
+                const int m = tid + k * T;
+                if (m < nb) {
+                    const int4 e = s_b[m];
+                    const float *c = s_c + e.x;
+                    put(k, m, fmaf(__int_as_float(e.w), c[2], fmaf(__int_as_float(e.z), c[1], __int_as_float(e.y) * c[0])));
+                }
             }
-            if (a.rebin) {
+            for (int m = tid + OBS_NBR * T; m < nb; m += T) {
                 const int4 e = s_b[m];
-                if (e.y <= e.x) return __int_as_float(e.z) * s_c[e.x];            // bin inside one pixel
-                float mid = 0.0f;                                                 // weights carry the 1/B
+                const float *c = s_c + e.x;
+                put(OBS_NBR, m, fmaf(__int_as_float(e.w), c[2], fmaf(__int_as_float(e.z), c[1], __int_as_float(e.y) * c[0])));
+            }
+        } else if (a.rebin) {                            // wide bins: first pixel, whole pixels, last pixel (weights carry 1/B)
+            auto wide = [&](int m) -> float {
+                const int4 e = s_b[m];
+                if (e.y <= e.x) return __int_as_float(e.z) * s_c[e.x];
+                float mid = 0.0f;
 #pragma unroll 1
                 for (int i = e.x + 1; i < e.y; ++i) mid += s_c[i];
                 return fmaf(__int_as_float(e.w), s_c[e.y], fmaf(mid, a.inv_bin_f, __int_as_float(e.z) * s_c[e.x]));
-            }
-            return s_c[m];
-        };
+            };
 #pragma unroll
-        for (int k = 0; k < OBS_NBR; ++k) {                                       // noise of these bins is in registers
-            const int m = tid + k * T;
-            if (m < a.nb) {
-                float v = rebinned(m);
-                if (nz) v = fmaf(nzr[k], a.inv_snr, v);
-                __stcs(dst + m, v);
+            for (int k = 0; k < OBS_NBR; ++k) {
+                const int m = tid + k * T;
+                if (m < nb) put(k, m, wide(m));
             }
+            for (int m = tid + OBS_NBR * T; m < nb; m += T) put(OBS_NBR, m, wide(m));
+        } else {
+#pragma unroll
+            for (int k = 0; k < OBS_NBR; ++k) {
+                const int m = tid + k * T;
+                if (m < nb) put(k, m, s_c[m]);
+            }
+            for (int m = tid + OBS_NBR * T; m < nb; m += T) put(OBS_NBR, m, s_c[m]);
         }
-        for (int m = tid + OBS_NBR * T; m < a.nb; m += T) {
-            float v = rebinned(m);
-            if (nz) v = fmaf(__ldcs(nz + m), a.inv_snr, v);
-            __stcs(dst + m, v);
-        }
+        dst += out_step;
+        if (nz) nz += out_step;
     }
 }
 
@@ -439,7 +465,8 @@ extern "C" lya_status lya_observe_rows(lya_ctx *ctx, size_t n_rows, int32_t n_pi
     a.L = -1;
     if (inst->fwhm_kms > 0.0) {
         const double sigma_px = inst->fwhm_kms / (2.0 * sqrt(2.0 * log(2.0))) / dv_kms;
-        const double kd = ceil(5.7 * sigma_px);                         // taps below exp(-5.7^2/2) = 9e-8 of the peak dropped
+        // taps beyond 5 sigma dropped: the two tails hold erfc(5 / sqrt 2) = 5.7e-7 of the kernel, so |error| <= 5.7e-7 max F
+        const double kd = ceil(5.0 * sigma_px);
         const int K = kd < 1.0 ? 1 : (kd > 1.0e6 ? 1000000 : (int)kd);
         a.Kl = K < (n_pix - 1) / 2 ? K : (n_pix - 1) / 2;
         a.Kr = K < n_pix / 2 ? K : n_pix / 2;
