@@ -7,10 +7,14 @@
 // from global memory, coalesced), applies the pass twiddles (one table look-up, the powers by at most four
 // complex products), does the R-point DFT in registers (radix-2 DIF with compile-time constants) and
 // scatters the result to the other shared-memory buffer, whose index is padded by one slot in 16 so that the
-// stride-R scatter of the first pass is bank-conflict free.  |X|^2 is accumulated in double per CTA and added
-// to the global accumulator once at the end.  4 B read per pixel; N = 1024 makes 3 passes = 2 shared-memory
-// round trips per point (the radix-2 version this replaces made 10, with a barrier each).  The butterflies'
-// complex additions are packed FP32 (add/sub.rn.f32x2) for rows of 512 pixels and more.
+// stride-R scatter of the first pass is bank-conflict free.  4 B read per pixel; N = 1024 makes 3 passes = 2
+// shared-memory round trips per point (the radix-2 version this replaces made 10, with a barrier each).  The
+// butterflies' complex additions are packed FP32 (add/sub.rn.f32x2) for rows of 512 pixels and more.
+// The two rows never have to be separated: |X_A(m)|^2 + |X_B(m)|^2 = (|Z(m)|^2 + |Z(N-m)|^2) / 2, and only the sum
+// over rows is wanted, so for the common sizes (256 ... 4096 pixels) the LAST pass keeps |Z(k)|^2 of its own outputs
+// in double registers across all the CTA's row pairs -- no final store, no read-out pass, two barriers per pair
+// instead of four -- and the host folds k and N - k once at the end.  Other sizes write the last pass to shared
+// memory and read the pairs (m, N - m) out (accumulated in double per CTA).
 #include "lya_internal.h"
 
 namespace {
@@ -91,9 +95,10 @@ template <int R> __device__ __forceinline__ constexpr int bitrev(int t)
 // FIRST: `in` is global memory (two rows -> one complex sequence, dF = F inv_mean - 1).
 // N_CT / NS_CT > 0: row length and ns known at compile time (the common sizes), which turns every shared-memory
 // offset below into an immediate; 0: taken from the arguments.
-template <int R, bool FIRST, int N_CT = 0, int NS_CT = 0>
+template <int R, bool FIRST, int N_CT = 0, int NS_CT = 0, bool LAST = false>
 __device__ __forceinline__ void stockham_pass(const PowArgs &a, const float *ra, const float *rb, bool has_b,
-                                              const float2 *in, float2 *out, const float2 *tw, int ns_rt)
+                                              const float2 *in, float2 *out, const float2 *tw, int ns_rt,
+                                              double *pacc = nullptr)
 {
     const int n = N_CT > 0 ? N_CT : a.n, m = n / R;
     const int ns = NS_CT > 0 ? NS_CT : ns_rt;
@@ -131,6 +136,14 @@ __device__ __forceinline__ void stockham_pass(const PowArgs &a, const float *ra,
             for (int t = 1; t < R; ++t) v[t] = cmul(v[t], w[t]);
         }
         dft_regs<R, (N_CT == 0 || N_CT >= 512)>(v);
+        if (LAST) {                                       // m <= blockDim.x here: one trip, pacc[t] belongs to output j + t ns
+#pragma unroll
+            for (int t = 0; t < R; ++t) {
+                const float2 z = v[bitrev<R>(t)];
+                pacc[t] += (double)fmaf(z.x, z.x, z.y * z.y);
+            }
+            continue;
+        }
         float2 *ob = out + pad16((j - k) * R + k);
         if (ns == 2 || ns == 4) {                         // never produced by the plans (radices 16 / 8 first)
 #pragma unroll
@@ -167,28 +180,32 @@ __global__ void __launch_bounds__(256) flux_power_kernel(const PowArgs a)
     }
     for (int m = tid; m <= nh; m += T) pw[m] = 0.0;
 
+    __syncthreads();                                       // tables built
+    constexpr int RL = N_CT > 0 ? (plan_radix(N_CT, 2) > 0 ? plan_radix(N_CT, 2) : plan_radix(N_CT, 1)) : 1;
+    double pacc[RL];                                       // compile-time plans: |Z(k)|^2 of this thread's last-pass outputs
+#pragma unroll
+    for (int t = 0; t < RL; ++t) pacc[t] = 0.0;
     const size_t n_pairs = (a.n_rows + 1) >> 1;
     for (size_t pair = blockIdx.x; pair < n_pairs; pair += gridDim.x) {
         const float *ra = a.flux + (2 * pair) * (size_t)n;
         const bool has_b = 2 * pair + 1 < a.n_rows;
         const float *rb = ra + n;
-        __syncthreads();                                   // previous pair's read-out done (and tables built)
+        // the buffer the first pass writes was last read in the previous pair's LAST pass (two-pass plans, and the
+        // read-out of the run-time plans); with three passes a barrier already lies in between
+        if constexpr (!(N_CT > 0 && plan_radix(N_CT, 2) > 0)) __syncthreads();
         float2 *src = bufB, *dst = bufA;
         if constexpr (N_CT > 0) {                          // compile-time plan: immediates everywhere
             constexpr int R0 = plan_radix(N_CT, 0), R1 = plan_radix(N_CT, 1), R2 = plan_radix(N_CT, 2);
             stockham_pass<R0, true, N_CT, 1>(a, ra, rb, has_b, nullptr, bufA, tw, 1);
-            __syncthreads();
-            src = bufA;
-            if constexpr (R1 > 0) {
+            __syncthreads();                               // (also: the previous pair's last pass has read bufB / bufA)
+            if constexpr (R2 > 0) {
                 stockham_pass<R1, false, N_CT, R0>(a, ra, rb, has_b, bufA, bufB, tw, R0);
                 __syncthreads();
-                src = bufB;
+                stockham_pass<R2, false, N_CT, R0 * R1, true>(a, ra, rb, has_b, bufB, nullptr, tw, R0 * R1, pacc);
+            } else {
+                stockham_pass<R1, false, N_CT, R0, true>(a, ra, rb, has_b, bufA, nullptr, tw, R0, pacc);
             }
-            if constexpr (R2 > 0) {
-                stockham_pass<R2, false, N_CT, R0 * R1>(a, ra, rb, has_b, bufB, bufA, tw, R0 * R1);
-                __syncthreads();
-                src = bufA;
-            }
+            continue;
         } else {
             int ns = 1;
 #pragma unroll 1
@@ -217,6 +234,12 @@ __global__ void __launch_bounds__(256) flux_power_kernel(const PowArgs a)
             pw[m] += (double)(ar * ar + ai * ai) + (double)(br * br + bi * bi);
         }
     }
+    if constexpr (N_CT > 0) {                              // output k = j + t ns of the last pass, j = tid < N / RL
+        if (tid < N_CT / RL)
+#pragma unroll
+            for (int t = 0; t < RL; ++t) atomicAdd(a.acc + tid + t * (N_CT / RL), pacc[t]);
+        return;
+    }
     __syncthreads();
     for (int m = tid; m <= nh; m += T)
         if (pw[m] != 0.0) atomicAdd(a.acc + m, pw[m]);
@@ -238,7 +261,9 @@ extern "C" lya_status lya_flux_power_rows(lya_ctx *ctx, size_t n_rows, int32_t n
         return lya_fail(ctx, LYA_EINVAL, "lya_flux_power_rows: n_pix must be a power of two in [8, 8192]");
     LYA_CUDA(ctx, cudaSetDevice(ctx->device));
     const int nk = n_pix / 2 + 1;
-    LYA_CUDA(ctx, cudaMemsetAsync(ctx->d_stats, 0, (size_t)nk * sizeof(double), ctx->stream));
+    const bool folded = n_pix >= 256 && n_pix <= 4096;     // compile-time plans leave sum |Z(k)|^2, k < n_pix, to fold here
+    const int n_acc = folded ? n_pix : nk;
+    LYA_CUDA(ctx, cudaMemsetAsync(ctx->d_stats, 0, (size_t)n_acc * sizeof(double), ctx->stream));
     PowArgs a;
     memset(&a, 0, sizeof(a));
     a.flux = flux; a.n_rows = n_rows; a.n = n_pix; a.log2n = log2n;
@@ -263,9 +288,10 @@ extern "C" lya_status lya_flux_power_rows(lya_ctx *ctx, size_t n_rows, int32_t n
     ctx->launches++;
     LYA_CUDA(ctx, cudaGetLastError());
     double *host = ctx->h_pinned + LYA_PINNED_STATS;                       // pinned: a true asynchronous DMA
-    LYA_CUDA(ctx, cudaMemcpyAsync(host, ctx->d_stats, (size_t)nk * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
+    LYA_CUDA(ctx, cudaMemcpyAsync(host, ctx->d_stats, (size_t)n_acc * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
     LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     const double scale = dv_kms / ((double)n_pix * (double)n_rows);        // V / N^2 / n_rows
-    for (int m = 0; m < nk; ++m) power[m] = host[m] * scale;
+    for (int m = 0; m < nk; ++m)                                           // |X_A|^2 + |X_B|^2 = (|Z(m)|^2 + |Z(N-m)|^2) / 2
+        power[m] = (folded ? 0.5 * (host[m] + host[(n_pix - m) & (n_pix - 1)]) : host[m]) * scale;
     return LYA_OK;
 }
