@@ -355,15 +355,15 @@ def bench_ours(args) -> dict:
         del noise, obs_out
         if w.cfg == 5:
             del flux_nr, Frows, tau_nr
-        # delta_b and v_x from a DM field (here: the workload's delta) -- one R2C, two k-space
-        # kernels, two C2R; the FFTs are cuFFT's
+        # delta_b and v_x from a DM field (here: the workload's delta) -- one R2C, one k-space
+        # kernel for both outputs, two C2R; the FFTs are cuFFT's
         if w.cfg <= 3 or args.fields:
             try:
                 t_fld = timed_ms(lambda: ctx.fields_from_dm(delta, w.box_mpch, w.h, w.z, w.omega_m, 6.5,
                                                             want=("delta_b", "v_x")), reps=3)
                 next_rows["fields_from_dm"] = {"outputs": "delta_b, v_x", "ms": t_fld,
-                                               "kspace_kernel_bytes": int(2 * 16 * (n // 2 + 1) * n * n),
-                                               "note": "3 cuFFT transforms + 2 k-space kernels (8 B in + 8 B out per mode)"}
+                                               "kspace_kernel_bytes": int(3 * 8 * (n // 2 + 1) * n * n),
+                                               "note": "3 cuFFT transforms + 1 k-space kernel (8 B in + 2 x 8 B out per mode)"}
             except lya.LyaError as exc:                   # cuFFT not installed on this box: the row is optional
                 next_rows["fields_from_dm"] = {"unavailable": str(exc)}
 

@@ -298,8 +298,9 @@ lya_status lya_growth_rate(double z, double omega_m, double *f_out);
 
 /* delta_dm: DEVICE [nz][ny][nx] fp32.  delta_b, v_x, v_y, v_z: DEVICE outputs of the same shape, any may be NULL
  * (v in km/s, proper, along +axis: what lya_tau_sightlines takes); no output may alias delta_dm or another output.  Asynchronous on ctx's stream apart from the first call's
- * plan creation.  Workspace (two complex half-spectra, 8 (nx/2+1) ny nz bytes each, plus cuFFT's) is cached in
- * ctx. */
+ * plan creation.  Workspace (one complex half-spectrum, 8 (nx/2+1) ny nz bytes, for delta(k) and one per requested
+ * output -- a single k-space kernel then serves all outputs from one read of delta(k); two in all if the device cannot
+ * hold that -- plus cuFFT's) is cached in ctx. */
 lya_status lya_fields_from_dm(lya_ctx *ctx, const lya_field_params *p, const float *delta_dm,
                               float *delta_b, float *v_x, float *v_y, float *v_z);
 

@@ -2,9 +2,9 @@
 // dark-matter density field.
 //   Eq.1  delta_b(k) = delta_DM(k) / (1 + k^2 / k_F^2)
 //   Eq.3  v_a(k)     = E_+ i k_a / k^2 delta_DM(k),  E_+ = H(z) f(z) / (1+z)   [km/s per comoving Mpc]
-// One real-to-complex 3D FFT of delta_DM, then per requested output one k-space kernel (8 B read + 8 B written
-// per half-spectrum mode, HBM-bound; the 1/N^3 of the unnormalised transforms is folded in) and one
-// complex-to-real FFT.  The FFTs are cuFFT's (library primitive), resolved with dlopen at first use so that
+// One real-to-complex 3D FFT of delta_DM, then ONE k-space kernel for all requested outputs (8 B read once + 8 B
+// written per output and half-spectrum mode, HBM-bound; the 1/N^3 of the unnormalised transforms is folded in) and
+// one complex-to-real FFT per output.  The FFTs are cuFFT's (library primitive), resolved with dlopen at first use so that
 // liblya.so itself does not depend on libcufft; everything else is this file.  Readings U1-U5: DESIGN.md 12.
 #include <cufft.h>
 #include <dlfcn.h>
@@ -49,39 +49,60 @@ CufftApi *cufft_api()
 
 struct KArgs {
     const float2 *in;
-    float2       *out;
+    float2       *out[4];             // per output (0: Eq.1 filter; 1, 2, 3: Eq.3 velocity along x, y, z), NULL: not wanted
     int           nxh, nx, ny, nz;
+    unsigned      rows_per_block;
+    size_t        n_rows;             // ny * nz
     float         dkx, dky, dkz;       // 2 pi h / L_i [Mpc^-1]
     float         inv_kf2;             // 1 / k_F^2 (0: no filtering)
-    float         scale;               // mode 0: 1/N^3; mode a: E_+ / N^3
-    int           mode;                // 0: Eq.1 filter; 1, 2, 3: Eq.3 velocity along x, y, z
+    float         scale0, scale_v;     // 1/N^3; E_+ / N^3
 };
 
-// grid (ny, nz), one block per (iz, iy) row of nx/2 + 1 modes
-__global__ void __launch_bounds__(128) kspace_kernel(const KArgs a)
+// One read of delta(k) (8 B per half-spectrum mode) serves EVERY requested output (8 B written each).  A block owns
+// KS_ROWS consecutive (iz, iy) rows of nx/2 + 1 modes as one flat range, so that the odd row length does not leave
+// most of a last trip idle (a block per row with 128 threads kept 257 modes busy 67 % of the time); a thread steps
+// through the range by the block size and carries (ix, iy, iz) along, so there is no division in the loop.
+constexpr int KS_THREADS = 256, KS_ROWS = 16;
+
+__global__ void __launch_bounds__(KS_THREADS) kspace_kernel(const KArgs a)
 {
-    const int iy = blockIdx.x, iz = blockIdx.y;
-    const int my = iy < (a.ny + 1) / 2 ? iy : iy - a.ny;           // signed frequency, -n/2 at the Nyquist slot
-    const int mz = iz < (a.nz + 1) / 2 ? iz : iz - a.nz;
-    const float ky = a.dky * (float)my, kz = a.dkz * (float)mz;
-    const float kyz2 = ky * ky + kz * kz;
-    const bool nyq_y = (a.ny % 2 == 0) && iy == a.ny / 2, nyq_z = (a.nz % 2 == 0) && iz == a.nz / 2;
-    const size_t row = ((size_t)iz * a.ny + iy) * a.nxh;
-    for (int ix = threadIdx.x; ix < a.nxh; ix += blockDim.x) {
-        const float kx = a.dkx * (float)ix;
-        const float k2 = fmaf(kx, kx, kyz2);
-        const float2 d = __ldcs(a.in + row + ix);
-        float2 o;
-        if (a.mode == 0) {
-            const float f = a.scale / fmaf(k2, a.inv_kf2, 1.0f);
-            o = make_float2(d.x * f, d.y * f);
-        } else {
-            const float ka = a.mode == 1 ? kx : (a.mode == 2 ? ky : kz);
-            const bool nyq = a.mode == 1 ? ((a.nx % 2 == 0) && ix == a.nx / 2) : (a.mode == 2 ? nyq_y : nyq_z);
-            const float c = (k2 > 0.0f && !nyq) ? a.scale * ka / k2 : 0.0f;      // U4
-            o = make_float2(-d.y * c, d.x * c);                                  // times i c
+    const size_t row0 = (size_t)blockIdx.x * a.rows_per_block;
+    const size_t rows = a.n_rows - row0 < a.rows_per_block ? a.n_rows - row0 : a.rows_per_block;
+    const unsigned count = (unsigned)rows * (unsigned)a.nxh;
+    unsigned l = threadIdx.x;
+    unsigned lr = l / (unsigned)a.nxh;
+    int ix = (int)(l - lr * (unsigned)a.nxh);
+    int iy = (int)((row0 + lr) % (size_t)a.ny), iz = (int)((row0 + lr) / (size_t)a.ny);
+    const int step_r = KS_THREADS / a.nxh, step_x = KS_THREADS - step_r * a.nxh;   // one step = step_r rows + step_x modes
+    const bool even_x = (a.nx & 1) == 0, even_y = (a.ny & 1) == 0, even_z = (a.nz & 1) == 0;
+    const float2 *in = a.in + row0 * a.nxh;
+    for (; l < count; l += KS_THREADS) {
+        const int my = iy < (a.ny + 1) / 2 ? iy : iy - a.ny;       // signed frequency, -n/2 at the Nyquist slot
+        const int mz = iz < (a.nz + 1) / 2 ? iz : iz - a.nz;
+        const float kx = a.dkx * (float)ix, ky = a.dky * (float)my, kz = a.dkz * (float)mz;
+        const float k2 = fmaf(kx, kx, fmaf(ky, ky, kz * kz));
+        const float2 d = __ldcs(in + l);
+        const size_t e = row0 * a.nxh + l;
+        if (a.out[0]) {
+            const float f = a.scale0 / fmaf(k2, a.inv_kf2, 1.0f);
+            __stcs(a.out[0] + e, make_float2(d.x * f, d.y * f));
         }
-        __stcs(a.out + row + ix, o);
+        const float g = k2 > 0.0f ? a.scale_v / k2 : 0.0f;                         // U4: no k = 0 mode
+        if (a.out[1]) {
+            const float c = (even_x && ix == a.nx / 2) ? 0.0f : g * kx;            // U4: no Nyquist plane of the axis
+            __stcs(a.out[1] + e, make_float2(-d.y * c, d.x * c));                  // times i c
+        }
+        if (a.out[2]) {
+            const float c = (even_y && iy == a.ny / 2) ? 0.0f : g * ky;
+            __stcs(a.out[2] + e, make_float2(-d.y * c, d.x * c));
+        }
+        if (a.out[3]) {
+            const float c = (even_z && iz == a.nz / 2) ? 0.0f : g * kz;
+            __stcs(a.out[3] + e, make_float2(-d.y * c, d.x * c));
+        }
+        ix += step_x; iy += step_r;
+        if (ix >= a.nxh) { ix -= a.nxh; ++iy; }
+        while (iy >= a.ny) { iy -= a.ny; ++iz; }
     }
 }
 
@@ -136,7 +157,20 @@ extern "C" lya_status lya_fields_from_dm(lya_ctx *ctx, const lya_field_params *p
     const int nxh = p->nx / 2 + 1;
     const size_t half = (size_t)p->nz * p->ny * nxh;
     ctx->forest_total = 0;                               // the shared workspace no longer holds lya_forest_host_begin's tau
-    lya_status st = ensure_ws(ctx, 2 * half * sizeof(float2) + 256);
+    int n_out = 0;
+    for (int i = 0; i < 4; ++i) n_out += outs[i] != nullptr;
+    if (n_out == 0) return LYA_OK;
+    // one spectrum buffer per output lets ONE k-space kernel serve them all from a single read of delta(k); if the
+    // device cannot hold that many, two buffers and one kernel per output do
+    int n_buf = n_out;
+    lya_status st = LYA_OK;
+    if (ctx->ws_bytes < (1 + (size_t)n_buf) * half * sizeof(float2) + 256) {
+        size_t free_b = 0, total_b = 0;
+        cudaMemGetInfo(&free_b, &total_b);
+        if (free_b + ctx->ws_bytes < (1 + (size_t)n_buf) * half * sizeof(float2) + ((size_t)1 << 30)) n_buf = 1;
+    }
+    st = ensure_ws(ctx, (1 + (size_t)n_buf) * half * sizeof(float2) + 256);
+    if (st != LYA_OK && n_buf > 1) { n_buf = 1; ctx->err[0] = 0; st = ensure_ws(ctx, 2 * half * sizeof(float2) + 256); }
     if (st != LYA_OK) return st;
     float2 *A = (float2 *)ctx->ws, *B = A + half;
 
@@ -164,16 +198,31 @@ extern "C" lya_status lya_fields_from_dm(lya_ctx *ctx, const lya_field_params *p
     const double dk = 2.0 * M_PI * p->h / p->box_mpch * (double)p->nx;        // 2 pi h / (cell size x n_i), per axis below
     KArgs a;
     memset(&a, 0, sizeof(a));
-    a.in = A; a.out = B; a.nxh = nxh; a.nx = p->nx; a.ny = p->ny; a.nz = p->nz;
+    a.in = A; a.nxh = nxh; a.nx = p->nx; a.ny = p->ny; a.nz = p->nz;
+    a.n_rows = (size_t)p->ny * p->nz;
+    a.rows_per_block = KS_ROWS;
     a.dkx = (float)(dk / p->nx); a.dky = (float)(dk / p->ny); a.dkz = (float)(dk / p->nz);
     a.inv_kf2 = p->k_filter_mpc > 0.0 ? (float)(1.0 / (p->k_filter_mpc * p->k_filter_mpc)) : 0.0f;
-    const dim3 grid(p->ny, p->nz);
-    if (p->ny > 65535 * 32767 || p->nz > 65535) return lya_fail(ctx, LYA_EINVAL, "lya_fields_from_dm: grid too large");
+    a.scale0 = (float)(1.0 / n3);
+    a.scale_v = (float)(eplus / n3);
+    const size_t n_blocks = (a.n_rows + KS_ROWS - 1) / KS_ROWS;
+    if (n_blocks > 0x7fffffffull || (size_t)KS_ROWS * nxh > 0x7fffffffull)
+        return lya_fail(ctx, LYA_EINVAL, "lya_fields_from_dm: grid too large");
+    if (n_buf == n_out) {                                  // one kernel, then the inverse transforms
+        int slot = 0;
+        for (int mode = 0; mode < 4; ++mode) a.out[mode] = outs[mode] ? B + (size_t)(slot++) * half : nullptr;
+        kspace_kernel<<<(unsigned)n_blocks, KS_THREADS, 0, ctx->stream>>>(a);
+        ctx->launches++;
+        LYA_CUDA(ctx, cudaGetLastError());
+        for (int mode = 0; mode < 4; ++mode)
+            if (outs[mode] && fft->ExecC2R(ctx->fft_c2r, a.out[mode], outs[mode]) != CUFFT_SUCCESS)
+                return lya_fail(ctx, LYA_ECUDA, "lya_fields_from_dm: cufftExecC2R failed");
+        return LYA_OK;
+    }
     for (int mode = 0; mode < 4; ++mode) {
         if (!outs[mode]) continue;
-        a.mode = mode;
-        a.scale = (float)((mode == 0 ? 1.0 : eplus) / n3);
-        kspace_kernel<<<grid, 128, 0, ctx->stream>>>(a);
+        for (int k = 0; k < 4; ++k) a.out[k] = k == mode ? B : nullptr;
+        kspace_kernel<<<(unsigned)n_blocks, KS_THREADS, 0, ctx->stream>>>(a);
         ctx->launches++;
         LYA_CUDA(ctx, cudaGetLastError());
         if (fft->ExecC2R(ctx->fft_c2r, B, outs[mode]) != CUFFT_SUCCESS)
