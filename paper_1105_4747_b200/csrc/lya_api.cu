@@ -1,6 +1,7 @@
 // lya_api.cu -- host side of the C ABI declared in include/lya.h: context, argument validation, the
 // double-precision scalars of DESIGN.md "Notation", and the kernel launch wrappers.  No CPU fallback.
 #include <math.h>
+#include <mutex>
 #include <new>
 
 #include "lya_internal.h"
@@ -18,6 +19,52 @@ bool params_ok(const lya_params *p)
 }
 
 }  // namespace
+
+// Dynamic shared-memory opt-in and occupancy of a kernel, asked from the driver once per (device, kernel, block,
+// bytes) and remembered process-wide: the two runtime calls cost several microseconds each, which is most of a
+// launch on the small grids.  The opt-in is only ever RAISED, so launches whose answer is cached stay valid whatever
+// another context on the same device asked for in between.
+lya_status lya_kernel_occupancy(lya_ctx *ctx, const void *fn, int threads, size_t smem, int *per_sm)
+{
+    struct Entry { int dev; const void *fn; int threads; size_t smem; int per_sm; };
+    static Entry table[256];
+    static int n_entries = 0;
+    static std::mutex mu;
+    std::lock_guard<std::mutex> lock(mu);
+    size_t raised = 0;
+    for (int i = 0; i < n_entries; ++i) {
+        const Entry &e = table[i];
+        if (e.dev != ctx->device || e.fn != fn) continue;
+        if (e.threads == threads && e.smem == smem) { *per_sm = e.per_sm; return LYA_OK; }
+        if (e.smem > raised) raised = e.smem;
+    }
+    if (smem > raised && smem > 48 * 1024)
+        LYA_CUDA(ctx, cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int n = 0;
+    LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, fn, threads, smem));
+    if (n_entries < 256) table[n_entries++] = Entry{ctx->device, fn, threads, smem, n};
+    *per_sm = n;
+    return LYA_OK;
+}
+
+lya_status lya_stats_begin(lya_ctx *ctx, size_t n_doubles)
+{
+    if (ctx->stats_dirty) {                                // an earlier statistics call failed midway: start clean
+        LYA_CUDA(ctx, cudaMemsetAsync(ctx->d_stats, 0, LYA_STATS_DOUBLES * sizeof(double), ctx->stream));
+        LYA_CUDA(ctx, cudaMemsetAsync(ctx->d_sched + 4, 0, sizeof(unsigned int), ctx->stream));
+    }
+    (void)n_doubles;
+    ctx->stats_dirty = 1;
+    return LYA_OK;
+}
+
+lya_status lya_stats_end(lya_ctx *ctx)
+{
+    LYA_CUDA(ctx, cudaGetLastError());
+    LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    ctx->stats_dirty = 0;
+    return LYA_OK;
+}
 
 extern "C" {
 
@@ -84,8 +131,9 @@ lya_status lya_create(lya_ctx **out, int device, void *cuda_stream)
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->d_partials, part_bytes);
     if (e == cudaSuccess) e = cudaMallocHost((void **)&ctx->h_pinned, (LYA_PINNED_STATS + LYA_STATS_DOUBLES) * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->d_stats, LYA_STATS_DOUBLES * sizeof(double));
-    if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->d_sched, 4 * sizeof(unsigned int));
-    if (e == cudaSuccess) e = cudaMemset(ctx->d_sched, 0, 4 * sizeof(unsigned int));
+    if (e == cudaSuccess) e = cudaMemset(ctx->d_stats, 0, LYA_STATS_DOUBLES * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->d_sched, 8 * sizeof(unsigned int));
+    if (e == cudaSuccess) e = cudaMemset(ctx->d_sched, 0, 8 * sizeof(unsigned int));
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking);
     for (int i = 0; i < 2 && e == cudaSuccess; ++i) {
         e = cudaEventCreateWithFlags(&ctx->ev_copy[i], cudaEventDisableTiming);

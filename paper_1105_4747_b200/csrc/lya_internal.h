@@ -21,7 +21,9 @@ struct lya_ctx {
     double       *d_partials;     // [2 parities][LYA_MAX_RED_BLOCKS][2*LYA_MAX_TRIALS]
     double       *h_pinned;       // pinned host memory: [0, 64) written by the kernels directly (UVA: S4 results,
                                   // partial sums), [LYA_PINNED_STATS, +LYA_STATS_DOUBLES) DMA target of the statistics
-    unsigned int *d_sched;        // tau kernels' work counter [0..1] (zeroed on the stream before every launch) and pair counter [2..3]
+    unsigned int *d_sched;        // tau kernels' work counter [0..1] (zeroed on the stream before every launch), pair counter [2..3],
+                                  // [4] ticket of the statistics kernels (the last CTA to finish writes the result to h_pinned)
+    int           stats_dirty;    // a statistics call did not complete: d_stats / the ticket are re-zeroed before the next one
     double       *d_stats;        // 8192 doubles: flux-PDF counts (as uint64) / power-spectrum accumulators
     float        *d_taps, *h_taps; // lya_observe_rows: Gaussian taps (device / host staging), grown on demand
     size_t        taps_cap;
@@ -47,6 +49,12 @@ struct lya_ctx {
 #define LYA_MAX_TRIALS     8
 #define LYA_STATS_DOUBLES   8192
 #define LYA_PINNED_STATS    64
+
+// Statistics kernels (flux PDF, S5 + PDF, flux power) accumulate into ctx->d_stats with atomics; the LAST CTA to finish
+// (ticket d_sched[4]) copies the totals to the mapped pinned mirror and leaves d_stats and the ticket zeroed for the next
+// call, so a call is one launch and one synchronisation: no memset, no copy to enqueue.
+lya_status lya_stats_begin(lya_ctx *ctx, size_t n_doubles);
+lya_status lya_stats_end(lya_ctx *ctx);                  // synchronises; the results are in h_pinned + LYA_PINNED_STATS
 
 static inline lya_status lya_fail(lya_ctx *ctx, lya_status s, const char *msg)
 {
@@ -81,6 +89,10 @@ static inline lya_status lya_cuda_fail(lya_ctx *ctx, cudaError_t e, const char *
 #define LYA_ALPHA_T    (-0.7)                 // recombination-rate temperature slope
 
 void lya_fields_release(lya_ctx *ctx);   // fields.cu: destroys the cached cuFFT plans
+
+// lya_api.cu: raises the kernel's dynamic shared-memory limit to `smem` if needed and returns the resident CTAs per SM
+// (both remembered process-wide per device, kernel, block size and byte count)
+lya_status lya_kernel_occupancy(lya_ctx *ctx, const void *fn, int threads, size_t smem, int *per_sm);
 
 // kernels' host launchers (each enqueues on ctx->stream and bumps ctx->launches)
 lya_status lya_launch_gas(lya_ctx *ctx, const float *delta, size_t n, float *n_hi, float *b,

@@ -384,7 +384,8 @@ constexpr int FPDF_THREADS = 128;
 
 __global__ void __launch_bounds__(FPDF_THREADS) flux_pdf_fused_kernel(const float *tau, size_t n, Trial tr, float *flux,
                                                                       const __grid_constant__ PdfEdges edges,
-                                                                      unsigned long long *__restrict__ counts)
+                                                                      unsigned long long *counts, unsigned long long *host,
+                                                                      unsigned int *ticket)
 {
     extern __shared__ unsigned int hist[];               // [n_bins][FPDF_THREADS], then n_bins + 1 thresholds
     const int n_bins = edges.n_bins;
@@ -428,6 +429,7 @@ __global__ void __launch_bounds__(FPDF_THREADS) flux_pdf_fused_kernel(const floa
         for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
         if (lane == 0 && sum) atomicAdd(counts + b, (unsigned long long)sum);
     }
+    lya_publish_last_cta(counts, n_bins, host, ticket);
 }
 
 // float4 in the subsample "every `every`-th chunk of 256 float4 of the aligned body of tau" (0: no subsample)
@@ -568,27 +570,29 @@ lya_status lya_run_flux_with_pdf(lya_ctx *ctx, const float *tau, size_t n, doubl
                                  double f_lo, double width, uint64_t *counts, double *pdf)
 {
     unsigned long long *d_counts = reinterpret_cast<unsigned long long *>(ctx->d_stats);
-    LYA_CUDA(ctx, cudaMemsetAsync(d_counts, 0, (size_t)n_bins * sizeof(unsigned long long), ctx->stream));
+    unsigned long long *host = reinterpret_cast<unsigned long long *>(ctx->h_pinned + LYA_PINNED_STATS);
     if (n > 0) {
         PdfEdges edges;
         lya_pdf_edges(n_bins, f_lo, width, &edges);
         const size_t smem = (size_t)n_bins * FPDF_THREADS * sizeof(unsigned int) + (size_t)(n_bins + 1) * sizeof(float);
-        LYA_CUDA(ctx, cudaFuncSetAttribute(flux_pdf_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         int per_sm = 0;
-        LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, flux_pdf_fused_kernel, FPDF_THREADS, smem));
+        lya_status st = lya_kernel_occupancy(ctx, (const void *)flux_pdf_fused_kernel, FPDF_THREADS, smem, &per_sm);
+        if (st != LYA_OK) return st;
         if (per_sm < 1) return lya_fail(ctx, LYA_EINVAL, "lya_flux_with_pdf: too many bins for shared memory");
         size_t want = (n / 4 + FPDF_THREADS - 1) / FPDF_THREADS;
         if (want < 1) want = 1;
         const size_t cap = (size_t)ctx->sm_count * per_sm;
+        st = lya_stats_begin(ctx, n_bins);
+        if (st != LYA_OK) return st;
+        // the last CTA to finish writes the totals straight to the pinned mirror and re-zeroes the device counters
         flux_pdf_fused_kernel<<<(int)(want < cap ? want : cap), FPDF_THREADS, smem, ctx->stream>>>(
-            tau, n, make_trial(a), flux, edges, d_counts);
+            tau, n, make_trial(a), flux, edges, d_counts, host, ctx->d_sched + 4);
         ctx->launches++;
-        LYA_CUDA(ctx, cudaGetLastError());
+        st = lya_stats_end(ctx);
+        if (st != LYA_OK) return st;
+    } else {
+        for (int b = 0; b < n_bins; ++b) host[b] = 0;
     }
-    // counts come back through the ctx's pinned mirror: a true asynchronous DMA, no pageable staging
-    uint64_t *host = reinterpret_cast<uint64_t *>(ctx->h_pinned + LYA_PINNED_STATS);
-    LYA_CUDA(ctx, cudaMemcpyAsync(host, d_counts, (size_t)n_bins * sizeof(uint64_t), cudaMemcpyDeviceToHost, ctx->stream));
-    LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     for (int b = 0; b < n_bins; ++b) {
         if (counts) counts[b] = host[b];
         if (pdf) pdf[b] = n ? (double)host[b] / ((double)n * width) : 0.0;

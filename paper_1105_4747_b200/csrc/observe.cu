@@ -383,7 +383,8 @@ constexpr int PDF_THREADS = 128;
 
 __global__ void __launch_bounds__(PDF_THREADS) flux_pdf_kernel(const float *__restrict__ flux, size_t n,
                                                                const __grid_constant__ PdfEdges edges,
-                                                               unsigned long long *__restrict__ counts)
+                                                               unsigned long long *counts, unsigned long long *host,
+                                                               unsigned int *ticket)
 {
     extern __shared__ unsigned int hist[];               // [n_bins][PDF_THREADS], then n_bins + 1 thresholds
     const int n_bins = edges.n_bins;
@@ -416,6 +417,7 @@ __global__ void __launch_bounds__(PDF_THREADS) flux_pdf_kernel(const float *__re
         for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
         if (lane == 0 && s) atomicAdd(counts + b, (unsigned long long)s);
     }
+    lya_publish_last_cta(counts, n_bins, host, ticket);
 }
 
 }  // namespace
@@ -566,9 +568,9 @@ extern "C" lya_status lya_observe_rows(lya_ctx *ctx, size_t n_rows, int32_t n_pi
 #undef LYA_LEAN
         }
         const size_t smem_l = ((size_t)n_pix + LT + 8 + n_pix + 4) * sizeof(float) + (a.rebin ? (size_t)nb * sizeof(int4) : 0);
-        LYA_CUDA(ctx, cudaFuncSetAttribute(lean, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_l));
         int per_sm_l = 0;
-        LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_l, lean, threads, smem_l));
+        lya_status st_l = lya_kernel_occupancy(ctx, (const void *)lean, threads, smem_l, &per_sm_l);
+        if (st_l != LYA_OK) return st_l;
         if (per_sm_l >= 1) {
             const size_t cap_l = (size_t)ctx->sm_count * per_sm_l;
             lean<<<(int)(n_rows < cap_l ? n_rows : cap_l), threads, smem_l, ctx->stream>>>(a, tp);
@@ -589,9 +591,9 @@ extern "C" lya_status lya_observe_rows(lya_ctx *ctx, size_t n_rows, int32_t n_pi
     const int halo = a.L >= 0 ? a.L : 0;
     const size_t smem = ((size_t)D * (a.n4 + ((halo + 3) & ~3) + 8) + (size_t)D * a.n4 + (((halo + 11) + 3) & ~3)) * sizeof(float);
     if (smem > (size_t)ctx->max_smem_optin) return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: row too long for shared memory");
-    LYA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
-    LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
+    lya_status st_g = lya_kernel_occupancy(ctx, (const void *)kern, threads, smem, &per_sm);
+    if (st_g != LYA_OK) return st_g;
     if (per_sm < 1) return lya_fail(ctx, LYA_EINVAL, "lya_observe_rows: row too long for shared memory");
     const size_t cap = (size_t)ctx->sm_count * per_sm;
     const size_t n_batches = (n_rows + D - 1) / D;
@@ -611,26 +613,29 @@ extern "C" lya_status lya_flux_pdf(lya_ctx *ctx, const float *flux, size_t n, in
     if (n_bins < 1 || n_bins > 256 || !(width > 0.0)) return lya_fail(ctx, LYA_EINVAL, "lya_flux_pdf: 1 <= n_bins <= 256 and width > 0 required");
     LYA_CUDA(ctx, cudaSetDevice(ctx->device));
     unsigned long long *d_counts = reinterpret_cast<unsigned long long *>(ctx->d_stats);
-    LYA_CUDA(ctx, cudaMemsetAsync(d_counts, 0, (size_t)n_bins * sizeof(unsigned long long), ctx->stream));
+    unsigned long long *host = reinterpret_cast<unsigned long long *>(ctx->h_pinned + LYA_PINNED_STATS);
     if (n > 0) {
         PdfEdges edges;
         lya_pdf_edges(n_bins, f_lo, width, &edges);
         const size_t smem = (size_t)n_bins * PDF_THREADS * sizeof(unsigned int) + (size_t)(n_bins + 1) * sizeof(float);
-        LYA_CUDA(ctx, cudaFuncSetAttribute(flux_pdf_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
         int per_sm = 0;
-        LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, flux_pdf_kernel, PDF_THREADS, smem));
+        lya_status st = lya_kernel_occupancy(ctx, (const void *)flux_pdf_kernel, PDF_THREADS, smem, &per_sm);
+        if (st != LYA_OK) return st;
         if (per_sm < 1) return lya_fail(ctx, LYA_EINVAL, "lya_flux_pdf: too many bins for shared memory");
         size_t want = (n / 4 + PDF_THREADS - 1) / PDF_THREADS;
         if (want < 1) want = 1;
         const size_t cap = (size_t)ctx->sm_count * per_sm;
-        flux_pdf_kernel<<<(int)(want < cap ? want : cap), PDF_THREADS, smem, ctx->stream>>>(flux, n, edges, d_counts);
+        st = lya_stats_begin(ctx, n_bins);
+        if (st != LYA_OK) return st;
+        // the last CTA to finish writes the totals straight to the pinned mirror and re-zeroes the device counters
+        flux_pdf_kernel<<<(int)(want < cap ? want : cap), PDF_THREADS, smem, ctx->stream>>>(flux, n, edges, d_counts, host,
+                                                                                           ctx->d_sched + 4);
         ctx->launches++;
-        LYA_CUDA(ctx, cudaGetLastError());
+        st = lya_stats_end(ctx);
+        if (st != LYA_OK) return st;
+    } else {
+        for (int b = 0; b < n_bins; ++b) host[b] = 0;
     }
-    // counts come back through the ctx's pinned mirror: a true asynchronous DMA, no pageable staging
-    uint64_t *host = reinterpret_cast<uint64_t *>(ctx->h_pinned + LYA_PINNED_STATS);
-    LYA_CUDA(ctx, cudaMemcpyAsync(host, d_counts, (size_t)n_bins * sizeof(uint64_t), cudaMemcpyDeviceToHost, ctx->stream));
-    LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     for (int b = 0; b < n_bins; ++b) {
         if (counts) counts[b] = host[b];
         if (pdf) pdf[b] = n ? (double)host[b] / ((double)n * width) : 0.0;

@@ -57,4 +57,24 @@ __device__ __forceinline__ int lya_pdf_bin(float f, const float *s_thr, int n_bi
     }
     return b;
 }
+
+// Epilogue of the statistics kernels, called by every thread of every CTA after the CTA's own atomics into acc[0 .. n):
+// the last CTA to arrive (ticket) moves the totals to `host` (mapped pinned memory) and leaves acc and the ticket zeroed
+// for the next launch.  T is unsigned long long (counts) or double (power sums).
+template <typename T>
+__device__ __forceinline__ void lya_publish_last_cta(T *acc, int n, T *host, unsigned int *ticket)
+{
+    __shared__ int s_last;
+    __threadfence();                                     // this thread's atomics are visible device-wide
+    __syncthreads();
+    if (threadIdx.x == 0) s_last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+    for (int i = threadIdx.x; i < n; i += blockDim.x) {
+        host[i] = __ldcg(acc + i);
+        acc[i] = (T)0;
+    }
+    if (threadIdx.x == 0) *ticket = 0u;
+}
 #endif

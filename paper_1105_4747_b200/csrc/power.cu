@@ -16,6 +16,7 @@
 // instead of four -- and the host folds k and N - k once at the end.  Other sizes write the last pass to shared
 // memory and read the pairs (m, N - m) out (accumulated in double per CTA).
 #include "lya_internal.h"
+#include "pdf_bin.h"
 
 namespace {
 
@@ -25,7 +26,10 @@ struct PowArgs {
     int          n, log2n;
     int          n_pass, radix[4];
     float        inv_mean;
-    double      *acc;          // device, n/2 + 1 doubles, zeroed by the host
+    double      *acc;          // device accumulators (n or n/2 + 1 doubles), zero on entry and left zero
+    double      *host;         // mapped pinned mirror: the last CTA to finish writes the totals there
+    unsigned int *ticket;
+    int          n_acc;
 };
 
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
@@ -238,11 +242,13 @@ __global__ void __launch_bounds__(256) flux_power_kernel(const PowArgs a)
         if (tid < N_CT / RL)
 #pragma unroll
             for (int t = 0; t < RL; ++t) atomicAdd(a.acc + tid + t * (N_CT / RL), pacc[t]);
+        lya_publish_last_cta(a.acc, a.n_acc, a.host, a.ticket);
         return;
     }
     __syncthreads();
     for (int m = tid; m <= nh; m += T)
         if (pw[m] != 0.0) atomicAdd(a.acc + m, pw[m]);
+    lya_publish_last_cta(a.acc, a.n_acc, a.host, a.ticket);
 }
 
 }  // namespace
@@ -263,11 +269,11 @@ extern "C" lya_status lya_flux_power_rows(lya_ctx *ctx, size_t n_rows, int32_t n
     const int nk = n_pix / 2 + 1;
     const bool folded = n_pix >= 256 && n_pix <= 4096;     // compile-time plans leave sum |Z(k)|^2, k < n_pix, to fold here
     const int n_acc = folded ? n_pix : nk;
-    LYA_CUDA(ctx, cudaMemsetAsync(ctx->d_stats, 0, (size_t)n_acc * sizeof(double), ctx->stream));
     PowArgs a;
     memset(&a, 0, sizeof(a));
     a.flux = flux; a.n_rows = n_rows; a.n = n_pix; a.log2n = log2n;
     a.inv_mean = (float)(1.0 / mean_flux); a.acc = ctx->d_stats;
+    a.host = ctx->h_pinned + LYA_PINNED_STATS; a.ticket = ctx->d_sched + 4; a.n_acc = n_acc;
     // radices of the passes (log2: 4, 3, 2), largest first
     static const int plan[14][4] = {{0}, {0}, {0}, {3}, {4}, {3, 2}, {3, 3}, {4, 3}, {4, 4}, {3, 3, 3}, {4, 3, 3},
                                     {4, 4, 3}, {4, 4, 4}, {4, 4, 3, 2}};
@@ -279,17 +285,18 @@ extern "C" lya_status lya_flux_power_rows(lya_ctx *ctx, size_t n_rows, int32_t n
     void (*kern)(const PowArgs) = n_pix == 256 ? flux_power_kernel<256> : n_pix == 512 ? flux_power_kernel<512>
                                 : n_pix == 1024 ? flux_power_kernel<1024> : n_pix == 2048 ? flux_power_kernel<2048>
                                 : n_pix == 4096 ? flux_power_kernel<4096> : flux_power_kernel<0>;
-    LYA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int per_sm = 0;
-    LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, threads, smem));
+    lya_status st = lya_kernel_occupancy(ctx, (const void *)kern, threads, smem, &per_sm);
+    if (st != LYA_OK) return st;
     if (per_sm < 1) return lya_fail(ctx, LYA_ECUDA, "flux_power_kernel: zero occupancy");
     const size_t n_pairs = (n_rows + 1) / 2, cap = (size_t)ctx->sm_count * per_sm;
-    kern<<<(int)(n_pairs < cap ? n_pairs : cap), threads, smem, ctx->stream>>>(a);
+    st = lya_stats_begin(ctx, n_acc);
+    if (st != LYA_OK) return st;
+    kern<<<(int)(n_pairs < cap ? n_pairs : cap), threads, smem, ctx->stream>>>(a);   // the last CTA writes the totals to a.host
     ctx->launches++;
-    LYA_CUDA(ctx, cudaGetLastError());
-    double *host = ctx->h_pinned + LYA_PINNED_STATS;                       // pinned: a true asynchronous DMA
-    LYA_CUDA(ctx, cudaMemcpyAsync(host, ctx->d_stats, (size_t)n_acc * sizeof(double), cudaMemcpyDeviceToHost, ctx->stream));
-    LYA_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    st = lya_stats_end(ctx);
+    if (st != LYA_OK) return st;
+    const double *host = a.host;
     const double scale = dv_kms / ((double)n_pix * (double)n_rows);        // V / N^2 / n_rows
     for (int m = 0; m < nk; ++m)                                           // |X_A|^2 + |X_B|^2 = (|Z(m)|^2 + |Z(N-m)|^2) / 2
         power[m] = (folded ? 0.5 * (host[m] + host[(n_pix - m) & (n_pix - 1)]) : host[m]) * scale;

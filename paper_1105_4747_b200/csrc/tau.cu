@@ -638,7 +638,10 @@ lya_status launch_x(lya_ctx *ctx, const TauArgs &a)
     long long want = (a.n_sl + ctx->sm_count - 1) / ctx->sm_count;
     if (groups > want) groups = (int)(want < 1 ? 1 : want);
     const size_t smem_bytes = (size_t)groups * per_group + mom_bytes;
-    LYA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
+    int resident = 0;
+    lya_status st = lya_kernel_occupancy(ctx, (const void *)kern, 32 * G * groups, smem_bytes, &resident);
+    if (st != LYA_OK) return st;
+    if (resident < 1) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: sightline too long for shared memory");
     long long ctas = (a.n_sl + groups - 1) / groups;
     const int grid = (int)(ctas < ctx->sm_count ? ctas : ctx->sm_count);
     kern<<<grid, 32 * G * groups, smem_bytes, ctx->stream>>>(a, G, groups);
@@ -651,9 +654,9 @@ template <int R, bool FUSED, bool WIN>
 lya_status launch_strided(lya_ctx *ctx, const TauArgs &a, size_t smem_bytes)
 {
     auto kern = tau_strided_kernel<R, FUSED, WIN>;
-    LYA_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes));
     int per_sm = 0;
-    LYA_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, TAU_THREADS, smem_bytes));
+    lya_status st = lya_kernel_occupancy(ctx, (const void *)kern, TAU_THREADS, smem_bytes, &per_sm);
+    if (st != LYA_OK) return st;
     if (per_sm < 1) return lya_fail(ctx, LYA_EINVAL, "lya_tau_sightlines: sightline too long for shared memory");
     long long cap = (long long)ctx->sm_count * per_sm;
     int grid = (int)(a.n_batches < cap ? a.n_batches : cap);
