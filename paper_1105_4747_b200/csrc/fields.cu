@@ -84,10 +84,10 @@ __global__ void __launch_bounds__(KS_THREADS) kspace_kernel(const KArgs a)
         const float2 d = __ldcs(in + l);
         const size_t e = row0 * a.nxh + l;
         if (a.out[0]) {
-            const float f = a.scale0 / fmaf(k2, a.inv_kf2, 1.0f);
+            const float f = __fdividef(a.scale0, fmaf(k2, a.inv_kf2, 1.0f));       // 2 ulp: far inside the FFT's own error
             __stcs(a.out[0] + e, make_float2(d.x * f, d.y * f));
         }
-        const float g = k2 > 0.0f ? a.scale_v / k2 : 0.0f;                         // U4: no k = 0 mode
+        const float g = k2 > 0.0f ? __fdividef(a.scale_v, k2) : 0.0f;              // U4: no k = 0 mode
         if (a.out[1]) {
             const float c = (even_x && ix == a.nx / 2) ? 0.0f : g * kx;            // U4: no Nyquist plane of the axis
             __stcs(a.out[1] + e, make_float2(-d.y * c, d.x * c));                  // times i c
