@@ -378,6 +378,132 @@ __global__ void __launch_bounds__(256) observe_rows_lean_kernel(const ObsArgs a,
     }
 }
 
+// ---- the lean kernel with EIGHT consecutive outputs per thread (packed path only: at most 41 tap slots; rows of
+// n % 8 == 0 pixels, n / 8 <= 256 threads).  The convolution then needs (LT + 8) / 4 LDS.128 per eight outputs instead
+// of (LT + 4) / 4 per four, fewer distinct weight pairs per pixel, and every per-thread cost (staging, row change,
+// barriers, address set-up) is spread over twice as many pixels: 66 -> ~45 instructions per pixel for the BOSS-like
+// instrument.  Lanes that own 8 pixels sit 32 bytes apart, which would make every LDS.128 of the staged row a 2-way
+// bank conflict; so the row is staged SPLIT by 16-byte chunk parity -- even chunks (4 pixels each) in one array, odd
+// chunks in another: a thread's window alternates between the two with immediate offsets, and within either array
+// neighbouring lanes read neighbouring chunks.
+struct __align__(16) ObsTaps8 {
+    float wp[64];                                        // wp[t + 7] = g(KO - t); zero outside the real taps
+    float wq[64];                                        // wq[k] = wp[k + 1]
+};
+#define OBS_WPAIR8(k) (((k) & 1) ? pack2(tp.wq[(k) - 1], tp.wq[(k)]) : pack2(tp.wp[(k)], tp.wp[(k) + 1]))
+
+template <int LT>                                        // LT >= L, multiple of 4, <= OBS_PACKED_LT
+__global__ void __launch_bounds__(256) observe_rows_lean8_kernel(const ObsArgs a, const __grid_constant__ ObsTaps8 tp)
+{
+    extern __shared__ __align__(16) float sm[];
+    const int n = a.n, T = blockDim.x, tid = threadIdx.x, nb = a.nb;
+    constexpr int NJ = (LT + 8) / 4;                     // chunks in a thread's window
+    const int nch = ((n + LT + 12) >> 3) + 1;            // chunks per half of the staged row (logical length n + LT + 12)
+    float4 *s_e = reinterpret_cast<float4 *>(sm);        // even chunks of s_in[h] = F[(h - KO) mod n], zero beyond n + L
+    float4 *s_o = s_e + nch;                             // odd chunks
+    float *s_c  = reinterpret_cast<float *>(s_o + nch);  // convolved row, n floats (+ 4 zeros for the 3-tap rebin)
+    int4  *s_b  = reinterpret_cast<int4 *>(s_c + n + 4); // bin table, nb entries (rebin only)
+    auto in_chunk = [&](int c) -> float4 * { return ((c & 1) ? s_o : s_e) + (c >> 1); };
+    for (int h = tid; h < 2 * nch; h += T) s_e[h] = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (tid < 4) s_c[n + tid] = 0.0f;
+    if (a.rebin)
+        for (int m = tid; m < nb; m += T) s_b[m] = a.bins[m];
+
+    const bool own = 8 * tid < n;                        // this thread owns pixels 8 tid .. 8 tid + 7
+    const bool has_halo = tid < a.L;
+    const int hsrc = tid < a.KO ? n - a.KO + tid : tid - a.KO;       // this thread's halo pixel and where it goes
+    const int hdst = tid < a.KO ? tid : n + tid;
+    float *hptr = reinterpret_cast<float *>(in_chunk(hdst >> 2)) + (hdst & 3);
+    float4 *own0 = in_chunk((a.KO >> 2) + 2 * tid), *own1 = in_chunk((a.KO >> 2) + 2 * tid + 1);
+    const float4 *we = s_e + tid, *wo = s_o + tid;       // window: chunk 2 tid + j is (j even) we[j / 2], (j odd) wo[j / 2]
+    const size_t row_step = gridDim.x;
+    const float *src = a.flux + (size_t)blockIdx.x * n;
+    const float *nz  = a.noise ? a.noise + (size_t)blockIdx.x * nb : nullptr;
+    float *dst = a.out + (size_t)blockIdx.x * nb;
+    const size_t src_step = row_step * n, out_step = row_step * nb;
+    float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = r0;
+    float hreg = 0.0f, nzr[OBS_NBR];
+    auto fetch = [&]() {
+        if (own) {
+            r0 = __ldcs(reinterpret_cast<const float4 *>(src + 8 * tid));
+            r1 = __ldcs(reinterpret_cast<const float4 *>(src + 8 * tid + 4));
+        }
+        if (has_halo) hreg = __ldg(src + hsrc);
+        src += src_step;
+    };
+    size_t row = blockIdx.x;
+    if (row < a.n_rows) fetch();
+    for (; row < a.n_rows; row += row_step) {
+        __syncthreads();                                 // previous row's staged row / s_c consumed
+        if (own) { *own0 = r0; *own1 = r1; }
+        if (has_halo) *hptr = hreg;
+        if (row + row_step < a.n_rows) fetch();
+        if (nz) {
+#pragma unroll
+            for (int k = 0; k < OBS_NBR; ++k) {
+                const int m = tid + k * T;
+                nzr[k] = m < nb ? __ldcs(nz + m) : 0.0f;
+            }
+        }
+        __syncthreads();
+        if (own) {
+            unsigned long long c[8];
+#pragma unroll
+            for (int r = 0; r < 8; ++r) c[r] = 0ull;
+#pragma unroll
+            for (int j = 0; j < NJ; ++j) {               // input u = 4 j + {0..3} and output r use wp[u - r + 7]
+                const float4 x = (j & 1) ? wo[j >> 1] : we[j >> 1];
+                const unsigned long long xy = pack2(x.x, x.y), zw = pack2(x.z, x.w);
+#pragma unroll
+                for (int r = 0; r < 8; ++r) {
+                    c[r] = ffma2(xy, OBS_WPAIR8(4 * j - r + 7), c[r]);
+                    c[r] = ffma2(zw, OBS_WPAIR8(4 * j - r + 9), c[r]);
+                }
+            }
+            float4 *d = reinterpret_cast<float4 *>(s_c + 8 * tid);
+            d[0] = make_float4(sum2(c[0]), sum2(c[1]), sum2(c[2]), sum2(c[3]));
+            d[1] = make_float4(sum2(c[4]), sum2(c[5]), sum2(c[6]), sum2(c[7]));
+        }
+        __syncthreads();
+
+        const float inv_snr = nz ? a.inv_snr : 0.0f;
+        auto put = [&](int k, int m, float v) {
+            if (nz) v = fmaf(k < OBS_NBR ? nzr[k < OBS_NBR ? k : 0] : __ldcs(nz + m), inv_snr, v);
+            __stcs(dst + m, v);
+        };
+        if (a.bins3) {                                   // bins <= 2 pixels wide: three pixels {i0, w0, w1, w2}
+#pragma unroll
+            for (int k = 0; k < OBS_NBR; ++k) {
+                const int m = tid + k * T;
+                if (m < nb) {
+                    const int4 e = s_b[m];
+                    const float *cc = s_c + e.x;
+                    put(k, m, fmaf(__int_as_float(e.w), cc[2], fmaf(__int_as_float(e.z), cc[1], __int_as_float(e.y) * cc[0])));
+                }
+            }
+            for (int m = tid + OBS_NBR * T; m < nb; m += T) {
+                const int4 e = s_b[m];
+                const float *cc = s_c + e.x;
+                put(OBS_NBR, m, fmaf(__int_as_float(e.w), cc[2], fmaf(__int_as_float(e.z), cc[1], __int_as_float(e.y) * cc[0])));
+            }
+        } else if (a.rebin) {                            // wide bins: first pixel, whole pixels, last pixel (weights carry 1/B)
+            auto wide = [&](int m) -> float {
+                const int4 e = s_b[m];
+                if (e.y <= e.x) return __int_as_float(e.z) * s_c[e.x];
+                float mid = 0.0f;
+#pragma unroll 1
+                for (int i = e.x + 1; i < e.y; ++i) mid += s_c[i];
+                return fmaf(__int_as_float(e.w), s_c[e.y], fmaf(mid, a.inv_bin_f, __int_as_float(e.z) * s_c[e.x]));
+            };
+            for (int m = tid, k = 0; m < nb; m += T, ++k) put(k < OBS_NBR ? k : OBS_NBR, m, wide(m));
+        } else {
+            for (int m = tid, k = 0; m < nb; m += T, ++k) put(k < OBS_NBR ? k : OBS_NBR, m, s_c[m]);
+        }
+        dst += out_step;
+        if (nz) nz += out_step;
+    }
+}
+
 // ---- flux PDF: private per-thread histograms in shared memory (hist[bin][thread]: conflict-free, no atomics)
 constexpr int PDF_THREADS = 128;
 
@@ -559,6 +685,33 @@ extern "C" lya_status lya_observe_rows(lya_ctx *ctx, size_t n_rows, int32_t n_pi
         }
         // LT: the smallest instantiated multiple of 4 that is >= L (every multiple of 4 up to 64, then 96, 124)
         const int LT = a.L <= 64 ? ((a.L + 3) & ~3) : (a.L <= 96 ? 96 : 124);
+        // eight outputs per thread where the packed convolution applies and the row gives every thread eight pixels
+        if (LT <= OBS_PACKED_LT && n_pix % 8 == 0 && n_pix >= 256 && n_pix <= 2048) {
+            ObsTaps8 t8;
+            memset(&t8, 0, sizeof(t8));
+            for (int t = 0; t <= a.L + 7 && t + 7 < 64; ++t) t8.wp[t + 4] = ctx->h_taps[t];      // h_taps[t + 3] = g(KO - t)
+            for (int t = 0; t < 63; ++t) t8.wq[t] = t8.wp[t + 1];
+            void (*lean8)(const ObsArgs, const ObsTaps8) = nullptr;
+            switch (LT) {
+#define LYA_LEAN8(N) case N: lean8 = observe_rows_lean8_kernel<N>; break;
+                LYA_LEAN8(0) LYA_LEAN8(4) LYA_LEAN8(8) LYA_LEAN8(12) LYA_LEAN8(16) LYA_LEAN8(20) LYA_LEAN8(24)
+                LYA_LEAN8(28) LYA_LEAN8(32) LYA_LEAN8(36) LYA_LEAN8(40)
+#undef LYA_LEAN8
+            }
+            const int threads8 = ((n_pix / 8 + 31) / 32) * 32;
+            const size_t nch = (((size_t)n_pix + LT + 12) >> 3) + 1;
+            const size_t smem8 = 2 * nch * sizeof(float4) + ((size_t)n_pix + 4) * sizeof(float) + (a.rebin ? (size_t)nb * sizeof(int4) : 0);
+            int per_sm8 = 0;
+            lya_status st8 = lya_kernel_occupancy(ctx, (const void *)lean8, threads8, smem8, &per_sm8);
+            if (st8 != LYA_OK) return st8;
+            if (lean8 && per_sm8 >= 1 && a.L <= threads8) {
+                const size_t cap8 = (size_t)ctx->sm_count * per_sm8;
+                lean8<<<(int)(n_rows < cap8 ? n_rows : cap8), threads8, smem8, ctx->stream>>>(a, t8);
+                ctx->launches++;
+                LYA_CUDA(ctx, cudaGetLastError());
+                return LYA_OK;
+            }
+        }
         void (*lean)(const ObsArgs, const ObsTaps) = nullptr;
         switch (LT) {
 #define LYA_LEAN(N) case N: lean = nv_lean == 1 ? observe_rows_lean_kernel<N, 1> : (nv_lean == 2 ? observe_rows_lean_kernel<N, 2> : observe_rows_lean_kernel<N, 4>); break;
