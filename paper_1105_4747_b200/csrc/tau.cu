@@ -5,17 +5,18 @@
 //
 // Every (i,j) pair is evaluated (N^2 per sightline): the kernel is bound by MUFU.EX2 (16 /clk/SM, measured),
 // and on sm_100a every extra FP32 instruction per pair costs MUFU rate long before the issue limit
-// ("pair loop"), so the pair body is 3.25 FP32 instructions + 1 MUFU:
+// ("pair loop"), so the pair body is packed FP32 on two SOURCES at a time -- 1.9 issue slots
+// + 1 MUFU per pair (see "the staged layout" below for the pairing):
 //
-//   staged per source cell j (once per sightline, in shared memory, one float4):
+//   staged per source cell j (once per sightline, in shared memory, four floats):
 //       m_j = j + P_j          P_j = round(v_pec/dv), reduced mod N          (integer-valued float, exact)
 //       w_j = (dv/b_j) sqrt(log2 e)                                          (so exp(-x^2) = ex2(-(x')^2))
 //       g_j = -f_j w_j         f_j = v_pec/dv - round(v_pec/dv)  in [-1/2,1/2] (exact fma residual)
 //       a_j = K 1e-5 nHI_j / b_j                                             (line-centre amplitude)
 //   a thread owns R CONSECUTIVE pixels i_0 .. i_0+R-1; per source cell:
-//       E   = (i_0 + R/2) - m_j (exact) ;  x_ref = fma(E, w_j, g_j)          (2 FP32 per R pairs)
-//       x_r = fma(r - R/2, w_j, x_ref)                                       (1 FFMA, none for r = R/2)
-//       e   = ex2(-x_r * x_r)  ;  acc_r = fma(a_j, e, acc_r)                 (FMUL + MUFU + FFMA)
+//       E   = (i_0 + R/2) - m_j (exact) ;  x_ref = fma(E, w_j, g_j)          (FADD2 + FFMA2 per 2 R pairs)
+//       x_r = fma(r - R/2, w_j, x_ref)                                       (1 FFMA2 / FADD2, none for r = R/2)
+//       e   = ex2(-x_r * x_r)  ;  acc_r = fma(a_j, e, acc_r)                 (FMUL2 + 2 MUFU + FFMA2)
 //
 // Keeping the integer part of the pixel separation exact is what holds the error at ~1e-6 for N = 2048
 // (forming u_j and v_i in fp32 km/s loses 3 digits there); x_ref is at most R/2 cells away
@@ -30,8 +31,8 @@
 // per-pair image choice.  Both loops evaluate all N^2 pairs.
 //
 // Mapping, sightlines along x (contiguous rows): a GROUP of G warps (G = 1 unless the row is too long for
-// enough groups to fit in shared memory) owns one sightline at a time: it stages the row with 128-byte
-// coalesced loads straight into its private float4 cells, syncs only itself (named barrier / __syncwarp),
+// enough groups to fit in shared memory) owns one sightline at a time: it stages the row (four consecutive cells
+// per thread from 128-bit loads) straight into its private cell slots, syncs only itself (named barrier / __syncwarp),
 // sums its tiles and stores R consecutive tau values per lane (128-bit).  Groups never wait for each other,
 // so the MUFU pipe always has warps in the pair loop while others stage; rows are handed out by a global
 // atomic counter, which removes the wave-quantisation tail of a static partition (65,536 rows over
@@ -42,8 +43,8 @@
 //
 // Variants behind lya_tau_sightlines_opt (template flags, same kernels): FUSED applies S1 (gas_cell.h) to delta
 // while staging, so n_HI and b never exist in memory; WIN (LYA_TAU_WINDOWED) lets every lane walk only the
-// 2 reach + R sources around its own pixels (tile_window, over a row staged unwrapped with a periodic halo) --
-// bit-identical output, ~3 % of the pairs at N = 1024.
+// 2 W + R sources around its own pixels (tile_window, over a row staged unwrapped with a periodic halo) --
+// bit-identical output, 3 % of the pairs at N = 1024.  The epilogue can leave per-sightline moments sum tau^k for S4.
 #include "gas_cell.h"
 #include "lya_internal.h"
 
