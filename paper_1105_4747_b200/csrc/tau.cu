@@ -171,8 +171,8 @@ __device__ __forceinline__ float stage4(const TauArgs &a, float jf, float4 nh, f
 // pixels per lane 23 issue slots per 8 pairs instead of 36, which is what the windowed variant, short of issue slots,
 // needs (profiles/r2_ncu_tau_windowed.md); each f32x2 lane is the scalar operation, bit for bit.  Every pixel keeps an
 // (even sources, odd sources) pair of partial sums, added at the end; the full and the windowed walks both start at an
-// even unwrapped source index, so they add the same terms in the same order and stay bit-identical.  The fast walks
-// need n % 4 == 0 (even segment ends for any tile); other rows take the general loop.
+// even unwrapped source index, so they add the same terms in the same order and stay bit-identical (the window needs
+// n % 4 == 0: whole pad groups in the halo; other rows take the full walk).
 // Slots are stored at cpos(slot): plain for the full sum (every lane reads the same slot: broadcast).  For
 // LYA_TAU_WINDOWED, where lane k reads slot s0 + R k, the row is stored UNWRAPPED with a periodic halo of TAU_HALO
 // cells on either side (slot j + TAU_HALO holds slot j; the halo copies carry m -/+ N, so a walk across the ends
@@ -274,7 +274,11 @@ __device__ __forceinline__ void pair_step(const float4 &A, const float4 &B, f32x
 }
 
 // Fast path, full sum: unwrapped walk over all n sources jj = start .. start + n - 1 around the tile centre (at
-// most one wrap), no per-pair image logic.  Lane owns pixels i0 + lane*R + r.  n % 4 == 0: start, j0 and n are even.
+// most one wrap), no per-pair image logic.  Lane owns pixels i0 + lane*R + r.  The walk is in whole pairs of slots: a
+// segment that would begin or end inside a pair takes the whole pair -- the extra source is then met at an image
+// n/2 - 16R + 1 or more pixels from every pixel of the tile, where the validity condition makes its term exactly 0 --
+// and an odd row's last pair holds a dummy cell of amplitude 0.  For n % 4 == 0 (the window's requirement) nothing is
+// extra: start, j0 and n are even.
 template <int R, bool PAD>
 __device__ __forceinline__ void tile_fast(const float4 *__restrict__ cs, int n, int i0, int lane, float (&acc)[R])
 {
@@ -289,7 +293,7 @@ __device__ __forceinline__ void tile_fast(const float4 *__restrict__ cs, int n, 
     for (int r = 0; r < R; ++r) acc2[r] = 0ull;
 #pragma unroll 1
     for (int seg = 0; seg < 2; ++seg) {
-        const int lo = seg ? 0 : j0, hi = seg ? j0 : n;
+        const int lo = seg ? 0 : (j0 & ~1), hi = seg ? ((j0 + 1) & ~1) : ((n + 1) & ~1);
         const f32x2 cref2 = pk(cref, cref);
 #pragma unroll 4
         for (int j = lo; j < hi; j += 2) pair_step<R>(cs[cpos<PAD, R>(j)], cs[cpos<PAD, R>(j + 1)], cref2, acc2);
@@ -344,7 +348,7 @@ __device__ __forceinline__ int tile_window(const float4 *__restrict__ cs, int n,
     return walked;
 }
 
-// General path: nearest image chosen per pair (tiny N, N % 4 != 0, or |v_pec| comparable to the box).
+// General path: nearest image chosen per pair (tiny N, or |v_pec| comparable to the box).
 template <int R, bool PAD>
 __device__ __forceinline__ void tile_general(const float4 *__restrict__ cs, int n, float n_f, float inv_n, int i0,
                                              int lane, float (&acc)[R])
@@ -377,13 +381,13 @@ __device__ __forceinline__ int tile_any(const TauArgs &a, const float4 *cs, floa
                                         float (&acc)[R])
 {
     const int n = a.n;
-    if ((n & 3) || !(reach <= (float)((n >> 1) - 16 * R))) {   // also catches +inf
+    if (!(reach <= (float)((n >> 1) - 16 * R))) {       // also catches +inf
         tile_general<R, WIN>(cs, n, a.n_f, a.inv_n, i0, lane, acc);
         return n;
     }
     if (WIN) {
         const int W = ((int)reach + R - 1) / R * R;         // floor(reach), then whole pad groups on either side
-        if (W + R + 2 <= TAU_HALO && n >= TAU_HALO) return tile_window<R>(cs, n, i0, lane, W, acc);
+        if (W + R + 2 <= TAU_HALO && n >= TAU_HALO && !(n & 3)) return tile_window<R>(cs, n, i0, lane, W, acc);
     }
     tile_fast<R, WIN>(cs, n, i0, lane, acc);
     return n;

@@ -144,7 +144,7 @@ def test_normalisation_on_heavy_tailed_tau_against_the_full_oracle(ctx, oracle, 
 
 
 # ------------------------------------------------------------------ S3 shapes: ragged, tiny, strided, slabs
-@pytest.mark.parametrize("n", [1, 2, 8, 13, 31, 32, 33, 64, 100, 128, 200, 257, 384])
+@pytest.mark.parametrize("n", [1, 2, 8, 13, 31, 32, 33, 64, 100, 128, 200, 257, 258, 384, 1001, 1002])
 def test_tau_ragged_lengths_x_axis(ctx, oracle, n):
     w = scaled(WORKLOADS[2], n)
     rng = np.random.default_rng(n)
