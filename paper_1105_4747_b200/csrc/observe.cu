@@ -386,17 +386,33 @@ __global__ void __launch_bounds__(256) observe_rows_lean_kernel(const ObsArgs a,
 // bank conflict; so the row is staged SPLIT by 16-byte chunk parity -- even chunks (4 pixels each) in one array, odd
 // chunks in another: a thread's window alternates between the two with immediate offsets, and within either array
 // neighbouring lanes read neighbouring chunks.
+// shared-memory loads by 32-bit shared address (the output loop below: no generic-to-shared conversion per access)
+__device__ __forceinline__ unsigned smem_addr(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ float lds_f32(unsigned addr)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(addr) : "memory");
+    return v;
+}
+__device__ __forceinline__ int4 lds_v4(unsigned addr)
+{
+    int4 v;
+    asm volatile("ld.shared.v4.s32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
+    return v;
+}
+
 struct __align__(16) ObsTaps8 {
     float wp[64];                                        // wp[t + 7] = g(KO - t); zero outside the real taps
     float wq[64];                                        // wq[k] = wp[k + 1]
 };
 #define OBS_WPAIR8(k) (((k) & 1) ? pack2(tp.wq[(k) - 1], tp.wq[(k)]) : pack2(tp.wp[(k)], tp.wp[(k) + 1]))
 
-template <int LT>                                        // LT >= L, multiple of 4, <= OBS_PACKED_LT
-__global__ void __launch_bounds__(256) observe_rows_lean8_kernel(const ObsArgs a, const __grid_constant__ ObsTaps8 tp)
+constexpr int OBS_NBR8 = 6;                              // noise draws per thread and row held in registers (8-pixel kernel)
+template <int LT, int T>                                 // LT >= L, multiple of 4, <= OBS_PACKED_LT; T = blockDim.x
+__global__ void __launch_bounds__(T) observe_rows_lean8_kernel(const ObsArgs a, const __grid_constant__ ObsTaps8 tp)
 {
     extern __shared__ __align__(16) float sm[];
-    const int n = a.n, T = blockDim.x, tid = threadIdx.x, nb = a.nb;
+    const int n = a.n, tid = threadIdx.x, nb = a.nb;
     constexpr int NJ = (LT + 8) / 4;                     // chunks in a thread's window
     const int nch = ((n + LT + 12) >> 3) + 1;            // chunks per half of the staged row (logical length n + LT + 12)
     float4 *s_e = reinterpret_cast<float4 *>(sm);        // even chunks of s_in[h] = F[(h - KO) mod n], zero beyond n + L
@@ -407,7 +423,12 @@ __global__ void __launch_bounds__(256) observe_rows_lean8_kernel(const ObsArgs a
     for (int h = tid; h < 2 * nch; h += T) s_e[h] = make_float4(0.f, 0.f, 0.f, 0.f);
     if (tid < 4) s_c[n + tid] = 0.0f;
     if (a.rebin)
-        for (int m = tid; m < nb; m += T) s_b[m] = a.bins[m];
+        for (int m = tid; m < nb; m += T) {
+            int4 e = a.bins[m];
+            if (a.bins3) e.x *= 4;                       // three-pixel bins: first pixel as a byte offset into s_c
+            s_b[m] = e;
+        }
+    const unsigned sc_addr = smem_addr(s_c), sb_addr = smem_addr(s_b) + 16u * tid;
 
     const bool own = 8 * tid < n;                        // this thread owns pixels 8 tid .. 8 tid + 7
     const bool has_halo = tid < a.L;
@@ -422,7 +443,7 @@ __global__ void __launch_bounds__(256) observe_rows_lean8_kernel(const ObsArgs a
     float *dst = a.out + (size_t)blockIdx.x * nb;
     const size_t src_step = row_step * n, out_step = row_step * nb;
     float4 r0 = make_float4(0.f, 0.f, 0.f, 0.f), r1 = r0;
-    float hreg = 0.0f, nzr[OBS_NBR];
+    float hreg = 0.0f, nzr[OBS_NBR8];
     auto fetch = [&]() {
         if (own) {
             r0 = __ldcs(reinterpret_cast<const float4 *>(src + 8 * tid));
@@ -440,7 +461,7 @@ __global__ void __launch_bounds__(256) observe_rows_lean8_kernel(const ObsArgs a
         if (row + row_step < a.n_rows) fetch();
         if (nz) {
 #pragma unroll
-            for (int k = 0; k < OBS_NBR; ++k) {
+            for (int k = 0; k < OBS_NBR8; ++k) {
                 const int m = tid + k * T;
                 nzr[k] = m < nb ? __ldcs(nz + m) : 0.0f;
             }
@@ -468,23 +489,28 @@ __global__ void __launch_bounds__(256) observe_rows_lean8_kernel(const ObsArgs a
 
         const float inv_snr = nz ? a.inv_snr : 0.0f;
         auto put = [&](int k, int m, float v) {
-            if (nz) v = fmaf(k < OBS_NBR ? nzr[k < OBS_NBR ? k : 0] : __ldcs(nz + m), inv_snr, v);
+            if (nz) v = fmaf(k < OBS_NBR8 ? nzr[k < OBS_NBR8 ? k : 0] : __ldcs(nz + m), inv_snr, v);
             __stcs(dst + m, v);
         };
-        if (a.bins3) {                                   // bins <= 2 pixels wide: three pixels {i0, w0, w1, w2}
+        if (a.bins3) {                                   // bins <= 2 pixels wide: three pixels {byte offset, w0, w1, w2}
+            float *dt = dst + tid;                       // every offset below is an immediate (T is a template parameter)
+            const float *nt = nz ? nz + tid : nullptr;
 #pragma unroll
-            for (int k = 0; k < OBS_NBR; ++k) {
-                const int m = tid + k * T;
-                if (m < nb) {
-                    const int4 e = s_b[m];
-                    const float *cc = s_c + e.x;
-                    put(k, m, fmaf(__int_as_float(e.w), cc[2], fmaf(__int_as_float(e.z), cc[1], __int_as_float(e.y) * cc[0])));
+            for (int k = 0; k < OBS_NBR8; ++k) {
+                if (tid + k * T < nb) {
+                    const int4 e = lds_v4(sb_addr + 16u * k * T);
+                    const unsigned ca = sc_addr + (unsigned)e.x;
+                    float v = fmaf(__int_as_float(e.w), lds_f32(ca + 8), fmaf(__int_as_float(e.z), lds_f32(ca + 4), __int_as_float(e.y) * lds_f32(ca)));
+                    if (nz) v = fmaf(nzr[k], inv_snr, v);
+                    __stcs(dt + k * T, v);
                 }
             }
-            for (int m = tid + OBS_NBR * T; m < nb; m += T) {
-                const int4 e = s_b[m];
-                const float *cc = s_c + e.x;
-                put(OBS_NBR, m, fmaf(__int_as_float(e.w), cc[2], fmaf(__int_as_float(e.z), cc[1], __int_as_float(e.y) * cc[0])));
+            for (int m = tid + OBS_NBR8 * T; m < nb; m += T) {
+                const int4 e = lds_v4(sb_addr + 16u * (m - tid));
+                const unsigned ca = sc_addr + (unsigned)e.x;
+                float v = fmaf(__int_as_float(e.w), lds_f32(ca + 8), fmaf(__int_as_float(e.z), lds_f32(ca + 4), __int_as_float(e.y) * lds_f32(ca)));
+                if (nz) v = fmaf(__ldcs(nt + (m - tid)), inv_snr, v);
+                __stcs(dt + (m - tid), v);
             }
         } else if (a.rebin) {                            // wide bins: first pixel, whole pixels, last pixel (weights carry 1/B)
             auto wide = [&](int m) -> float {
@@ -495,9 +521,9 @@ __global__ void __launch_bounds__(256) observe_rows_lean8_kernel(const ObsArgs a
                 for (int i = e.x + 1; i < e.y; ++i) mid += s_c[i];
                 return fmaf(__int_as_float(e.w), s_c[e.y], fmaf(mid, a.inv_bin_f, __int_as_float(e.z) * s_c[e.x]));
             };
-            for (int m = tid, k = 0; m < nb; m += T, ++k) put(k < OBS_NBR ? k : OBS_NBR, m, wide(m));
+            for (int m = tid, k = 0; m < nb; m += T, ++k) put(k < OBS_NBR8 ? k : OBS_NBR8, m, wide(m));
         } else {
-            for (int m = tid, k = 0; m < nb; m += T, ++k) put(k < OBS_NBR ? k : OBS_NBR, m, s_c[m]);
+            for (int m = tid, k = 0; m < nb; m += T, ++k) put(k < OBS_NBR8 ? k : OBS_NBR8, m, s_c[m]);
         }
         dst += out_step;
         if (nz) nz += out_step;
@@ -692,21 +718,23 @@ extern "C" lya_status lya_observe_rows(lya_ctx *ctx, size_t n_rows, int32_t n_pi
             for (int t = 0; t <= a.L + 7 && t + 7 < 64; ++t) t8.wp[t + 4] = ctx->h_taps[t];      // h_taps[t + 3] = g(KO - t)
             for (int t = 0; t < 63; ++t) t8.wq[t] = t8.wp[t + 1];
             void (*lean8)(const ObsArgs, const ObsTaps8) = nullptr;
+            const int threads8 = ((n_pix / 8 + 31) / 32) * 32;
+            const int t8c = threads8 <= 32 ? 32 : (threads8 <= 64 ? 64 : (threads8 <= 128 ? 128 : 256));   // instantiated block sizes
             switch (LT) {
-#define LYA_LEAN8(N) case N: lean8 = observe_rows_lean8_kernel<N>; break;
+#define LYA_LEAN8(N) case N: lean8 = t8c == 32 ? observe_rows_lean8_kernel<N, 32> : (t8c == 64 ? observe_rows_lean8_kernel<N, 64> \
+                             : (t8c == 128 ? observe_rows_lean8_kernel<N, 128> : observe_rows_lean8_kernel<N, 256>)); break;
                 LYA_LEAN8(0) LYA_LEAN8(4) LYA_LEAN8(8) LYA_LEAN8(12) LYA_LEAN8(16) LYA_LEAN8(20) LYA_LEAN8(24)
                 LYA_LEAN8(28) LYA_LEAN8(32) LYA_LEAN8(36) LYA_LEAN8(40)
 #undef LYA_LEAN8
             }
-            const int threads8 = ((n_pix / 8 + 31) / 32) * 32;
             const size_t nch = (((size_t)n_pix + LT + 12) >> 3) + 1;
             const size_t smem8 = 2 * nch * sizeof(float4) + ((size_t)n_pix + 4) * sizeof(float) + (a.rebin ? (size_t)nb * sizeof(int4) : 0);
             int per_sm8 = 0;
-            lya_status st8 = lya_kernel_occupancy(ctx, (const void *)lean8, threads8, smem8, &per_sm8);
+            lya_status st8 = lya_kernel_occupancy(ctx, (const void *)lean8, t8c, smem8, &per_sm8);
             if (st8 != LYA_OK) return st8;
-            if (lean8 && per_sm8 >= 1 && a.L <= threads8) {
+            if (lean8 && per_sm8 >= 1 && a.L <= t8c) {
                 const size_t cap8 = (size_t)ctx->sm_count * per_sm8;
-                lean8<<<(int)(n_rows < cap8 ? n_rows : cap8), threads8, smem8, ctx->stream>>>(a, t8);
+                lean8<<<(int)(n_rows < cap8 ? n_rows : cap8), t8c, smem8, ctx->stream>>>(a, t8);
                 ctx->launches++;
                 LYA_CUDA(ctx, cudaGetLastError());
                 return LYA_OK;
