@@ -61,6 +61,50 @@ def test_sharded_normalisation_two_ranks_gloo(tmp_path, oracle, f_target, moment
     assert abs(f - f_target) < 1e-9 and iters <= (6 if moments else 20)
 
 
+def _nested_worker(rank: int, world: int, port: int, f_target: float, out_path: str):
+    """The nested iteration of normalize_mean_flux_sharded (A = 0 pass, subsample passes, then passes over all of
+    tau) with numpy standing in for lya_flux_moment_sums_sub: every `every`-th chunk of 1024 pixels of the local tau."""
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    from paper_1105_4747_b200 import lya
+    rng = np.random.default_rng(4748)
+    tau_all = rng.lognormal(mean=-0.6, sigma=2.2, size=400_000).astype(np.float32)     # heavy tail: max ~ 1e4 x median
+    lo, hi = (0, 150_000) if rank == 0 else (150_000, tau_all.size)
+    tau = tau_all[lo:hi].astype(np.float64)
+    calls = []
+
+    def kernel_sums(a, every):
+        t = tau if every <= 1 else np.concatenate([tau[c: c + 1024] for c in range(0, tau.size, 1024 * every)])
+        e = np.exp(-a * t)
+        calls.append(every)
+        return [float((t ** k * e).sum()) for k in range(5)], int(t.size)
+
+    stats = {}
+    A, f, passes = lya.normalize_mean_flux_sharded(None, None, f_target, tau_all.size, rel_tol=1e-9, kernel_sums=kernel_sums,
+                                                   sub_every=8, sub_min_pix=0, stats=stats)
+    got = torch.tensor([A, f, float(passes), float(stats["sub_passes"]), float(sum(1 for c in calls if c <= 1))], dtype=torch.float64)
+    gathered = [torch.zeros_like(got) for _ in range(world)]
+    dist.all_gather(gathered, got)
+    if rank == 0:
+        np.save(out_path, np.stack([g.numpy() for g in gathered]))
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("f_target", [0.80, 0.35])
+def test_sharded_nested_iteration_two_ranks_gloo(tmp_path, oracle, f_target):
+    out = str(tmp_path / "res.npy")
+    mp.spawn(_nested_worker, args=(2, _free_port(), f_target, out), nprocs=2, join=True)
+    res = np.load(out)
+    assert np.array_equal(res[0], res[1]), "ranks disagree"
+    A, f, passes, sub_passes, full_calls = res[0]
+    rng = np.random.default_rng(4748)
+    tau_all = rng.lognormal(mean=-0.6, sigma=2.2, size=400_000).astype(np.float32).astype(np.float64)
+    A_ref, _, _ = oracle.normalize_mean_flux(tau_all, f_target)
+    assert abs(A / A_ref - 1.0) < 1e-8 and abs(f - f_target) < 1e-9
+    # the subsample did the climbing: the A = 0 pass plus at most two passes over all of tau
+    assert sub_passes >= 2 and passes == full_calls <= 3
+
+
 def test_sharded_weak_scaling_slabs_are_independent_problems():
     """bench.py's N > 1 layout: rank r generates ITS slab from (seed + 100 r): no rank needs another's cells."""
     from paper_1105_4747_b200 import inputs
