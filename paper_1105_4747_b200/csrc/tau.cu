@@ -254,9 +254,35 @@ __device__ __forceinline__ void fill_halo(float4 *cs, int n, float n_f, int t0, 
     }
 }
 
+// 2^(-q) for q >= 0 on the FMA pipe, two values at a time (degree-5 minimax polynomial on the fractional part, relative
+// error 2.3e-7 in fp32 -- MUFU.EX2's own is 2^-22 = 2.4e-7 -- and the exponent put in by an integer multiply-add).
+// q >= 127.5 gives exactly 0 (the scale factor's exponent is clamped), which is all the windowed variant relies on:
+// the terms it skips have q >= 127.69.
+__device__ __forceinline__ f32x2 ex2_poly2_neg(f32x2 q2)                 // 2^(-q), q >= 0
+{
+    const f32x2 magic = pk(12582912.0f, 12582912.0f);             // 1.5 * 2^23
+    const f32x2 tn = sub2(magic, q2);                             // low mantissa bits = rint(-q)
+    const f32x2 h  = add2(q2, sub2(tn, magic));                   // q + rint(-q) = -(fractional part) in [-1/2, 1/2], exact
+    f32x2 p = fma2(pk(-1.327647245e-03f, -1.327647245e-03f), h, pk(9.675540961e-03f, 9.675540961e-03f));   // odd signs flipped
+    p = fma2(p, h, pk(-5.550713092e-02f, -5.550713092e-02f));
+    p = fma2(p, h, pk(2.402212024e-01f, 2.402212024e-01f));
+    p = fma2(p, h, pk(-6.931469440e-01f, -6.931469440e-01f));
+    p = fma2(p, h, pk(1.000000119e+00f, 1.000000119e+00f));
+    float n0, n1;
+    unpk(tn, n0, n1);
+    // scale = 2^max(n, -127): bits (n + 127) << 23 with n + 127 = bits(tn) - (0x4B400000 - 127), clamped at 0 -> 0.0f
+    const int k0 = max(__float_as_int(n0), 0x4B400000 - 127), k1 = max(__float_as_int(n1), 0x4B400000 - 127);
+    const float s0 = __int_as_float((k0 - (0x4B400000 - 127)) << 23), s1 = __int_as_float((k1 - (0x4B400000 - 127)) << 23);
+    return mul2(p, pk(s0, s1));
+}
+
 // Two sources (one pair of slots) against the R pixels of a lane: cref2 = (c, c) with c the reference pixel's
 // (unwrapped) index, so E = c - m is the exact integer separation; acc2[r] = (sum over even, sum over odd sources).
-template <int R>
+// POLY: the exponentials of the lane's LAST pixel go to the FMA pipe (ex2_poly2) instead of the MUFU pipe.  The walks
+// set POLY on every second source pair (odd pair index, an absolute property of the pair), so one exponential in
+// eight leaves the pipe that bounds the kernel; the packed loop has the issue slots and the FMA cycles to spare
+// (DESIGN.md section 6).  R < 4 (rows shorter than 128 pixels: launch-bound) never takes it.
+template <int R, bool POLY>
 __device__ __forceinline__ void pair_step(const float4 &A, const float4 &B, f32x2 cref2, f32x2 (&acc2)[R])
 {
     constexpr int RH = R / 2;
@@ -267,9 +293,13 @@ __device__ __forceinline__ void pair_step(const float4 &A, const float4 &B, f32x
         // x_r = (r - RH) w + x_ref, one rounding: +-1 as a packed add / subtract, the others as a packed fma
         const f32x2 x = (r == RH) ? xr : (r == RH + 1) ? add2(xr, w2) : (r == RH - 1) ? sub2(xr, w2)
                                        : fma2(pk((float)(r - RH), (float)(r - RH)), w2, xr);
-        float t0, t1;
-        unpk(mul2(x, x), t0, t1);
-        acc2[r] = fma2(a2, pk(ex2_ftz(-t0), ex2_ftz(-t1)), acc2[r]);
+        if (POLY && R >= 4 && r == R - 1) {
+            acc2[r] = fma2(a2, ex2_poly2_neg(mul2(x, x)), acc2[r]);
+        } else {
+            float t0, t1;
+            unpk(mul2(x, x), t0, t1);
+            acc2[r] = fma2(a2, pk(ex2_ftz(-t0), ex2_ftz(-t1)), acc2[r]);
+        }
     }
 }
 
@@ -295,8 +325,17 @@ __device__ __forceinline__ void tile_fast(const float4 *__restrict__ cs, int n, 
     for (int seg = 0; seg < 2; ++seg) {
         const int lo = seg ? 0 : (j0 & ~1), hi = seg ? ((j0 + 1) & ~1) : ((n + 1) & ~1);
         const f32x2 cref2 = pk(cref, cref);
-#pragma unroll 4
-        for (int j = lo; j < hi; j += 2) pair_step<R>(cs[cpos<PAD, R>(j)], cs[cpos<PAD, R>(j + 1)], cref2, acc2);
+        int j = lo;
+        if ((j & 2) && j < hi) {                          // odd pair index first: get onto a multiple of 4
+            pair_step<R, true>(cs[cpos<PAD, R>(j)], cs[cpos<PAD, R>(j + 1)], cref2, acc2);
+            j += 2;
+        }
+#pragma unroll 2
+        for (; j + 2 < hi; j += 4) {
+            pair_step<R, false>(cs[cpos<PAD, R>(j)], cs[cpos<PAD, R>(j + 1)], cref2, acc2);
+            pair_step<R, true>(cs[cpos<PAD, R>(j + 2)], cs[cpos<PAD, R>(j + 3)], cref2, acc2);
+        }
+        if (j < hi) pair_step<R, false>(cs[cpos<PAD, R>(j)], cs[cpos<PAD, R>(j + 1)], cref2, acc2);
         cref -= (float)n;
     }
 #pragma unroll
@@ -333,10 +372,12 @@ __device__ __forceinline__ int tile_window(const float4 *__restrict__ cs, int n,
     f32x2 acc2[R];
 #pragma unroll
     for (int r = 0; r < R; ++r) acc2[r] = 0ull;
+    // pair parity is absolute: s0l is a multiple of 4 for R = 4 (slots 0, 1 of a pad group: even pair; 2, 3: odd pair);
+    // R < 4 never takes the polynomial
 #pragma unroll 2
     for (int g = 0; g < groups; ++g) {
-#pragma unroll
-        for (int k = 0; k < PG; k += 2) pair_step<R>(q4[k], q4[k + 1], cref2, acc2);
+        pair_step<R, false>(q4[0], q4[1], cref2, acc2);
+        if (PG == 4) pair_step<R, true>(q4[2], q4[3], cref2, acc2);
         q4 += R > 1 ? R + 1 : 2;
     }
 #pragma unroll
