@@ -6,7 +6,8 @@
 // Every (i,j) pair is evaluated (N^2 per sightline): the kernel is bound by MUFU.EX2 (16 /clk/SM, measured),
 // and on sm_100a every extra FP32 instruction per pair costs MUFU rate long before the issue limit
 // ("pair loop"), so the pair body is packed FP32 on two SOURCES at a time -- 1.9 issue slots
-// + 1 MUFU per pair (see "the staged layout" below for the pairing):
+// + 1 MUFU per pair (see "the staged layout" below for the pairing) -- and one exponential in eight is a packed
+// polynomial on the otherwise half-idle FMA pipe (ex2_poly2_neg), which lifts the bound to 16 / (1 - 1/8) per clk and SM:
 //
 //   staged per source cell j (once per sightline, in shared memory, four floats):
 //       m_j = j + P_j          P_j = round(v_pec/dv), reduced mod N          (integer-valued float, exact)
