@@ -198,6 +198,23 @@ lya_status lya_root_update_moments(lya_root_state *s, const double *sums5);
 lya_status lya_flux_moment_sums_sub(lya_ctx *ctx, const float *tau, size_t n_pix, double a_trial, int32_t every,
                                     double *sums5, uint64_t *n_sub);
 
+/* The same five sums (the pass over tau behind every trial A) for callers that may NOT allocate -- code
+ * under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.  The call allocates nothing and
+ * frees nothing (no cudaMalloc / cudaFree, no allocating library routine) and does not synchronise: it enqueues two
+ * kernels on ctx's stream.  Its per-block scratch is a file-scope static __device__ array of
+ * 16384 blocks x 5 doubles = 655,360 B, which every GPU that loads the library holds until the process exits.
+ *   tau    DEVICE, n_pix floats (4-byte aligned; 128-bit loads if 16-byte aligned), may be NULL if n_pix == 0;
+ *   sums5  DEVICE, 5 doubles (8-byte aligned), owned by the caller: valid once the stream has reached this call.
+ * Block b sums the fixed pixel range [b, b + 1) * 65536, so the result does not depend on the SM count; it agrees
+ * with lya_flux_moment_sums to fp32-grouping rounding (~1e-8 relative).  LYA_EINVAL (message: lya_last_error) for
+ * n_pix > LYA_STATIC_MAX_PIX, for a null / misaligned pointer and for a trial outside [0, 1e30).  All calls on a
+ * device SHARE the array: calls that overlap on the GPU (different streams with no ordering between them, different
+ * ctx or threads) race; calls on one stream are safe back to back.  Nothing in the array has to start at zero: each
+ * call writes every partial it reads.  The first call on a device resolves the array's device address
+ * (cudaGetSymbolAddress): make that one outside stream capture. */
+#define LYA_STATIC_MAX_PIX ((size_t)1 << 30)
+lya_status lya_flux_moment_sums_static(lya_ctx *ctx, const float *tau, size_t n_pix, double a_trial, double *sums5);
+
 /* S5.  tau, flux: DEVICE, n_pix floats; flux == tau (in place) allowed.  Asynchronous. */
 lya_status lya_flux(lya_ctx *ctx, const float *tau, size_t n_pix, double a, float *flux);
 

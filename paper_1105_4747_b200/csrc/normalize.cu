@@ -599,3 +599,100 @@ lya_status lya_run_flux_with_pdf(lya_ctx *ctx, const float *tau, size_t n, doubl
     }
     return LYA_OK;
 }
+
+// ---------------------------------------------------------------------------------------------------------------------
+// lya_flux_moment_sums_static: the five tilted moments of S4 for callers that may not allocate -- code
+// under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc.  The per-block partials, which every other
+// reduction of this file keeps in ctx->d_partials (cudaMalloc'ed by lya_create), live in the file-scope array below:
+// LYA_STATIC_MAX_BLOCKS x 5 doubles = 655,360 B of device memory held by every GPU that loads the library, until exit.
+// Block b owns the FIXED pixel range [b, b + 1) * LYA_STATIC_PIX_PER_BLOCK, so the result does not depend on the SM
+// count, and the largest input is LYA_STATIC_MAX_PIX = 16384 * 65536 = 2^30 pixels (config 4's whole grid).
+// Every partial the finishing kernel reads is written by the same call first: nothing has to start at zero.  All calls
+// on a device share the array: calls that overlap on the GPU (different streams, no ordering) race.
+// ---------------------------------------------------------------------------------------------------------------------
+#define LYA_STATIC_PIX_PER_BLOCK 65536
+#define LYA_STATIC_MAX_BLOCKS    16384
+
+static __device__ __align__(256) double lya_static_partials[(size_t)LYA_STATIC_MAX_BLOCKS * 5];
+
+namespace {
+
+__global__ void __launch_bounds__(RED_THREADS) static_moment_sums_kernel(const float *__restrict__ tau, size_t n, const Trial tr,
+                                                                        double *partials)
+{
+    __shared__ double sh[5 * 32];
+    const size_t lo = (size_t)blockIdx.x * LYA_STATIC_PIX_PER_BLOCK;
+    const size_t hi = lo + LYA_STATIC_PIX_PER_BLOCK < n ? lo + LYA_STATIC_PIX_PER_BLOCK : n;
+    double s[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+    float q[5];
+    auto add1 = [&](float t) {
+        float p = flux_of(t, tr);
+#pragma unroll
+        for (int k = 0; k < 5; ++k) { q[k] += p; p *= t; }
+    };
+    auto flush = [&]() {                                 // fp32 inside a group of up to 16 pixels, double above
+#pragma unroll
+        for (int k = 0; k < 5; ++k) { s[k] += (double)q[k]; q[k] = 0.0f; }
+    };
+#pragma unroll
+    for (int k = 0; k < 5; ++k) q[k] = 0.0f;
+    if (((uintptr_t)tau & 15) == 0) {                    // lo is a multiple of 4 pixels: 128-bit loads
+        const float4 *t4 = reinterpret_cast<const float4 *>(tau + lo);
+        const size_t n4 = (hi - lo) >> 2;
+        size_t i = threadIdx.x;
+        for (; i + 3 * RED_THREADS < n4; i += 4 * RED_THREADS) {
+            const float4 t0 = __ldg(t4 + i), t1 = __ldg(t4 + i + RED_THREADS), t2 = __ldg(t4 + i + 2 * RED_THREADS),
+                         t3 = __ldg(t4 + i + 3 * RED_THREADS);
+            add1(t0.x); add1(t0.y); add1(t0.z); add1(t0.w);
+            add1(t1.x); add1(t1.y); add1(t1.z); add1(t1.w);
+            add1(t2.x); add1(t2.y); add1(t2.z); add1(t2.w);
+            add1(t3.x); add1(t3.y); add1(t3.z); add1(t3.w);
+            flush();
+        }
+        for (; i < n4; i += RED_THREADS) {
+            const float4 t0 = __ldg(t4 + i);
+            add1(t0.x); add1(t0.y); add1(t0.z); add1(t0.w);
+            flush();
+        }
+        for (size_t e = lo + (n4 << 2) + threadIdx.x; e < hi; e += RED_THREADS) { add1(tau[e]); flush(); }
+    } else {
+        for (size_t e = lo + threadIdx.x; e < hi; e += RED_THREADS) { add1(tau[e]); flush(); }
+    }
+    block_sum<5>(s, sh);
+    if (threadIdx.x == 0)
+#pragma unroll
+        for (int k = 0; k < 5; ++k) partials[(size_t)blockIdx.x * 5 + k] = s[k];
+}
+
+// device address of lya_static_partials per device (the array's name is only a host-side stand-in in host code)
+constexpr int STATIC_MAX_DEVICES = 64;
+double *g_static_addr[STATIC_MAX_DEVICES];
+
+}  // namespace
+
+extern "C" lya_status lya_flux_moment_sums_static(lya_ctx *ctx, const float *tau, size_t n_pix, double a_trial, double *sums5)
+{
+    if (!ctx) return LYA_EINVAL;
+    ctx->err[0] = 0;
+    if ((n_pix > 0 && (!tau || ((uintptr_t)tau & 3))) || !sums5 || ((uintptr_t)sums5 & 7))
+        return lya_fail(ctx, LYA_EINVAL, "lya_flux_moment_sums_static: null or misaligned pointer");
+    if (!(a_trial >= 0.0) || !(a_trial < 1.0e30))
+        return lya_fail(ctx, LYA_EINVAL, "lya_flux_moment_sums_static: trial A must be finite and >= 0");
+    if (n_pix > (size_t)LYA_STATIC_MAX_PIX)
+        return lya_fail(ctx, LYA_EINVAL, "lya_flux_moment_sums_static: n_pix exceeds LYA_STATIC_MAX_PIX (2^30 pixels: the static "
+                                         "scratch holds 16384 blocks of 65536 pixels); split the input or use lya_flux_moment_sums");
+    if (ctx->device < 0 || ctx->device >= STATIC_MAX_DEVICES)
+        return lya_fail(ctx, LYA_EINVAL, "lya_flux_moment_sums_static: device index beyond 63");
+    LYA_CUDA(ctx, cudaSetDevice(ctx->device));
+    double *part = g_static_addr[ctx->device];
+    if (!part) {                                         // set-up, once per device, with that device current
+        LYA_CUDA(ctx, cudaGetSymbolAddress((void **)&part, lya_static_partials));
+        g_static_addr[ctx->device] = part;               // (two threads racing here store the same address)
+    }
+    const int grid = (int)((n_pix + LYA_STATIC_PIX_PER_BLOCK - 1) / LYA_STATIC_PIX_PER_BLOCK);
+    if (grid > 0) static_moment_sums_kernel<<<grid, RED_THREADS, 0, ctx->stream>>>(tau, n_pix, make_trial(a_trial), part);
+    finish_sums_kernel<<<1, RED_THREADS, 0, ctx->stream>>>(part, grid, 5, sums5);        // n_pix == 0: five zeros
+    ctx->launches += grid > 0 ? 2 : 1;
+    LYA_CUDA(ctx, cudaGetLastError());
+    return LYA_OK;
+}

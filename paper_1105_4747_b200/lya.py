@@ -93,7 +93,9 @@ EXPORTS = ("lya_version", "lya_status_string", "lya_scalars_from_params", "lya_c
            "lya_root_update_moments", "lya_flux_with_pdf", "lya_forest_host_begin", "lya_forest_moment_sums",
            "lya_forest_host_finish", "lya_measure_hbm_peak", "lya_normalize_mean_flux_rows", "lya_row_moment_sums",
            "lya_set_normalize_subsample", "lya_last_normalize_stats", "lya_flux_moment_sums_sub",
-           "lya_forest_moment_sums_sub")
+           "lya_forest_moment_sums_sub", "lya_flux_moment_sums_static")
+
+STATIC_MAX_PIX = 1 << 30                                 # LYA_STATIC_MAX_PIX of include/lya.h
 
 _lib = None
 
@@ -129,6 +131,7 @@ def lib() -> C.CDLL:
     L.lya_root_init.argtypes = [C.POINTER(CRootState), C.c_double, C.c_double, C.c_double]
     L.lya_root_update.argtypes = [C.POINTER(CRootState), C.c_double, C.c_double]
     L.lya_flux_moment_sums.argtypes = [vp, fp, C.c_size_t, C.c_double, dp]
+    L.lya_flux_moment_sums_static.argtypes = [vp, fp, C.c_size_t, C.c_double, vp]
     L.lya_root_update_moments.argtypes = [C.POINTER(CRootState), dp]
     L.lya_flux_moment_sums_sub.argtypes = [vp, fp, C.c_size_t, C.c_double, C.c_int32, dp, C.POINTER(C.c_uint64)]
     L.lya_forest_moment_sums_sub.argtypes = [vp, C.c_double, C.c_int32, dp, C.POINTER(C.c_uint64)]
@@ -322,6 +325,14 @@ class Context:
         s5 = (C.c_double * 5)()
         self._check(lib().lya_flux_moment_sums(self._h, _dev(tau, "tau"), tau.numel(), a_trial, s5))
         return list(s5)
+
+    def flux_moment_sums_static(self, tau, a_trial: float, out):
+        """lya_flux_moment_sums_static: the five sums into `out` (5 float64 on the device, the caller's), asynchronous; the
+        call allocates nothing (static device scratch; at most STATIC_MAX_PIX pixels; overlapping calls race)."""
+        if not (out.is_cuda and out.dtype == torch.float64 and out.is_contiguous() and out.numel() == 5):
+            raise TypeError("out: 5 contiguous float64 on the device required")
+        self._check(lib().lya_flux_moment_sums_static(self._h, _dev(tau, "tau"), tau.numel(), a_trial, out.data_ptr()))
+        return out
 
     def flux_moment_sums_sub(self, tau, a_trial: float, every: int):
         """The five tilted moments over every `every`-th 4 KiB chunk of tau; returns (sums5, pixels summed over)."""
