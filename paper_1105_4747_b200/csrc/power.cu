@@ -15,6 +15,9 @@
 // in double registers across all the CTA's row pairs -- no final store, no read-out pass, two barriers per pair
 // instead of four -- and the host folds k and N - k once at the end.  Other sizes write the last pass to shared
 // memory and read the pairs (m, N - m) out (accumulated in double per CTA).
+// Rows of 1024 and 2048 pixels (configs 4 and 5) take flux_power_warp_kernel instead: ONE WARP per transform (32 x 32
+// in two register passes, 2048 as two such transforms by a radix-2 split shared by a team of two warps), the next row
+// pair prefetched by cp.async, no CTA barrier in the loop: 1.30 -> 0.91 ms on 1024^3, 1.36 -> 1.04 ms on 2048-pixel rows.
 #include "lya_internal.h"
 #include "pdf_bin.h"
 
@@ -251,6 +254,192 @@ __global__ void __launch_bounds__(256) flux_power_kernel(const PowArgs a)
     lya_publish_last_cta(a.acc, a.n_acc, a.host, a.ticket);
 }
 
+// ---- one WARP per row pair, two passes, no CTA barrier (rows of N = N1 * N2 pixels, N2 = 32 or 64) --------------------
+// ncu on the kernel above (1024-pixel rows): issue slots 55 % busy, barrier stall 5.0 and long-scoreboard 3.0 cycles per
+// issued instruction, half of the threads idle in the radix-16 passes; prefetching the next pair with cp.async changed
+// nothing (1.30 -> 1.26 ms), so the limit is the pass -> barrier -> pass chain itself.  Here a warp owns a whole
+// transform (Cooley-Tukey, n = n2 + N2 n1, k = k1 + N1 k2):
+//   pass 1  lane holds x[n2 + N2 n1], n1 < N1, for its residues n2 = lane (+ 32): coalesced 128-byte loads, an N1-point
+//           DFT in registers, the twiddles W_N^(n2 k1) from a per-CTA table [k1][n2], the result to the warp's private
+//           exchange buffer [k1][n2] (row stride N2 + 1 float2: conflict-free both ways);
+//   pass 2  lane holds Y[n2][k1], n2 < N2, for its k1 = lane (+ 32): an N2-point DFT in registers, |Z(k)|^2 added to
+//           fp32 accumulators in registers -- flushed to the double device accumulators every 256 pairs and at the end
+//           (through a per-CTA sum in shared memory), so an fp32 accumulator never holds more than 256 terms.
+// Only __syncwarp() orders the two passes; every load of a pair (64 per lane at N = 1024) is in flight at once.
+__device__ __forceinline__ unsigned pw_smem_addr(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void cp_async16(unsigned dst, const void *src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+template <int R, bool PACK>
+__device__ __forceinline__ void dft_regs64(float2 (&v)[R])   // as dft_regs, twiddles W_64^q (R <= 64)
+{
+    constexpr float C[32] = {1.f, 0.99518472667219693f, 0.98078528040323043f, 0.95694033573220882f, 0.92387953251128674f,
+        0.88192126434835505f, 0.83146961230254524f, 0.77301045336273699f, 0.70710678118654757f, 0.63439328416364549f,
+        0.55557023301960229f, 0.47139673682599781f, 0.38268343236508984f, 0.29028467725446233f, 0.19509032201612833f,
+        0.09801714032956077f, 0.f, -0.098017140329560645f, -0.19509032201612819f, -0.29028467725446216f,
+        -0.38268343236508973f, -0.4713967368259977f, -0.55557023301960196f, -0.63439328416364538f, -0.70710678118654746f,
+        -0.77301045336273699f, -0.83146961230254535f, -0.88192126434835494f, -0.92387953251128674f, -0.95694033573220882f,
+        -0.98078528040323043f, -0.99518472667219682f};
+    constexpr float S[32] = {0.f, 0.098017140329560604f, 0.19509032201612825f, 0.29028467725446233f, 0.38268343236508978f,
+        0.47139673682599764f, 0.55557023301960218f, 0.63439328416364549f, 0.70710678118654746f, 0.77301045336273699f,
+        0.83146961230254524f, 0.88192126434835494f, 0.92387953251128674f, 0.95694033573220894f, 0.98078528040323043f,
+        0.99518472667219682f, 1.f, 0.99518472667219693f, 0.98078528040323043f, 0.95694033573220894f, 0.92387953251128674f,
+        0.88192126434835505f, 0.83146961230254546f, 0.7730104533627371f, 0.70710678118654757f, 0.63439328416364549f,
+        0.55557023301960218f, 0.47139673682599786f, 0.38268343236508989f, 0.29028467725446239f, 0.19509032201612861f,
+        0.098017140329560826f};
+#pragma unroll
+    for (int len = R; len >= 2; len >>= 1) {
+        const int half = len >> 1;
+#pragma unroll
+        for (int s = 0; s < R; s += len) {
+#pragma unroll
+            for (int p = 0; p < half; ++p) {
+                const float2 a = v[s + p], b = v[s + p + half];
+                v[s + p] = PACK ? cadd(a, b) : make_float2(a.x + b.x, a.y + b.y);
+                const float2 d = PACK ? csub(a, b) : make_float2(a.x - b.x, a.y - b.y);
+                const int q = p * (64 / len);              // W_len^p = exp(-2 pi i q / 64), q < 32
+                if (q == 0)       v[s + p + half] = d;
+                else if (q == 16) v[s + p + half] = make_float2(d.y, -d.x);          // times -i
+                else              v[s + p + half] = cmul(d, make_float2(C[q], -S[q]));
+            }
+        }
+    }
+}
+
+constexpr int PW_FLUSH = 256;                            // pairs between two flushes of the fp32 accumulators
+
+// NT = N1 N2 is the transform a warp does in two passes.  SPLIT: rows of N = 2 NT pixels, by one radix-2 decimation
+// in frequency at load time -- Z(2 k') = DFT_NT(z[m] + z[m + NT]), Z(2 k' + 1) = DFT_NT((z[m] - z[m + NT]) W_N^m) -- so
+// the two halves are independent NT-point transforms whose outputs are final (no combining step): a TEAM of two warps
+// shares one staged pair, warp h of the team takes half h, and only two 64-thread named barriers per pair tie them
+// together (pair landed / pair read).  A serial version (one warp, both halves) fits only 8 warps per SM next to its
+// 16 KiB stage buffers and measured 1.40 ms on 2048-pixel rows, no better than the CTA-per-pair kernel.
+// STAGE (16-byte aligned flux; required by SPLIT): the NEXT pair streams into the stage buffer (cp.async, 8 N bytes)
+// while the current one is transformed, so no warp waits out an HBM latency (1024-pixel rows: 0.99 -> 0.92 ms).
+template <int N1, int N2, bool SPLIT, bool STAGE, int WARPS, int MINB>
+__global__ void __launch_bounds__(WARPS * 32, MINB) flux_power_warp_kernel(const PowArgs a)
+{
+    constexpr int NT = N1 * N2, H = SPLIT ? 2 : 1, N = H * NT;
+    constexpr int UNITS = WARPS / H;                     // row pairs in flight per CTA (a unit = a warp, or a team of two)
+    constexpr int S1 = N2 / 32, S2 = N1 / 32;            // residues n2 (pass 1) / outputs k1 (pass 2) per lane
+    constexpr int XS = N2 + 1;                           // exchange row stride [float2]
+    static_assert(N1 % 32 == 0 && N2 % 32 == 0 && (STAGE || !SPLIT) && WARPS % H == 0 && UNITS <= 15, "unsupported plan");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int unit = SPLIT ? warp >> 1 : warp, h = SPLIT ? warp & 1 : 0;
+    float2 *tw  = reinterpret_cast<float2 *>(smem_raw);  // [N1][N2]: W_NT^(n2 k1)
+    float2 *tw2 = tw + NT;                               // SPLIT: [NT] inv_mean W_N^m
+    float2 *ex  = tw2 + (SPLIT ? NT : 0) + warp * (N1 * XS);
+    float *stg  = reinterpret_cast<float *>(tw2 + (SPLIT ? NT : 0) + WARPS * (N1 * XS)) + unit * (2 * N);
+    auto stage = [&](size_t pair) {                      // rows 2 pair (and 2 pair + 1 if it exists): contiguous floats
+        const float *src = a.flux + (2 * pair) * (size_t)N;
+        const int chunks = (2 * pair + 1 < a.n_rows ? 2 * N : N) >> 2;
+        const unsigned d = pw_smem_addr(stg);
+        for (int c = lane + 32 * h; c < chunks; c += 32 * H) cp_async16(d + 16u * c, src + 4 * c);
+    };
+    auto unit_sync = [&]() {                             // the warps that share a stage buffer
+        if (SPLIT) asm volatile("bar.sync %0, 64;" ::"r"(unit + 1) : "memory");
+        else       __syncwarp();
+    };
+    for (int i = threadIdx.x; i < NT; i += WARPS * 32) {
+        const int k1 = i / N2, n2 = i - k1 * N2;
+        float sn, cs;
+        sincospif(2.0f * (float)((k1 * n2) & (NT - 1)) / (float)NT, &sn, &cs);
+        tw[i] = make_float2(cs, -sn);
+        if (SPLIT) {
+            sincospif(2.0f * (float)i / (float)N, &sn, &cs);
+            tw2[i] = make_float2(cs * a.inv_mean, -sn * a.inv_mean);
+        }
+    }
+    __syncthreads();
+    float acc[S2][N2];
+#pragma unroll
+    for (int s = 0; s < S2; ++s)
+#pragma unroll
+        for (int t = 0; t < N2; ++t) acc[s][t] = 0.0f;
+    auto flush = [&]() {                                 // fp32 accumulators -> the device's doubles
+#pragma unroll
+        for (int s = 0; s < S2; ++s)
+#pragma unroll
+            for (int t = 0; t < N2; ++t) {               // transform output k' = k1 + N1 k2 is Z(H k' + h)
+                atomicAdd(a.acc + H * ((lane + 32 * s) + N1 * t) + h, (double)acc[s][bitrev<N2>(t)]);
+                acc[s][bitrev<N2>(t)] = 0.0f;
+            }
+    };
+    const size_t n_pairs = (a.n_rows + 1) >> 1, step = (size_t)gridDim.x * UNITS;
+    const float im = a.inv_mean;
+    int since = 0;
+    size_t pair = (size_t)blockIdx.x * UNITS + unit;
+    if (STAGE) {
+        if (pair < n_pairs) stage(pair);
+        cp_async_commit();
+    }
+    for (; pair < n_pairs; pair += step) {
+        const float *ra = STAGE ? stg : a.flux + (2 * pair) * (size_t)N, *rb = ra + N;
+        const bool has_b = 2 * pair + 1 < a.n_rows;
+        if (STAGE) {
+            cp_async_wait_all();
+            unit_sync();                                 // every lane's chunks of this pair have landed
+        }
+#pragma unroll
+        for (int s = 0; s < S1; ++s) {                   // pass 1 for residue n2 = lane + 32 s: points m = n2 + N2 t
+            const int n2 = lane + 32 * s;
+            float2 v[N1];
+            if (!SPLIT) {
+#pragma unroll
+                for (int t = 0; t < N1; ++t) v[t].x = STAGE ? ra[n2 + N2 * t] : __ldcs(ra + n2 + N2 * t);
+#pragma unroll
+                for (int t = 0; t < N1; ++t) v[t].y = !has_b ? 0.0f : STAGE ? rb[n2 + N2 * t] : __ldcs(rb + n2 + N2 * t);
+            } else {                                     // z[m] +- z[m + NT] of the raw fluxes (dF is applied below)
+#pragma unroll
+                for (int t = 0; t < N1; ++t) {
+                    const int m = n2 + N2 * t;
+                    const float xa = ra[m], ya = ra[m + NT], xb = has_b ? rb[m] : 0.0f, yb = has_b ? rb[m + NT] : 0.0f;
+                    v[t] = h == 0 ? make_float2(xa + ya, xb + yb) : make_float2(xa - ya, xb - yb);
+                }
+            }
+            if (STAGE && s == S1 - 1) {                  // the stage buffer has been read: fetch the next pair into it
+                unit_sync();
+                if (pair + step < n_pairs) stage(pair + step);
+                cp_async_commit();
+            }
+            if (!SPLIT) {
+#pragma unroll
+                for (int t = 0; t < N1; ++t) v[t] = make_float2(fmaf(v[t].x, im, -1.0f), has_b ? fmaf(v[t].y, im, -1.0f) : 0.0f);
+            } else if (h == 0) {
+#pragma unroll
+                for (int t = 0; t < N1; ++t) v[t] = make_float2(fmaf(v[t].x, im, -2.0f), has_b ? fmaf(v[t].y, im, -2.0f) : 0.0f);
+            } else {
+#pragma unroll
+                for (int t = 0; t < N1; ++t) v[t] = cmul(v[t], tw2[n2 + N2 * t]);   // the -1 cancels; tw2 carries inv_mean
+            }
+            dft_regs64<N1, true>(v);
+            ex[n2] = v[0];                               // k1 = 0: twiddle 1
+#pragma unroll
+            for (int k1 = 1; k1 < N1; ++k1) ex[k1 * XS + n2] = cmul(v[bitrev<N1>(k1)], tw[k1 * N2 + n2]);
+        }
+        __syncwarp();
+#pragma unroll
+        for (int s = 0; s < S2; ++s) {                   // pass 2 for output residue k1 = lane + 32 s
+            const float2 *row = ex + (lane + 32 * s) * XS;
+            float2 u[N2];
+#pragma unroll
+            for (int t = 0; t < N2; ++t) u[t] = row[t];
+            dft_regs64<N2, true>(u);
+#pragma unroll
+            for (int t = 0; t < N2; ++t) acc[s][t] = fmaf(u[t].x, u[t].x, fmaf(u[t].y, u[t].y, acc[s][t]));
+        }
+        __syncwarp();                                    // the exchange buffer is free again
+        if (++since == PW_FLUSH) { flush(); since = 0; }
+    }
+    flush();
+    lya_publish_last_cta(a.acc, a.n_acc, a.host, a.ticket);
+}
+
 }  // namespace
 
 extern "C" lya_status lya_flux_power_rows(lya_ctx *ctx, size_t n_rows, int32_t n_pix, double dv_kms,
@@ -279,17 +468,31 @@ extern "C" lya_status lya_flux_power_rows(lya_ctx *ctx, size_t n_rows, int32_t n
                                     {4, 4, 3}, {4, 4, 4}, {4, 4, 3, 2}};
     for (int i = 0; i < 4 && plan[log2n][i]; ++i) a.radix[a.n_pass++] = 1 << plan[log2n][i];
     const int npad = n_pix + (n_pix >> 4) + 1;
-    const size_t smem = (size_t)(nk + 1) * sizeof(double) + 2 * (size_t)npad * sizeof(float2) + (size_t)(n_pix / 2) * sizeof(float2);
+    size_t smem = (size_t)(nk + 1) * sizeof(double) + 2 * (size_t)npad * sizeof(float2) + (size_t)(n_pix / 2) * sizeof(float2);
     int threads = n_pix / 8;
     threads = threads < 32 ? 32 : (threads > 256 ? 256 : threads);
     void (*kern)(const PowArgs) = n_pix == 256 ? flux_power_kernel<256> : n_pix == 512 ? flux_power_kernel<512>
                                 : n_pix == 1024 ? flux_power_kernel<1024> : n_pix == 2048 ? flux_power_kernel<2048>
                                 : n_pix == 4096 ? flux_power_kernel<4096> : flux_power_kernel<0>;
+    // rows of 1024 / 2048 pixels: one warp per row pair (flux_power_warp_kernel); 2048 needs 16-byte aligned flux
+    int warp_kernel = 0;
+    const bool al16 = ((uintptr_t)flux & 15) == 0;
+    if (n_pix == 1024) {
+        kern = al16 ? flux_power_warp_kernel<32, 32, false, true, 4, 3> : flux_power_warp_kernel<32, 32, false, false, 4, 3>;
+        warp_kernel = 4;
+        threads = 4 * 32;
+        smem = (size_t)1024 * sizeof(float2) + 4 * (size_t)32 * 33 * sizeof(float2) + (al16 ? 4 * 2 * (size_t)1024 * sizeof(float) : 0);
+    } else if (n_pix == 2048 && al16) {                    // 6 teams of two warps, one CTA per SM
+        kern = flux_power_warp_kernel<32, 32, true, true, 12, 1>;
+        warp_kernel = 6;
+        smem = 2 * (size_t)1024 * sizeof(float2) + 12 * (size_t)32 * 33 * sizeof(float2) + 6 * 2 * (size_t)2048 * sizeof(float);
+        threads = 12 * 32;
+    }
     int per_sm = 0;
     lya_status st = lya_kernel_occupancy(ctx, (const void *)kern, threads, smem, &per_sm);
     if (st != LYA_OK) return st;
     if (per_sm < 1) return lya_fail(ctx, LYA_ECUDA, "flux_power_kernel: zero occupancy");
-    const size_t n_pairs = (n_rows + 1) / 2, cap = (size_t)ctx->sm_count * per_sm;
+    const size_t n_pairs = warp_kernel ? ((n_rows + 1) / 2 + warp_kernel - 1) / warp_kernel : (n_rows + 1) / 2, cap = (size_t)ctx->sm_count * per_sm;
     st = lya_stats_begin(ctx, n_acc);
     if (st != LYA_OK) return st;
     kern<<<(int)(n_pairs < cap ? n_pairs : cap), threads, smem, ctx->stream>>>(a);   // the last CTA writes the totals to a.host
