@@ -429,6 +429,17 @@ __global__ void __launch_bounds__(T) observe_rows_lean8_kernel(const ObsArgs a, 
             s_b[m] = e;
         }
     const unsigned sc_addr = smem_addr(s_c), sb_addr = smem_addr(s_b) + 16u * tid;
+    // three-pixel bins: a thread serves the SAME bins tid + k T in every row, so their table entries live in registers
+    // (the per-bin LDS.128 was 2.8 of the ~13 shared-memory wavefronts per 32 pixels; ncu: shared-memory pipe 74 %)
+    int4 eb[OBS_NBR8];
+#pragma unroll
+    for (int k = 0; k < OBS_NBR8; ++k) {
+        eb[k] = make_int4(0, 0, 0, 0);
+        if (a.bins3 && tid + k * T < nb) {
+            eb[k] = a.bins[tid + k * T];
+            eb[k].x *= 4;
+        }
+    }
 
     const bool own = 8 * tid < n;                        // this thread owns pixels 8 tid .. 8 tid + 7
     const bool has_halo = tid < a.L;
@@ -498,7 +509,7 @@ __global__ void __launch_bounds__(T) observe_rows_lean8_kernel(const ObsArgs a, 
 #pragma unroll
             for (int k = 0; k < OBS_NBR8; ++k) {
                 if (tid + k * T < nb) {
-                    const int4 e = lds_v4(sb_addr + 16u * k * T);
+                    const int4 e = eb[k];
                     const unsigned ca = sc_addr + (unsigned)e.x;
                     float v = fmaf(__int_as_float(e.w), lds_f32(ca + 8), fmaf(__int_as_float(e.z), lds_f32(ca + 4), __int_as_float(e.y) * lds_f32(ca)));
                     if (nz) v = fmaf(nzr[k], inv_snr, v);
