@@ -151,6 +151,42 @@ def test_flux_power_lengths_and_errors(ctx, obs, n):
         ctx.flux_power_rows(F[:, : n - 1].contiguous(), 2.0, 0.5)   # not a power of two
 
 
+@pytest.mark.parametrize("n", [256, 512, 1024, 2048, 4096])
+@pytest.mark.parametrize("n_rows", [1, 7, 22])
+def test_flux_power_kernels_of_the_config_row_lengths(ctx, obs, n, n_rows):
+    """Every compile-time plan (256 ... 4096) and both warp-per-transform kernels (1024: one warp per row pair; 2048: a
+    team of two warps per pair) against the oracle's direct DFT: odd row counts (a last pair with no second row), fewer
+    pairs than warps, and a 4-byte-aligned view (the kernels without cp.async staging)."""
+    rng = np.random.default_rng(1000 * n + n_rows)
+    host = rng.uniform(0.0, 1.0, (n_rows, n)).astype(np.float32)
+    host[0] = 0.8                                                    # a constant row: only the k = 0 mode
+    ref = obs.flux_power(host, 3.5, 0.6)
+    buf = torch.empty(n_rows * n + 4, device="cuda")
+    for off in (0, 1):                                               # 16-byte aligned, then 4-byte aligned only
+        F = buf[off: off + n_rows * n].view(n_rows, n)
+        F.copy_(torch.from_numpy(host))
+        assert (F.data_ptr() % 16 == 0) == (off == 0)
+        P = ctx.flux_power_rows(F, 3.5, 0.6)
+        assert np.all(np.abs(P - ref) <= 1e-4 * ref + 1e-9 * ref.max()), (off, np.abs(P / ref - 1).max())
+
+
+@pytest.mark.parametrize("n", [1024, 2048])
+def test_flux_power_at_full_size_by_tiling(ctx, obs, n):
+    """Configs 4 and 5 at the size bench.py times (2^30 pixels: about 295 row pairs per warp, so the fp32 accumulators'
+    flush every 256 pairs is taken): the mean over rows of a block of rows repeated many times is the block's own, which
+    the oracle can compute."""
+    block, reps = 32, (1 << 30) // (32 * n)
+    rng = np.random.default_rng(n)
+    host = np.exp(-rng.lognormal(-1.0, 1.5, (block, n))).astype(np.float32)      # F = exp(-tau), heavy-tailed tau
+    fbar = float(host.astype(np.float64).mean())
+    ref = obs.flux_power(host, 51.5, fbar)
+    F = torch.from_numpy(host).cuda().repeat(reps, 1)
+    assert F.shape == (block * reps, n)
+    P = ctx.flux_power_rows(F, 51.5, fbar)
+    assert np.all(np.abs(P - ref) <= 1e-4 * ref + 1e-9 * ref.max()), np.abs(P / ref - 1).max()
+    assert np.allclose(P, ctx.flux_power_rows(F, 51.5, fbar), rtol=1e-12)          # atomics: order-dependent only in the last bits
+
+
 def test_flux_with_pdf_equals_the_two_calls(ctx, flux_rows):
     """S5 and the PDF fused in one pass: F and the counts are bit-identical to lya_flux + lya_flux_pdf."""
     w = WORKLOADS[2]
