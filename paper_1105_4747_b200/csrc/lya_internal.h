@@ -54,6 +54,16 @@ struct lya_ctx {
 // (ticket d_sched[4]) copies the totals to the mapped pinned mirror and leaves d_stats and the ticket zeroed for the next
 // call, so a call is one launch and one synchronisation: no memset, no copy to enqueue.
 lya_status lya_stats_begin(lya_ctx *ctx, size_t n_doubles);
+// replicas of an n-entry accumulator inside d_stats (a CTA adds into replica blockIdx.x % reps; the last CTA sums them).
+// They matter when the launch is short: all CTAs finish together and their atomics to the same n addresses serialise
+// (256^3: 25 of the flux-PDF kernel's 47 us).  On long launches the CTAs drift apart and the replicas only add work to
+// the last CTA, so inputs beyond 2^28 pixels take one copy; max_reps bounds the last CTA's n * reps loads.
+static inline int lya_stats_replicas(size_t n, size_t n_pixels, int max_reps)
+{
+    size_t r = n ? LYA_STATS_DOUBLES / n : 1;
+    if (n_pixels > ((size_t)1 << 28)) return 1;
+    return (int)(r < 1 ? 1 : (r > (size_t)max_reps ? (size_t)max_reps : r));
+}
 lya_status lya_stats_end(lya_ctx *ctx);                  // synchronises; the results are in h_pinned + LYA_PINNED_STATS
 
 static inline lya_status lya_fail(lya_ctx *ctx, lya_status s, const char *msg)

@@ -385,7 +385,7 @@ constexpr int FPDF_THREADS = 128;
 __global__ void __launch_bounds__(FPDF_THREADS) flux_pdf_fused_kernel(const float *tau, size_t n, Trial tr, float *flux,
                                                                       const __grid_constant__ PdfEdges edges,
                                                                       unsigned long long *counts, unsigned long long *host,
-                                                                      unsigned int *ticket)
+                                                                      unsigned int *ticket, int reps)
 {
     extern __shared__ unsigned int hist[];               // [n_bins][FPDF_THREADS], then n_bins + 1 thresholds
     const int n_bins = edges.n_bins;
@@ -427,9 +427,9 @@ __global__ void __launch_bounds__(FPDF_THREADS) flux_pdf_fused_kernel(const floa
         for (int t = lane; t < FPDF_THREADS; t += 32) sum += hist[b * FPDF_THREADS + t];
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o);
-        if (lane == 0 && sum) atomicAdd(counts + b, (unsigned long long)sum);
+        if (lane == 0 && sum) atomicAdd(counts + (blockIdx.x % reps) * n_bins + b, (unsigned long long)sum);
     }
-    lya_publish_last_cta(counts, n_bins, host, ticket);
+    lya_publish_last_cta(counts, n_bins, host, ticket, reps);
 }
 
 // float4 in the subsample "every `every`-th chunk of 256 float4 of the aligned body of tau" (0: no subsample)
@@ -586,7 +586,7 @@ lya_status lya_run_flux_with_pdf(lya_ctx *ctx, const float *tau, size_t n, doubl
         if (st != LYA_OK) return st;
         // the last CTA to finish writes the totals straight to the pinned mirror and re-zeroes the device counters
         flux_pdf_fused_kernel<<<(int)(want < cap ? want : cap), FPDF_THREADS, smem, ctx->stream>>>(
-            tau, n, make_trial(a), flux, edges, d_counts, host, ctx->d_sched + 4);
+            tau, n, make_trial(a), flux, edges, d_counts, host, ctx->d_sched + 4, lya_stats_replicas(n_bins, n, 16));
         ctx->launches++;
         st = lya_stats_end(ctx);
         if (st != LYA_OK) return st;

@@ -547,7 +547,7 @@ constexpr int PDF_THREADS = 128;
 __global__ void __launch_bounds__(PDF_THREADS) flux_pdf_kernel(const float *__restrict__ flux, size_t n,
                                                                const __grid_constant__ PdfEdges edges,
                                                                unsigned long long *counts, unsigned long long *host,
-                                                               unsigned int *ticket)
+                                                               unsigned int *ticket, int reps)
 {
     extern __shared__ unsigned int hist[];               // [n_bins][PDF_THREADS], then n_bins + 1 thresholds
     const int n_bins = edges.n_bins;
@@ -578,9 +578,9 @@ __global__ void __launch_bounds__(PDF_THREADS) flux_pdf_kernel(const float *__re
         for (int t = lane; t < PDF_THREADS; t += 32) s += hist[b * PDF_THREADS + t];
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
-        if (lane == 0 && s) atomicAdd(counts + b, (unsigned long long)s);
+        if (lane == 0 && s) atomicAdd(counts + (blockIdx.x % reps) * n_bins + b, (unsigned long long)s);
     }
-    lya_publish_last_cta(counts, n_bins, host, ticket);
+    lya_publish_last_cta(counts, n_bins, host, ticket, reps);
 }
 
 }  // namespace
@@ -821,7 +821,7 @@ extern "C" lya_status lya_flux_pdf(lya_ctx *ctx, const float *flux, size_t n, in
         if (st != LYA_OK) return st;
         // the last CTA to finish writes the totals straight to the pinned mirror and re-zeroes the device counters
         flux_pdf_kernel<<<(int)(want < cap ? want : cap), PDF_THREADS, smem, ctx->stream>>>(flux, n, edges, d_counts, host,
-                                                                                           ctx->d_sched + 4);
+                                                                                           ctx->d_sched + 4, lya_stats_replicas(n_bins, n, 16));
         ctx->launches++;
         st = lya_stats_end(ctx);
         if (st != LYA_OK) return st;

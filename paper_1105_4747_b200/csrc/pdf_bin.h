@@ -58,11 +58,13 @@ __device__ __forceinline__ int lya_pdf_bin(float f, const float *s_thr, int n_bi
     return b;
 }
 
-// Epilogue of the statistics kernels, called by every thread of every CTA after the CTA's own atomics into acc[0 .. n):
-// the last CTA to arrive (ticket) moves the totals to `host` (mapped pinned memory) and leaves acc and the ticket zeroed
-// for the next launch.  T is unsigned long long (counts) or double (power sums).
+// Epilogue of the statistics kernels, called by every thread of every CTA after the CTA's own atomics into ITS replica
+// acc[(blockIdx.x % reps) * n + (0 .. n)): the last CTA to arrive (ticket) moves the totals over the replicas to `host`
+// (mapped pinned memory) and leaves acc and the ticket zeroed for the next launch.  T is unsigned long long (counts) or
+// double (power sums).  Replicas exist because all CTAs of a launch finish together: 2368 CTAs adding into the same 21
+// addresses took ~25 us of same-address atomic serialisation on a 256^3 grid (the kernel: 47 us for 64 MiB).
 template <typename T>
-__device__ __forceinline__ void lya_publish_last_cta(T *acc, int n, T *host, unsigned int *ticket)
+__device__ __noinline__ void lya_publish_last_cta(T *acc, int n, T *host, unsigned int *ticket, int reps)
 {
     __shared__ int s_last;
     __threadfence();                                     // this thread's atomics are visible device-wide
@@ -71,10 +73,16 @@ __device__ __forceinline__ void lya_publish_last_cta(T *acc, int n, T *host, uns
     __syncthreads();
     if (!s_last) return;
     __threadfence();
+    // loads first (independent: eight in flight per thread; more would cost every kernel that inlines this registers),
+    // zeroing after
     for (int i = threadIdx.x; i < n; i += blockDim.x) {
-        host[i] = __ldcg(acc + i);
-        acc[i] = (T)0;
+        T sum = (T)0;
+#pragma unroll 8
+        for (int r = 0; r < reps; ++r) sum += __ldcg(acc + (size_t)r * n + i);
+        host[i] = sum;
     }
+    __syncthreads();                                     // (s_last is uniform over the CTA) every replica has been read
+    for (int i = threadIdx.x; i < n * reps; i += blockDim.x) acc[i] = (T)0;
     if (threadIdx.x == 0) *ticket = 0u;
 }
 #endif

@@ -33,6 +33,7 @@ struct PowArgs {
     double      *host;         // mapped pinned mirror: the last CTA to finish writes the totals there
     unsigned int *ticket;
     int          n_acc;
+    int          reps;         // replicas of the n_acc accumulators (lya_stats_replicas): CTA b adds into replica b % reps
 };
 
 __device__ __forceinline__ float2 cmul(float2 a, float2 b) { return make_float2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
@@ -169,7 +170,7 @@ __host__ __device__ constexpr int plan_radix(int n, int i)
          : n == 2048 ? (i < 2 ? 16 : (i == 2 ? 8 : 0)) : n == 4096 ? (i < 3 ? 16 : 0) : 0;
 }
 
-template <int N_CT>
+template <int N_CT, bool REP = false>                    // REP: replicated accumulators (short launches only; see lya_stats_replicas)
 __global__ void __launch_bounds__(256) flux_power_kernel(const PowArgs a)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -244,14 +245,14 @@ __global__ void __launch_bounds__(256) flux_power_kernel(const PowArgs a)
     if constexpr (N_CT > 0) {                              // output k = j + t ns of the last pass, j = tid < N / RL
         if (tid < N_CT / RL)
 #pragma unroll
-            for (int t = 0; t < RL; ++t) atomicAdd(a.acc + tid + t * (N_CT / RL), pacc[t]);
-        lya_publish_last_cta(a.acc, a.n_acc, a.host, a.ticket);
+            for (int t = 0; t < RL; ++t) atomicAdd(a.acc + (REP ? (blockIdx.x % a.reps) * a.n_acc : 0) + tid + t * (N_CT / RL), pacc[t]);
+        lya_publish_last_cta(a.acc, a.n_acc, a.host, a.ticket, REP ? a.reps : 1);
         return;
     }
     __syncthreads();
     for (int m = tid; m <= nh; m += T)
-        if (pw[m] != 0.0) atomicAdd(a.acc + m, pw[m]);
-    lya_publish_last_cta(a.acc, a.n_acc, a.host, a.ticket);
+        if (pw[m] != 0.0) atomicAdd(a.acc + (REP ? (blockIdx.x % a.reps) * a.n_acc : 0) + m, pw[m]);
+    lya_publish_last_cta(a.acc, a.n_acc, a.host, a.ticket, REP ? a.reps : 1);
 }
 
 // ---- one WARP per row pair, two passes, no CTA barrier (rows of N = N1 * N2 pixels, N2 = 32 or 64) --------------------
@@ -361,12 +362,13 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) flux_power_warp_kernel(const
     for (int s = 0; s < S2; ++s)
 #pragma unroll
         for (int t = 0; t < N2; ++t) acc[s][t] = 0.0f;
+    double *mine = a.acc + (blockIdx.x % a.reps) * a.n_acc;   // this CTA's replica of the accumulators
     auto flush = [&]() {                                 // fp32 accumulators -> the device's doubles
 #pragma unroll
         for (int s = 0; s < S2; ++s)
 #pragma unroll
             for (int t = 0; t < N2; ++t) {               // transform output k' = k1 + N1 k2 is Z(H k' + h)
-                atomicAdd(a.acc + H * ((lane + 32 * s) + N1 * t) + h, (double)acc[s][bitrev<N2>(t)]);
+                atomicAdd(mine + H * ((lane + 32 * s) + N1 * t) + h, (double)acc[s][bitrev<N2>(t)]);
                 acc[s][bitrev<N2>(t)] = 0.0f;
             }
     };
@@ -437,7 +439,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) flux_power_warp_kernel(const
         if (++since == PW_FLUSH) { flush(); since = 0; }
     }
     flush();
-    lya_publish_last_cta(a.acc, a.n_acc, a.host, a.ticket);
+    lya_publish_last_cta(a.acc, a.n_acc, a.host, a.ticket, a.reps);
 }
 
 }  // namespace
@@ -462,7 +464,7 @@ extern "C" lya_status lya_flux_power_rows(lya_ctx *ctx, size_t n_rows, int32_t n
     memset(&a, 0, sizeof(a));
     a.flux = flux; a.n_rows = n_rows; a.n = n_pix; a.log2n = log2n;
     a.inv_mean = (float)(1.0 / mean_flux); a.acc = ctx->d_stats;
-    a.host = ctx->h_pinned + LYA_PINNED_STATS; a.ticket = ctx->d_sched + 4; a.n_acc = n_acc;
+    a.host = ctx->h_pinned + LYA_PINNED_STATS; a.ticket = ctx->d_sched + 4; a.n_acc = n_acc; a.reps = n_rows * (size_t)n_pix <= ((size_t)1 << 25) ? lya_stats_replicas(n_acc, n_rows * (size_t)n_pix, 4) : 1;   // measured: 512^3 is slower with replicas
     // radices of the passes (log2: 4, 3, 2), largest first
     static const int plan[14][4] = {{0}, {0}, {0}, {3}, {4}, {3, 2}, {3, 3}, {4, 3}, {4, 4}, {3, 3, 3}, {4, 3, 3},
                                     {4, 4, 3}, {4, 4, 4}, {4, 4, 3, 2}};
@@ -474,6 +476,10 @@ extern "C" lya_status lya_flux_power_rows(lya_ctx *ctx, size_t n_rows, int32_t n
     void (*kern)(const PowArgs) = n_pix == 256 ? flux_power_kernel<256> : n_pix == 512 ? flux_power_kernel<512>
                                 : n_pix == 1024 ? flux_power_kernel<1024> : n_pix == 2048 ? flux_power_kernel<2048>
                                 : n_pix == 4096 ? flux_power_kernel<4096> : flux_power_kernel<0>;
+    if (a.reps > 1)                                        // short launch: replicated accumulators
+        kern = n_pix == 256 ? flux_power_kernel<256, true> : n_pix == 512 ? flux_power_kernel<512, true>
+             : n_pix == 1024 ? flux_power_kernel<1024, true> : n_pix == 2048 ? flux_power_kernel<2048, true>
+             : n_pix == 4096 ? flux_power_kernel<4096, true> : flux_power_kernel<0, true>;
     // rows of 1024 / 2048 pixels: one warp per row pair (flux_power_warp_kernel); 2048 needs 16-byte aligned flux
     int warp_kernel = 0;
     const bool al16 = ((uintptr_t)flux & 15) == 0;
