@@ -521,9 +521,23 @@ def cpu_baseline(w, d, vv, budget_s=12.0) -> dict:
     t0 = time.perf_counter()
     _oracle_sample(orc, w, d[:rows], vv[:rows])
     dt = time.perf_counter() - t0
-    return {"value": rows * float(n) ** 2 / dt, "unit": UNIT, "cores": orc.threads(), "kind": "oracle",
+    rate = rows * float(n) ** 2 / dt
+    return {"value": rate, "unit": UNIT, "cores": orc.threads(), "kind": "oracle",
             "sample": f"first {rows} of {n * n} sightlines of {w.name}, whole path S1..S5 in double, "
-                      f"plain mode, {dt:.1f} s"}
+                      f"plain mode, {dt:.1f} s",
+            "cpu_model": _cpu_model(),
+            "extrapolated_full_grid_s": float(n) ** 4 * len(w.axes) / rate}     # labelled as an extrapolation
+
+
+def _cpu_model() -> str:
+    try:
+        with open("/proc/cpuinfo") as fh:
+            for line in fh:
+                if line.startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
 
 
 def bench_reference(args) -> dict:
