@@ -142,10 +142,19 @@ def bench_ours(args) -> dict:
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    # LYA_BENCH_BACKEND=gloo with LYA_BENCH_ONE_DEVICE=1 exists for ONE purpose: tests/test_bench_contract.py runs the
+    # N > 1 code path (per-rank slabs, global A, barriers, max over ranks) with two ranks on a one-GPU box.  Its numbers
+    # are not measurements (the ranks time-slice one GPU) and the line says so in config.parallelism.
+    backend = os.environ.get("LYA_BENCH_BACKEND", "nccl")
+    if os.environ.get("LYA_BENCH_ONE_DEVICE") == "1":
+        local = 0
     if world > 1:
-        os.environ.setdefault("NCCL_DEBUG", "INFO")            # communicator lines stay on: the driver counts ranks
-        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if backend == "nccl":
+            os.environ.setdefault("NCCL_DEBUG", "INFO")        # communicator lines stay on: the driver counts ranks
+            os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group(backend)
     torch.cuda.set_device(local)
     if args.cfg is None:
         args.cfg = default_cfg()
@@ -449,7 +458,9 @@ def bench_ours(args) -> dict:
                    "pixels_per_sightline": n, "axes": list(w.axes), "f_target": w.f_target, "slab_nz": slab_nz,
                    "l2": "256 MiB memset between steps (outside the event spans); working set %d MiB" %
                          (6 * 4 * n_cells >> 20),
-                   "parallelism": "z-slabs per rank; S4 all-reduce of 5 doubles per pass" if world > 1 else "1 GPU"},
+                   "parallelism": ("z-slabs per rank; S4 all-reduce of 5 doubles per pass"
+                                   + ("" if backend == "nccl" else f" [TEST RUN over {backend}: ranks may share a GPU, not a measurement]"))
+                   if world > 1 else "1 GPU"},
         "sightline_pixels_per_s": pix_per_step / (ms_per_step * 1e-3),
         "tau_kernel_pixels_per_s": float(slab_cells) / (k_ms["tau"] * 1e-3),
         "A": results["A"], "mean_flux": results["f"], "normalize_passes": passes,

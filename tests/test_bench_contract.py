@@ -38,6 +38,26 @@ def test_bench_line_has_the_contract_keys():
     assert abs(d["mean_flux"] - 0.80) < 1e-6
 
 
+@pytest.mark.gpu
+def test_two_rank_bench_path_on_one_gpu():
+    """The N > 1 path of bench.py (per-rank slabs of one taller grid, ONE global A through the sharded S4, barriers, max
+    over ranks, rank 0 alone prints) with two gloo ranks time-slicing GPU 0: the code path, not a measurement."""
+    env = dict(os.environ, LYA_BENCH_BACKEND="gloo", LYA_BENCH_ONE_DEVICE="1", MASTER_ADDR="127.0.0.1")
+    r = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+                        "--master-addr", "127.0.0.1", "--master-port", "29541", os.path.join(ROOT, "bench.py"),
+                        "--gpus", "2", "--cfg", "1", "--steps", "3", "--warmup", "3"],
+                       capture_output=True, text=True, cwd=ROOT, timeout=900, env=env)
+    assert r.returncode == 0, (r.stdout[-1500:], r.stderr[-3000:])
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1                                              # rank 0 alone prints
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["scaling"] == "weak" and d["config"]["grid"] == [64, 64, 128]
+    assert d["config"]["sightlines"] == 2 * 64 * 64 and "all-reduce" in d["config"]["parallelism"]
+    assert d["value"] == pytest.approx(2 * 64.0 ** 4 / (d["ms_per_step"] * 1e-3), rel=1e-9)
+    assert abs(d["mean_flux"] - 0.80) < 1e-6                            # the global A reaches the target over BOTH slabs
+    assert d["e2e"]["value"] > 0 and "one global A" in d["e2e"]["note"]
+
+
 def test_reference_arm_line():                                          # no GPU needed: the oracle on the host cores
     d = _run("--impl", "reference", "--cfg", "1", "--steps", "1", "--warmup", "0")
     assert d["impl"] == "reference" and d["metric"] == "tau_pixel_pair_evals_per_s" and d["gpu_launches"] == 0
