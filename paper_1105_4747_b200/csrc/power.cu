@@ -255,7 +255,7 @@ __global__ void __launch_bounds__(256) flux_power_kernel(const PowArgs a)
     lya_publish_last_cta(a.acc, a.n_acc, a.host, a.ticket, REP ? a.reps : 1);
 }
 
-// ---- one WARP per row pair, two passes, no CTA barrier (rows of N = N1 * N2 pixels, N2 = 32 or 64) --------------------
+// ---- one WARP per row pair, two passes, no CTA barrier (N1 x N2 points, multiples of 32; instantiated: 32 x 32) --------
 // ncu on the kernel above (1024-pixel rows): issue slots 55 % busy, barrier stall 5.0 and long-scoreboard 3.0 cycles per
 // issued instruction, half of the threads idle in the radix-16 passes; prefetching the next pair with cp.async changed
 // nothing (1.30 -> 1.26 ms), so the limit is the pass -> barrier -> pass chain itself.  Here a warp owns a whole
@@ -264,9 +264,10 @@ __global__ void __launch_bounds__(256) flux_power_kernel(const PowArgs a)
 //           DFT in registers, the twiddles W_N^(n2 k1) from a per-CTA table [k1][n2], the result to the warp's private
 //           exchange buffer [k1][n2] (row stride N2 + 1 float2: conflict-free both ways);
 //   pass 2  lane holds Y[n2][k1], n2 < N2, for its k1 = lane (+ 32): an N2-point DFT in registers, |Z(k)|^2 added to
-//           fp32 accumulators in registers -- flushed to the double device accumulators every 256 pairs and at the end
-//           (through a per-CTA sum in shared memory), so an fp32 accumulator never holds more than 256 terms.
-// Only __syncwarp() orders the two passes; every load of a pair (64 per lane at N = 1024) is in flight at once.
+//           fp32 accumulators in registers -- flushed to the double device accumulators (atomicAdd) every 256 pairs and
+//           at the end, so an fp32 accumulator never holds more than 256 terms.
+// Only __syncwarp() orders the two passes; without the cp.async stage below every load of a pair (64 per lane at
+// N = 1024) is in flight at once.
 __device__ __forceinline__ unsigned pw_smem_addr(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void cp_async16(unsigned dst, const void *src)
 {
