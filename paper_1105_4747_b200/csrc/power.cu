@@ -268,13 +268,33 @@ __global__ void __launch_bounds__(256) flux_power_kernel(const PowArgs a)
 //           at the end, so an fp32 accumulator never holds more than 256 terms.
 // Only __syncwarp() orders the two passes; without the cp.async stage below every load of a pair (64 per lane at
 // N = 1024) is in flight at once.
+// mbarrier + 1-D bulk copy (TMA unit; SASS: SYNCS, UBLKCP): one lane moves a whole row pair, 8 N bytes, per instruction
 __device__ __forceinline__ unsigned pw_smem_addr(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void cp_async16(unsigned dst, const void *src)
+__device__ __forceinline__ void mbar_init(unsigned long long *bar, unsigned count)
 {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(pw_smem_addr(bar)), "r"(count) : "memory");
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(pw_smem_addr(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long *bar, unsigned parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_%=:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra DONE_%=;\n"
+        "bra WAIT_%=;\n"
+        "DONE_%=:\n"
+        "}\n" ::"r"(pw_smem_addr(bar)), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(void *dst, const void *src, unsigned bytes, unsigned long long *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(pw_smem_addr(dst)), "l"(src), "r"(bytes), "r"(pw_smem_addr(bar)) : "memory");
+}
 
 template <int R, bool PACK>
 __device__ __forceinline__ void dft_regs64(float2 (&v)[R])   // as dft_regs, twiddles W_64^q (R <= 64)
@@ -320,7 +340,8 @@ constexpr int PW_FLUSH = 256;                            // pairs between two fl
 // shares one staged pair, warp h of the team takes half h, and only two 64-thread named barriers per pair tie them
 // together (pair landed / pair read).  A serial version (one warp, both halves) fits only 8 warps per SM next to its
 // 16 KiB stage buffers and measured 1.40 ms on 2048-pixel rows, no better than the CTA-per-pair kernel.
-// STAGE (16-byte aligned flux; required by SPLIT): the NEXT pair streams into the stage buffer (cp.async, 8 N bytes)
+// STAGE (16-byte aligned flux; required by SPLIT): the NEXT pair streams into the stage buffer (ONE cp.async.bulk of 8 N
+// bytes issued by one lane, completion counted on the unit's mbarrier)
 // while the current one is transformed, so no warp waits out an HBM latency (1024-pixel rows: 0.99 -> 0.92 ms).
 template <int N1, int N2, bool SPLIT, bool STAGE, int WARPS, int MINB>
 __global__ void __launch_bounds__(WARPS * 32, MINB) flux_power_warp_kernel(const PowArgs a)
@@ -337,12 +358,19 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) flux_power_warp_kernel(const
     float2 *tw2 = tw + NT;                               // SPLIT: [NT] inv_mean W_N^m
     float2 *ex  = tw2 + (SPLIT ? NT : 0) + warp * (N1 * XS);
     float *stg  = reinterpret_cast<float *>(tw2 + (SPLIT ? NT : 0) + WARPS * (N1 * XS)) + unit * (2 * N);
+    unsigned long long *mbar = reinterpret_cast<unsigned long long *>(
+        reinterpret_cast<float *>(tw2 + (SPLIT ? NT : 0) + WARPS * (N1 * XS)) + UNITS * (2 * N)) + unit;
+    const bool issuer = STAGE && lane == 0 && h == 0;    // the one thread of a unit that talks to the copy unit
     auto stage = [&](size_t pair) {                      // rows 2 pair (and 2 pair + 1 if it exists): contiguous floats
-        const float *src = a.flux + (2 * pair) * (size_t)N;
-        const int chunks = (2 * pair + 1 < a.n_rows ? 2 * N : N) >> 2;
-        const unsigned d = pw_smem_addr(stg);
-        for (int c = lane + 32 * h; c < chunks; c += 32 * H) cp_async16(d + 16u * c, src + 4 * c);
+        const unsigned bytes = (2 * pair + 1 < a.n_rows ? 2 * N : N) * (unsigned)sizeof(float);
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the buffer was read through the generic proxy
+        mbar_expect_tx(mbar, bytes);
+        bulk_g2s(stg, a.flux + (2 * pair) * (size_t)N, bytes, mbar);
     };
+    if (issuer) {
+        mbar_init(mbar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
     auto unit_sync = [&]() {                             // the warps that share a stage buffer
         if (SPLIT) asm volatile("bar.sync %0, 64;" ::"r"(unit + 1) : "memory");
         else       __syncwarp();
@@ -377,16 +405,14 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) flux_power_warp_kernel(const
     const float im = a.inv_mean;
     int since = 0;
     size_t pair = (size_t)blockIdx.x * UNITS + unit;
-    if (STAGE) {
-        if (pair < n_pairs) stage(pair);
-        cp_async_commit();
-    }
+    if (issuer && pair < n_pairs) stage(pair);           // (the mbarrier was initialised before the __syncthreads above)
+    unsigned phase = 0;
     for (; pair < n_pairs; pair += step) {
         const float *ra = STAGE ? stg : a.flux + (2 * pair) * (size_t)N, *rb = ra + N;
         const bool has_b = 2 * pair + 1 < a.n_rows;
         if (STAGE) {
-            cp_async_wait_all();
-            unit_sync();                                 // every lane's chunks of this pair have landed
+            mbar_wait(mbar, phase);                      // this pair has landed (complete_tx on the unit's mbarrier)
+            phase ^= 1u;
         }
 #pragma unroll
         for (int s = 0; s < S1; ++s) {                   // pass 1 for residue n2 = lane + 32 s: points m = n2 + N2 t
@@ -407,8 +433,7 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) flux_power_warp_kernel(const
             }
             if (STAGE && s == S1 - 1) {                  // the stage buffer has been read: fetch the next pair into it
                 unit_sync();
-                if (pair + step < n_pairs) stage(pair + step);
-                cp_async_commit();
+                if (issuer && pair + step < n_pairs) stage(pair + step);
             }
             if (!SPLIT) {
 #pragma unroll
@@ -488,11 +513,11 @@ extern "C" lya_status lya_flux_power_rows(lya_ctx *ctx, size_t n_rows, int32_t n
         kern = al16 ? flux_power_warp_kernel<32, 32, false, true, 4, 3> : flux_power_warp_kernel<32, 32, false, false, 4, 3>;
         warp_kernel = 4;
         threads = 4 * 32;
-        smem = (size_t)1024 * sizeof(float2) + 4 * (size_t)32 * 33 * sizeof(float2) + (al16 ? 4 * 2 * (size_t)1024 * sizeof(float) : 0);
+        smem = (size_t)1024 * sizeof(float2) + 4 * (size_t)32 * 33 * sizeof(float2) + (al16 ? 4 * 2 * (size_t)1024 * sizeof(float) : 0) + 4 * sizeof(unsigned long long);
     } else if (n_pix == 2048 && al16) {                    // 6 teams of two warps, one CTA per SM
         kern = flux_power_warp_kernel<32, 32, true, true, 12, 1>;
         warp_kernel = 6;
-        smem = 2 * (size_t)1024 * sizeof(float2) + 12 * (size_t)32 * 33 * sizeof(float2) + 6 * 2 * (size_t)2048 * sizeof(float);
+        smem = 2 * (size_t)1024 * sizeof(float2) + 12 * (size_t)32 * 33 * sizeof(float2) + 6 * 2 * (size_t)2048 * sizeof(float) + 6 * sizeof(unsigned long long);
         threads = 12 * 32;
     }
     int per_sm = 0;
