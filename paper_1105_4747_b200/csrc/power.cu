@@ -17,7 +17,8 @@
 // memory and read the pairs (m, N - m) out (accumulated in double per CTA).
 // Rows of 1024 and 2048 pixels (configs 4 and 5) take flux_power_warp_kernel instead: ONE WARP per transform (32 x 32
 // in two register passes, 2048 as two such transforms by a radix-2 split shared by a team of two warps), the next row
-// pair prefetched by cp.async, no CTA barrier in the loop: 1.30 -> 0.91 ms on 1024^3, 1.36 -> 1.04 ms on 2048-pixel rows.
+// pair prefetched by one cp.async.bulk, no CTA barrier in the loop: 1.30 -> 0.88 ms on 1024^3, 1.36 -> 0.97 ms on
+// 2048-pixel rows.
 #include "lya_internal.h"
 #include "pdf_bin.h"
 
@@ -342,7 +343,8 @@ constexpr int PW_FLUSH = 256;                            // pairs between two fl
 // 16 KiB stage buffers and measured 1.40 ms on 2048-pixel rows, no better than the CTA-per-pair kernel.
 // STAGE (16-byte aligned flux; required by SPLIT): the NEXT pair streams into the stage buffer (ONE cp.async.bulk of 8 N
 // bytes issued by one lane, completion counted on the unit's mbarrier)
-// while the current one is transformed, so no warp waits out an HBM latency (1024-pixel rows: 0.99 -> 0.92 ms).
+// while the current one is transformed, so no warp waits out an HBM latency (1024-pixel rows: 0.99 -> 0.92 ms with
+// LDGSTS, 0.88 ms with the bulk copy).
 template <int N1, int N2, bool SPLIT, bool STAGE, int WARPS, int MINB>
 __global__ void __launch_bounds__(WARPS * 32, MINB) flux_power_warp_kernel(const PowArgs a)
 {
