@@ -395,7 +395,7 @@ __global__ void __launch_bounds__(FPDF_THREADS) flux_pdf_fused_kernel(const floa
     __syncthreads();
     unsigned int *mine = hist + threadIdx.x;
     const float f_lo = edges.f_lo, inv_width = edges.inv_width, eps = edges.eps, ome = edges.one_minus_eps;
-    auto bin = [&](float f) { mine[lya_pdf_bin(f, s_thr, n_bins, f_lo, inv_width, eps, ome) * FPDF_THREADS] += 1u; };
+    auto bin = [&](float f) { atomicAdd(mine + lya_pdf_bin(f, s_thr, n_bins, f_lo, inv_width, eps, ome) * FPDF_THREADS, 1u); };
     const size_t gtid = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     const size_t gsz  = (size_t)gridDim.x * blockDim.x;
     size_t head = ((16 - ((uintptr_t)tau & 15)) & 15) >> 2;

@@ -557,7 +557,7 @@ __global__ void __launch_bounds__(PDF_THREADS) flux_pdf_kernel(const float *__re
     __syncthreads();
     unsigned int *mine = hist + threadIdx.x;
     const float f_lo = edges.f_lo, inv_width = edges.inv_width, eps = edges.eps, ome = edges.one_minus_eps;
-    auto add = [&](float f) { mine[lya_pdf_bin(f, s_thr, n_bins, f_lo, inv_width, eps, ome) * PDF_THREADS] += 1u; };
+    auto add = [&](float f) { atomicAdd(mine + lya_pdf_bin(f, s_thr, n_bins, f_lo, inv_width, eps, ome) * PDF_THREADS, 1u); };
     const size_t gtid = (size_t)blockIdx.x * PDF_THREADS + threadIdx.x, gsz = (size_t)gridDim.x * PDF_THREADS;
     size_t head = ((16 - ((uintptr_t)flux & 15)) & 15) >> 2;
     if (head > n) head = n;
