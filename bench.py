@@ -363,7 +363,7 @@ def bench_ours(args) -> dict:
             "observe_rows": row(t_obs, b_obs, instrument="FWHM 224 km/s, 1.0375 A bins, S/N 5 (PAPER.md:130)", bins_per_row=int(nb)),
             "flux_pdf": row(t_pdf, 4 * nr_cells),
             "flux_with_pdf": row(t_fpdf, 8 * nr_cells, note="S5 and the flux PDF in one pass (replaces flux + flux_pdf: 12 B/pixel)"),
-            "flux_power_rows": row(t_pow, 4 * nr_cells, note="one warp per two-row complex FFT for 1024- / 2048-pixel rows (two 32-point register passes), Stockham radix-16/8 per CTA otherwise: bound by issue slots, FMA pipe and shared memory together, not by HBM")}
+            "flux_power_rows": row(t_pow, 4 * nr_cells, note="one warp per two-row complex FFT for rows of 256 ... 2048 pixels (two register passes, rows prefetched by cp.async.bulk), Stockham radix-16/8 per CTA otherwise: bound by issue slots, FMA pipe and shared memory together, not by HBM")}
         del noise, obs_out
         if w.cfg == 5:
             del flux_nr, Frows, tau_nr

@@ -289,7 +289,7 @@ lya_status lya_flux_with_pdf(lya_ctx *ctx, const float *tau, size_t n_pix, doubl
 
 /* 1D flux power spectrum: P(k_m) = (V/N^2) <|sum_i dF_i exp(-2 pi i m i/N)|^2> over the
  * rows, dF = F/mean_flux - 1, V = n_pix dv, k_m = 2 pi m / V [s/km], m = 0 .. n_pix/2.  n_pix must be a power
- * of two between 8 and 8192 (two rows per complex FFT: one warp per transform for 1024- and 2048-pixel rows, a Stockham
+ * of two between 8 and 8192 (two rows per complex FFT: one warp per transform for rows of 256 to 2048 pixels, a Stockham
  * radix-16/8/4 FFT per CTA in shared memory otherwise).  flux DEVICE [n_rows][n_pix];
  * power HOST, n_pix/2 + 1 doubles [km/s].  Synchronises the stream. */
 lya_status lya_flux_power_rows(lya_ctx *ctx, size_t n_rows, int32_t n_pix, double dv_kms, const float *flux,

@@ -15,7 +15,7 @@
 // in double registers across all the CTA's row pairs -- no final store, no read-out pass, two barriers per pair
 // instead of four -- and the host folds k and N - k once at the end.  Other sizes write the last pass to shared
 // memory and read the pairs (m, N - m) out (accumulated in double per CTA).
-// Rows of 1024 and 2048 pixels (configs 4 and 5) take flux_power_warp_kernel instead: ONE WARP per transform (32 x 32
+// Rows of 256 ... 2048 pixels (configs 2-5) take flux_power_warp_kernel / _short_kernel instead: ONE WARP per transform (32 x 32
 // in two register passes, 2048 as two such transforms by a radix-2 split shared by a team of two warps), the next row
 // pair prefetched by one cp.async.bulk, no CTA barrier in the loop: 1.30 -> 0.88 ms on 1024^3, 1.36 -> 0.97 ms on
 // 2048-pixel rows.
@@ -466,7 +466,137 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) flux_power_warp_kernel(const
         __syncwarp();                                    // the exchange buffer is free again
         if (++since == PW_FLUSH) { flush(); since = 0; }
     }
-    flush();
+    // last flush through the CTA: the warps' accumulators meet in shared memory first (in double, one warp after the
+    // other into the now idle exchange buffers: no atomics, a fixed order), so a CTA sends ONE double atomic per output
+    // instead of one per warp -- all warps of the grid finish together and their atomics to the same N addresses serialise
+    __syncthreads();
+    double *cta = reinterpret_cast<double *>(tw2 + (SPLIT ? NT : 0));
+    for (int i = threadIdx.x; i < N; i += WARPS * 32) cta[i] = 0.0;
+    __syncthreads();
+    for (int w = 0; w < WARPS; ++w) {
+        if (warp == w)
+#pragma unroll
+            for (int s = 0; s < S2; ++s)
+#pragma unroll
+                for (int t = 0; t < N2; ++t) cta[H * ((lane + 32 * s) + N1 * t) + h] += (double)acc[s][bitrev<N2>(t)];
+        __syncthreads();
+    }
+    for (int i = threadIdx.x; i < N; i += WARPS * 32) atomicAdd(mine + i, cta[i]);
+    lya_publish_last_cta(a.acc, a.n_acc, a.host, a.ticket, a.reps);
+}
+
+// The same design for SHORT rows (256 and 512 pixels = N1 x 32 with N1 = 8, 16): a warp step takes a BUNDLE of
+// PPW = 32 / N1 consecutive row pairs -- 1024 complex points again, one bulk copy of 8 KiB -- so that the second pass
+// still has a 32-point DFT for every lane: pass 1 runs PPW times (all lanes, an N1-point DFT each), pass 2 once, lane
+// q N1 + k1 transforming output residue k1 of pair q.  Lanes of different pairs add into the same accumulators at flush.
+template <int N1, bool STAGE, int WARPS, int MINB>
+__global__ void __launch_bounds__(WARPS * 32, MINB) flux_power_warp_short_kernel(const PowArgs a)
+{
+    constexpr int N = N1 * 32, PPW = 32 / N1, RPB = 2 * PPW, XS = 33;   // RPB: rows per bundle
+    static_assert(N1 == 8 || N1 == 16, "unsupported plan");
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    float2 *tw = reinterpret_cast<float2 *>(smem_raw);   // [N1][32]: W_N^(n2 k1)
+    float2 *ex = tw + N + warp * (32 * XS);              // row q N1 + k1, column n2
+    float *stg = reinterpret_cast<float *>(tw + N + WARPS * (32 * XS)) + warp * (RPB * N);
+    unsigned long long *mbar = reinterpret_cast<unsigned long long *>(
+        reinterpret_cast<float *>(tw + N + WARPS * (32 * XS)) + WARPS * (RPB * N)) + warp;
+    const bool issuer = STAGE && lane == 0;
+    auto stage = [&](size_t bundle) {                    // up to RPB consecutive rows: contiguous floats
+        const size_t row0 = bundle * RPB;
+        const unsigned rows = a.n_rows - row0 < (size_t)RPB ? (unsigned)(a.n_rows - row0) : (unsigned)RPB;
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        mbar_expect_tx(mbar, rows * N * (unsigned)sizeof(float));
+        bulk_g2s(stg, a.flux + row0 * N, rows * N * (unsigned)sizeof(float), mbar);
+    };
+    if (issuer) {
+        mbar_init(mbar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    for (int i = threadIdx.x; i < N; i += WARPS * 32) {
+        const int k1 = i >> 5, n2 = i & 31;
+        float sn, cs;
+        sincospif(2.0f * (float)((k1 * n2) & (N - 1)) / (float)N, &sn, &cs);
+        tw[i] = make_float2(cs, -sn);
+    }
+    __syncthreads();
+    float acc[32];
+#pragma unroll
+    for (int t = 0; t < 32; ++t) acc[t] = 0.0f;
+    double *mine = a.acc + (blockIdx.x % a.reps) * a.n_acc;
+    const int k1l = lane & (N1 - 1);                     // pass 2: this lane's output residue (of pair lane / N1)
+    auto flush = [&]() {
+#pragma unroll
+        for (int t = 0; t < 32; ++t) {                   // output k = k1 + N1 k2
+            atomicAdd(mine + k1l + N1 * t, (double)acc[bitrev<32>(t)]);
+            acc[bitrev<32>(t)] = 0.0f;
+        }
+    };
+    const size_t n_bundles = (a.n_rows + RPB - 1) / RPB, step = (size_t)gridDim.x * WARPS;
+    const float im = a.inv_mean;
+    int since = 0;
+    size_t bundle = (size_t)blockIdx.x * WARPS + warp;
+    if (issuer && bundle < n_bundles) stage(bundle);
+    unsigned phase = 0;
+    for (; bundle < n_bundles; bundle += step) {
+        const size_t row0 = bundle * RPB;
+        const float *base = STAGE ? stg : a.flux + row0 * N;
+        if (STAGE) {
+            mbar_wait(mbar, phase);
+            phase ^= 1u;
+        }
+        float2 v[PPW][N1];
+#pragma unroll
+        for (int q = 0; q < PPW; ++q) {
+            const bool has_a = row0 + 2 * q < a.n_rows, has_b = row0 + 2 * q + 1 < a.n_rows;
+            const float *ra = base + (2 * q) * N, *rb = ra + N;
+#pragma unroll
+            for (int t = 0; t < N1; ++t) {
+                const float xa = !has_a ? 0.0f : STAGE ? ra[lane + 32 * t] : __ldcs(ra + lane + 32 * t);
+                const float xb = !has_b ? 0.0f : STAGE ? rb[lane + 32 * t] : __ldcs(rb + lane + 32 * t);
+                v[q][t] = make_float2(has_a ? fmaf(xa, im, -1.0f) : 0.0f, has_b ? fmaf(xb, im, -1.0f) : 0.0f);
+            }
+        }
+        if (STAGE) {                                     // the stage buffer has been read: fetch the next bundle into it
+            __syncwarp();
+            if (issuer && bundle + step < n_bundles) stage(bundle + step);
+        }
+#pragma unroll
+        for (int q = 0; q < PPW; ++q) {                  // pass 1 of pair q: an N1-point DFT per lane (n2 = lane)
+            dft_regs64<N1, true>(v[q]);
+            float2 *e = ex + (q * N1) * XS + lane;
+            e[0] = v[q][0];
+#pragma unroll
+            for (int k1 = 1; k1 < N1; ++k1) e[k1 * XS] = cmul(v[q][bitrev<N1>(k1)], tw[k1 * 32 + lane]);
+        }
+        __syncwarp();
+        {                                                // pass 2: row `lane` of the exchange buffer
+            const float2 *row = ex + lane * XS;
+            float2 u[32];
+#pragma unroll
+            for (int t = 0; t < 32; ++t) u[t] = row[t];
+            dft_regs64<32, true>(u);
+#pragma unroll
+            for (int t = 0; t < 32; ++t) acc[t] = fmaf(u[t].x, u[t].x, fmaf(u[t].y, u[t].y, acc[t]));
+        }
+        __syncwarp();
+        if (++since == PW_FLUSH) { flush(); since = 0; }
+    }
+    __syncthreads();                                     // last flush through the CTA, as in flux_power_warp_kernel
+    double *cta = reinterpret_cast<double *>(tw + N);
+    for (int i = threadIdx.x; i < N; i += WARPS * 32) cta[i] = 0.0;
+    __syncthreads();
+    for (int w = 0; w < WARPS; ++w) {
+        if (warp == w)
+            for (int q = 0; q < PPW; ++q) {              // lanes of different pairs own the same outputs: one pair at a time
+                if ((lane / N1) == q)
+#pragma unroll
+                    for (int t = 0; t < 32; ++t) cta[k1l + N1 * t] += (double)acc[bitrev<32>(t)];
+                __syncwarp();
+            }
+        __syncthreads();
+    }
+    for (int i = threadIdx.x; i < N; i += WARPS * 32) atomicAdd(mine + i, cta[i]);
     lya_publish_last_cta(a.acc, a.n_acc, a.host, a.ticket, a.reps);
 }
 
@@ -516,6 +646,12 @@ extern "C" lya_status lya_flux_power_rows(lya_ctx *ctx, size_t n_rows, int32_t n
         warp_kernel = 4;
         threads = 4 * 32;
         smem = (size_t)1024 * sizeof(float2) + 4 * (size_t)32 * 33 * sizeof(float2) + (al16 ? 4 * 2 * (size_t)1024 * sizeof(float) : 0) + 4 * sizeof(unsigned long long);
+    } else if (n_pix == 256 || n_pix == 512) {             // bundles of 4 / 2 row pairs per warp step
+        kern = n_pix == 256 ? (al16 ? flux_power_warp_short_kernel<8, true, 4, 3> : flux_power_warp_short_kernel<8, false, 4, 3>)
+                            : (al16 ? flux_power_warp_short_kernel<16, true, 4, 3> : flux_power_warp_short_kernel<16, false, 4, 3>);
+        warp_kernel = 4 * (1024 / n_pix);                  // row pairs per CTA step
+        threads = 4 * 32;
+        smem = (size_t)n_pix * sizeof(float2) + 4 * (size_t)32 * 33 * sizeof(float2) + (al16 ? 4 * 2 * (size_t)1024 * sizeof(float) : 0) + 4 * sizeof(unsigned long long);
     } else if (n_pix == 2048 && al16) {                    // 6 teams of two warps, one CTA per SM
         kern = flux_power_warp_kernel<32, 32, true, true, 12, 1>;
         warp_kernel = 6;
