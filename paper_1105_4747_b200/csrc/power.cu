@@ -466,22 +466,24 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) flux_power_warp_kernel(const
         __syncwarp();                                    // the exchange buffer is free again
         if (++since == PW_FLUSH) { flush(); since = 0; }
     }
-    // last flush through the CTA: the warps' accumulators meet in shared memory first (in double, one warp after the
-    // other into the now idle exchange buffers: no atomics, a fixed order), so a CTA sends ONE double atomic per output
+    // last flush through the CTA: every warp parks its fp32 accumulators in its own (now idle) exchange buffer, then the
+    // CTA's threads add the warps' values per output in double, in a fixed order, and send ONE atomic per output and CTA
     // instead of one per warp -- all warps of the grid finish together and their atomics to the same N addresses serialise
     __syncthreads();
-    double *cta = reinterpret_cast<double *>(tw2 + (SPLIT ? NT : 0));
-    for (int i = threadIdx.x; i < N; i += WARPS * 32) cta[i] = 0.0;
+    float *park = reinterpret_cast<float *>(ex);         // [NT]: transform output k' = k1 + N1 k2
+#pragma unroll
+    for (int s = 0; s < S2; ++s)
+#pragma unroll
+        for (int t = 0; t < N2; ++t) park[(lane + 32 * s) + N1 * t] = acc[s][bitrev<N2>(t)];
     __syncthreads();
-    for (int w = 0; w < WARPS; ++w) {
-        if (warp == w)
+    const float *park0 = reinterpret_cast<const float *>(tw2 + (SPLIT ? NT : 0));
+    for (int o = threadIdx.x; o < N; o += WARPS * 32) {  // output o = H k' + h comes from the warps H u + h, u < UNITS
+        const float *src = park0 + (size_t)(o % H) * (2 * N1 * XS) + o / H;
+        double sum = 0.0;
 #pragma unroll
-            for (int s = 0; s < S2; ++s)
-#pragma unroll
-                for (int t = 0; t < N2; ++t) cta[H * ((lane + 32 * s) + N1 * t) + h] += (double)acc[s][bitrev<N2>(t)];
-        __syncthreads();
+        for (int u = 0; u < UNITS; ++u) sum += (double)src[(size_t)u * H * (2 * N1 * XS)];
+        atomicAdd(mine + o, sum);
     }
-    for (int i = threadIdx.x; i < N; i += WARPS * 32) atomicAdd(mine + i, cta[i]);
     lya_publish_last_cta(a.acc, a.n_acc, a.host, a.ticket, a.reps);
 }
 
@@ -583,20 +585,19 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) flux_power_warp_short_kernel
         if (++since == PW_FLUSH) { flush(); since = 0; }
     }
     __syncthreads();                                     // last flush through the CTA, as in flux_power_warp_kernel
-    double *cta = reinterpret_cast<double *>(tw + N);
-    for (int i = threadIdx.x; i < N; i += WARPS * 32) cta[i] = 0.0;
-    __syncthreads();
-    for (int w = 0; w < WARPS; ++w) {
-        if (warp == w)
-            for (int q = 0; q < PPW; ++q) {              // lanes of different pairs own the same outputs: one pair at a time
-                if ((lane / N1) == q)
+    float *park = reinterpret_cast<float *>(ex);         // [PPW][N]: lanes of different pairs own the same outputs
 #pragma unroll
-                    for (int t = 0; t < 32; ++t) cta[k1l + N1 * t] += (double)acc[bitrev<32>(t)];
-                __syncwarp();
-            }
-        __syncthreads();
+    for (int t = 0; t < 32; ++t) park[(lane / N1) * N + k1l + N1 * t] = acc[bitrev<32>(t)];
+    __syncthreads();
+    const float *park0 = reinterpret_cast<const float *>(tw + N);
+    for (int o = threadIdx.x; o < N; o += WARPS * 32) {
+        double sum = 0.0;
+#pragma unroll
+        for (int w = 0; w < WARPS; ++w)
+#pragma unroll
+            for (int q = 0; q < PPW; ++q) sum += (double)park0[(size_t)w * (2 * 32 * XS) + q * N + o];
+        atomicAdd(mine + o, sum);
     }
-    for (int i = threadIdx.x; i < N; i += WARPS * 32) atomicAdd(mine + i, cta[i]);
     lya_publish_last_cta(a.acc, a.n_acc, a.host, a.ticket, a.reps);
 }
 
